@@ -1,0 +1,393 @@
+"""Pins for the 2d part of the CPU oracle (oracle/sldg_oracle.c): characteristic tracing (eq. 14-15,
+PAPER.md:206-218), the coefficients C of eq. (18) and the update (17).
+
+The references below never call the oracle: golden values from SURVEY.md's independent 40-digit
+derivation, numpy-only exact quadrature over the whole upstream quadrilateral, a brute-force
+point-in-quadrilateral midpoint rule, the 1d brute-force projection (tensor product), closed-form rotation,
+scipy's ODE integrator, and invariants (column sums = mass conservation).  No GPU needed.
+"""
+import math
+import os
+
+import numpy as np
+import pytest
+
+import oracle
+from paper_2212_03036_b200 import inputs
+from paper_2212_03036_b200.inputs import GridSpec
+
+from test_oracle_1d import _brute_shift, _lag, _np_gl
+
+
+def _bilinear_quad(cf, xi, eta):
+    return ((1 - xi) * (1 - eta))[..., None] * cf[0] + (xi * (1 - eta))[..., None] * cf[1] \
+        + (xi * eta)[..., None] * cf[2] + ((1 - xi) * eta)[..., None] * cf[3]
+
+
+def _np_phistar_coef(o, node_feet):
+    """phi*_m = sum_ab c[ab, m] x^a y^b with phi*_m(foot_m') = delta, numpy solve."""
+    V = np.array([[fx ** a * fy ** b for b in range(o) for a in range(o)] for fx, fy in node_feet])
+    return np.linalg.solve(V, np.eye(o * o))  # [a + o*b][m]
+
+
+def _np_phistar(o, coef, x, y):
+    basis = np.stack([x ** a * y ** b for b in range(o) for a in range(o)], axis=-1)  # [..., ab]
+    return basis @ coef  # [..., m]
+
+
+def _np_phi(o, x, y):
+    """DG basis phi_k, k = p + o q, on the unit cell."""
+    xn, _ = _np_gl(o)
+    return np.stack([_lag(xn, k % o, x) * _lag(xn, k // o, y) for k in range(o * o)], axis=-1)
+
+
+# --------------------------------------------------------------------------------- worked example
+def _read_golden(golden_dir):
+    g = {"corner": {}, "nodefoot": {}, "area": {}, "C": {}, "unew": {}}
+    with open(os.path.join(golden_dir, "worked_example_2d.txt")) as fh:
+        for line in fh:
+            if line.startswith("#") or not line.strip():
+                continue
+            t = line.split()
+            if t[0] in ("corner", "nodefoot"):
+                g[t[0]][int(t[1])] = (float(t[2]), float(t[3]))
+            elif t[0] == "area":
+                g["area"][(int(t[1]), int(t[2]))] = float(t[3])
+            elif t[0] == "C":
+                g["C"][(int(t[1]), int(t[2]), int(t[3]), int(t[4]))] = float(t[5])
+            elif t[0] == "unew":
+                g["unew"][int(t[1])] = float(t[2])
+    return g
+
+
+def test_worked_example_golden(golden_dir):
+    """SURVEY.md 8(c)-2 worked example (independent 40-digit derivation of eq. 16-18)."""
+    g = _read_golden(golden_dir)
+    cf = np.array([g["corner"][k] for k in range(4)])
+    nf = np.array([g["nodefoot"][k] for k in range(4)])
+    xg, wg = _np_gl(2)
+    # the fixture's node feet are the bilinear image of the GL nodes
+    for q in range(2):
+        for p in range(2):
+            img = _bilinear_quad(cf, np.float64(xg[p]), np.float64(xg[q]))
+            assert np.abs(img - nf[p + 2 * q]).max() < 1e-15
+    unew = np.zeros(4)
+    for (r, s), area in g["area"].items():
+        C, rc = oracle.cell_coefficients(2, cf, nf, r, s)
+        assert rc == 1
+        assert abs(C.sum() - area) < 1e-15
+        unew += C.sum(axis=1)
+        for (rr, ss, k, m), val in g["C"].items():
+            if (rr, ss) == (r, s):
+                assert abs(C[m, k] - val) < 1e-15, (r, s, k, m, C[m, k], val)
+    W = np.array([wg[m % 2] * wg[m // 2] for m in range(4)])
+    for m in range(4):
+        assert abs(unew[m] / W[m] - g["unew"][m]) < 1e-14
+    # cells outside the bounding box give nothing
+    for (r, s) in [(-1, 0), (2, 0), (0, 2), (0, -1)]:
+        C, rc = oracle.cell_coefficients(2, cf, nf, r, s)
+        assert rc == 0 and np.all(C == 0.0)
+
+
+# ------------------------------------------------- exact whole-quadrilateral identity (numpy only)
+def _random_quad(rng, shift, deform=0.25):
+    base = np.array([(0.0, 0.0), (1.0, 0.0), (1.0, 1.0), (0.0, 1.0)])
+    return base + shift + rng.uniform(-deform, deform, size=(4, 2))
+
+
+@pytest.mark.parametrize("o", [2, 3])
+def test_sum_over_pieces_equals_integral_over_quad(o):
+    """For data u that is a global Q^{o-1} polynomial (exactly representable), sum_{rs,k} C^m_{rs,k} u_{rs,k}
+    = int_{A*} u phi*_m, which numpy evaluates exactly with a tensor Gauss rule on the bilinear map of
+    the quadrilateral -- no clipping involved.  A wrong clip, a dropped piece, a wrong orientation or a
+    transposed C index fails this at O(1e-2)."""
+    rng = np.random.default_rng(42 + o)
+    xn, _ = _np_gl(o)
+    xq, wq = _np_gl(8)
+    XI, ETA = np.meshgrid(xq, xq, indexing="ij")
+    WQ = wq[:, None] * wq[None, :]
+    for trial in range(12):
+        shift = rng.uniform(-1.6, 1.6, size=2)
+        cf = _random_quad(rng, shift)
+        nodes_ref = np.array([(xn[p], xn[q]) for q in range(o) for p in range(o)])
+        nf = _bilinear_quad(cf, nodes_ref[:, 0], nodes_ref[:, 1]) + rng.uniform(-0.02, 0.02, size=(o * o, 2))
+        pc = rng.standard_normal((o, o))  # u(x,y) = sum pc[a,b] x^a y^b
+        u = lambda x, y: sum(pc[a, b] * x ** a * y ** b for a in range(o) for b in range(o))
+        # reference: exact quadrature over the whole quadrilateral
+        P = _bilinear_quad(cf, XI, ETA)
+        dxi = (1 - ETA)[..., None] * (cf[1] - cf[0]) + ETA[..., None] * (cf[2] - cf[3])
+        deta = (1 - XI)[..., None] * (cf[3] - cf[0]) + XI[..., None] * (cf[2] - cf[1])
+        jac = dxi[..., 0] * deta[..., 1] - dxi[..., 1] * deta[..., 0]
+        coef = _np_phistar_coef(o, nf)
+        ps = _np_phistar(o, coef, P[..., 0], P[..., 1])  # [.., .., m]
+        ref = np.einsum("ij,ij,ijm->m", WQ * jac, u(P[..., 0], P[..., 1]), ps)
+        # oracle: sum over all candidate source cells
+        got = np.zeros(o * o)
+        r0, r1 = int(np.floor(cf[:, 0].min())), int(np.ceil(cf[:, 0].max()))
+        s0, s1 = int(np.floor(cf[:, 1].min())), int(np.ceil(cf[:, 1].max()))
+        area = 0.0
+        for s in range(s0 - 1, s1 + 1):
+            for r in range(r0 - 1, r1 + 1):
+                C, rc = oracle.cell_coefficients(o, cf, nf, r, s)
+                unodes = np.array([u(r + xn[k % o], s + xn[k // o]) for k in range(o * o)])
+                got += C @ unodes
+                area += C.sum()
+        shoelace = 0.5 * sum(cf[k, 0] * cf[(k + 1) % 4, 1] - cf[(k + 1) % 4, 0] * cf[k, 1] for k in range(4))
+        assert abs(area - shoelace) < 1e-13
+        assert np.abs(got - ref).max() < 2e-12 * max(1.0, np.abs(ref).max())
+
+
+@pytest.mark.parametrize("o", [2, 3])
+def test_single_piece_matches_bruteforce_point_in_quad(o):
+    """Brute force (north_star): midpoint rule on a fine grid of one source cell with a
+    point-in-quadrilateral test.  Pins each individual block C_{rs}, not only their sum."""
+    rng = np.random.default_rng(7 + o)
+    cf = _random_quad(rng, np.array([0.35, -0.4]), deform=0.2)
+    xn, _ = _np_gl(o)
+    nodes_ref = np.array([(xn[p], xn[q]) for q in range(o) for p in range(o)])
+    nf = _bilinear_quad(cf, nodes_ref[:, 0], nodes_ref[:, 1])
+    coef = _np_phistar_coef(o, nf)
+    M = 1200
+    t = (np.arange(M) + 0.5) / M
+    X, Y = np.meshgrid(t, t, indexing="ij")
+    nonempty = 0
+    for s in (-1, 0, 1):
+        for r in (0, 1):
+            gx, gy = X + r, Y + s
+            inside = np.ones_like(gx, dtype=bool)
+            for k in range(4):
+                p0, p1 = cf[k], cf[(k + 1) % 4]
+                inside &= ((p1[0] - p0[0]) * (gy - p0[1]) - (p1[1] - p0[1]) * (gx - p0[0])) >= 0
+            phi = _np_phi(o, X, Y)                      # source basis in local coordinates
+            ps = _np_phistar(o, coef, gx, gy)           # adjoint polynomial in the target frame
+            ref = np.einsum("ij,ijm,ijk->mk", inside / (M * M), ps, phi)
+            C, rc = oracle.cell_coefficients(o, cf, nf, r, s)
+            if inside.any():
+                nonempty += 1
+            assert np.abs(C - ref).max() < 3e-3 * max(np.abs(ref).max(), 0.05), (r, s)
+    assert nonempty >= 4
+
+
+# ------------------------------------------------------------------------------------- tracing
+def test_trace_rotation_closed_form():
+    """u = (-y, x) is reproduced exactly by bilinear interpolation, so eq. (14) gives X - tau J X and
+    the midpoint form of eq. (15) gives (I - tau J + tau^2 J^2 / 2) X, with J = [[0,-1],[1,0]]."""
+    spec = inputs.bumps_grid(16, 1, 2)
+    a, b = inputs.rotation_velocity(spec)
+    hx, hy = spec.h[0], spec.h[1]
+    J = np.array([[0.0, -1.0], [1.0, 0.0]])
+    tau = 0.11
+    for (i, j, xi, eta) in [(3, 4, 0.0, 0.0), (3, 4, 1.0, 1.0), (10, 2, 0.2113, 0.7887), (0, 15, 0.5, 0.1)]:
+        X = np.array([spec.lo[0] + (i + xi) * hx, spec.lo[1] + (j + eta) * hy])
+        for order, M in ((1, np.eye(2) - tau * J), (2, np.eye(2) - tau * J + 0.5 * tau ** 2 * J @ J)):
+            foot = oracle.trace(spec, a[0], b[0], i, j, xi, eta, tau, order, 0)
+            phys = np.array([spec.lo[0] + (i + foot[0]) * hx, spec.lo[1] + (j + foot[1]) * hy])
+            assert np.abs(phys - M @ X).max() < 1e-14
+
+
+def test_trace_order2_is_third_order_accurate_locally():
+    """Against scipy's integration of the frozen piecewise-bilinear swirl field: the midpoint foot has
+    O(tau^3) local error (ratio ~8 when tau halves), the Euler foot O(tau^2) (ratio ~4)."""
+    from scipy.integrate import solve_ivp
+    from scipy.interpolate import RegularGridInterpolator
+
+    spec = inputs.bumps_grid(32, 1, 2)
+    a, b = inputs.swirl_velocity(spec, 0.0)
+    xv, yv = spec.vertex_coords(0), spec.vertex_coords(1)
+    ia = RegularGridInterpolator((yv, xv), a[0], method="linear", bounds_error=False, fill_value=None)
+    ib = RegularGridInterpolator((yv, xv), b[0], method="linear", bounds_error=False, fill_value=None)
+    rhs = lambda t, X: [-ia([[X[1], X[0]]])[0], -ib([[X[1], X[0]]])[0]]  # backward in time
+    hx, hy = spec.h[0], spec.h[1]
+    i, j, xi, eta = 20, 9, 0.31, 0.64
+    X0 = [spec.lo[0] + (i + xi) * hx, spec.lo[1] + (j + eta) * hy]
+    errs = {1: [], 2: []}
+    for tau in (0.08, 0.04):
+        sol = solve_ivp(rhs, (0.0, tau), X0, rtol=1e-12, atol=1e-14, max_step=tau / 64)
+        exact = sol.y[:, -1]
+        for order in (1, 2):
+            foot = oracle.trace(spec, a[0], b[0], i, j, xi, eta, tau, order, 1)
+            phys = np.array([spec.lo[0] + (i + foot[0]) * hx, spec.lo[1] + (j + foot[1]) * hy])
+            errs[order].append(np.abs(phys - exact).max())
+    assert 2.5 < errs[1][0] / errs[1][1] < 6.0
+    assert errs[2][0] / errs[2][1] > 5.0
+    assert errs[2][1] < 0.1 * errs[1][1]
+
+
+def test_trace_periodic_images_agree():
+    """With a bitwise-periodic field and vel_periodic=1 the two periodic images of a boundary vertex get
+    the same foot (relative to the vertex), for both trace orders -- the upstream mesh tiles."""
+    spec = inputs.bumps_grid(16, 1, 2)
+    a, b = inputs.swirl_velocity(spec, 0.3)
+    rng = np.random.default_rng(0)
+    # perturb to something non-symmetric but still bitwise periodic
+    pa = rng.standard_normal((16, 16)) * 0.3
+    a[0, :16, :16] += pa
+    b[0, :16, :16] -= pa.T
+    for u in (a[0], b[0]):
+        u[16, :] = u[0, :]
+        u[:, 16] = u[:, 0]
+    tau = 0.35
+    for order in (1, 2):
+        for j in range(16):
+            left = oracle.trace(spec, a[0], b[0], 0, j, 0.0, 0.0, tau, order, 1)
+            right = oracle.trace(spec, a[0], b[0], 15, j, 1.0, 0.0, tau, order, 1)
+            assert np.abs(left - (right - np.array([1.0, 0.0]))).max() < 3e-16
+            bot = oracle.trace(spec, a[0], b[0], j, 0, 0.0, 0.0, tau, order, 1)
+            top = oracle.trace(spec, a[0], b[0], j, 15, 0.0, 1.0, tau, order, 1)
+            assert np.abs(bot - (top - np.array([0.0, 1.0]))).max() < 3e-16
+
+
+# ----------------------------------------------------------------------------- plane geometry
+def _periodic_random_velocity(spec, seed, amp):
+    nx, ny = spec.n[0], spec.n[1]
+    rng = np.random.default_rng(seed)
+    xv = np.arange(nx) / nx
+    yv = np.arange(ny) / ny
+    X, Y = np.meshgrid(xv, yv, indexing="xy")
+    a = np.zeros((ny, nx))
+    b = np.zeros((ny, nx))
+    for _ in range(4):
+        kx, ky = rng.integers(0, 3, size=2)
+        a += rng.uniform(-1, 1) * np.cos(2 * np.pi * (kx * X + ky * Y) + rng.uniform(0, 6.28))
+        b += rng.uniform(-1, 1) * np.cos(2 * np.pi * (kx * X + ky * Y) + rng.uniform(0, 6.28))
+    A = np.empty((ny + 1, nx + 1))
+    B = np.empty_like(A)
+    for dst, src in ((A, a), (B, b)):
+        dst[:ny, :nx] = src * amp / max(np.abs(a).max(), np.abs(b).max())
+        dst[ny, :nx] = dst[0, :nx]
+        dst[:, nx] = dst[:, 0]
+    return A, B
+
+
+@pytest.mark.parametrize("o", [2, 3])
+@pytest.mark.parametrize("trace_order", [1, 2])
+def test_column_sum_identity_is_mass_conservation(o, trace_order):
+    """sum_{ij} sum_m C^{ij,m}_{rs,k} = W_k = w_p w_q for every source DOF (SURVEY.md 8(c)-2 pin (i)):
+    sum_m phi*_m == 1 and the upstream quadrilaterals tile the plane.  Pins tracing consistency between
+    neighbouring cells, clipping and integration with no data at all."""
+    spec = GridSpec(n=(9, 7, 1, 1), order=(o, o, 1, 1), lo=(0.0, 0.0, 0, 0), hi=(1.8, 2.1, 1, 1))
+    nx, ny = spec.n[0], spec.n[1]
+    a, b = _periodic_random_velocity(spec, 5, 1.0)
+    tau = 0.9 * min(spec.h[0], spec.h[1])  # displacements up to 0.9 cells
+    offs, er, es, eC = oracle.xy_plane_geometry(spec, a, b, tau, trace_order, 1)
+    _, wg = _np_gl(o)
+    col = np.zeros((ny, nx, o * o))
+    for e in range(er.size):
+        col[es[e] % ny, er[e] % nx] += eC[e].sum(axis=0)
+    W = np.array([wg[k % o] * wg[k // o] for k in range(o * o)])
+    assert np.abs(col - W).max() < 2e-14
+    # row sums with u == 1: new nodal values times W sum to the upstream area of each cell
+    for t in range(nx * ny):
+        assert eC[offs[t]:offs[t + 1]].sum() > 0.0
+
+
+@pytest.mark.parametrize("o", [2, 3])
+def test_zero_velocity_is_identity(o):
+    spec = GridSpec(n=(5, 4, 2, 3), order=(o, o, 1, 2), lo=(0, 0, 0, 0), hi=(1, 1, 1, 1))
+    rng = np.random.default_rng(1)
+    f = rng.standard_normal(spec.shape)
+    a = np.zeros((spec.shape[0], 5, 6))
+    out = oracle.advect_xy(spec, f, a, a, 0.7, 2, 1)
+    assert np.abs(out - f).max() < 1e-14 * o * o * np.abs(f).max()
+
+
+@pytest.mark.parametrize("o", [2, 3])
+@pytest.mark.parametrize("trace_order", [1, 2])
+def test_constant_velocity_is_tensor_product_of_1d_steps(o, trace_order):
+    """north_star pin: a constant-velocity 2d step equals the tensor product of two 1d steps; the 1d
+    reference is the brute-force projection of test_oracle_1d (not the oracle)."""
+    spec = GridSpec(n=(6, 5, 1, 2), order=(o, o, 1, 1), lo=(0.0, -1.0, 0, 0), hi=(3.0, 1.5, 1, 1))
+    Nz, Nv, Ny, Nx = spec.shape
+    rng = np.random.default_rng(9)
+    f = rng.standard_normal(spec.shape)
+    for (ca, cb) in [(0.37, -0.52), (-1.8, 2.3), (0.0, 0.6), (1.0, -2.0)]:  # Courant numbers
+        tau = 0.25
+        a = np.full((Nz, spec.n[1] + 1, spec.n[0] + 1), ca * spec.h[0] / tau)
+        b = np.full_like(a, cb * spec.h[1] / tau)
+        got = oracle.advect_xy(spec, f, a, b, tau, trace_order, 0)
+        ref = np.empty_like(f)
+        for z in range(Nz):
+            for v in range(Nv):
+                tmp = np.stack([_brute_shift(f[z, v, Y, :].copy(), o, ca) for Y in range(Ny)], axis=0)
+                ref[z, v] = np.stack([_brute_shift(tmp[:, X].copy(), o, cb) for X in range(Nx)], axis=1)
+        assert np.abs(got - ref).max() < 5e-12 * np.abs(ref).max()
+
+
+def test_velocity_and_data_planes_are_paired_per_z():
+    """Geometry is per z-node and reused for every v (Algorithm 3): plane z uses a[z], b[z]."""
+    spec = GridSpec(n=(4, 4, 2, 2), order=(2, 2, 2, 1), lo=(0, 0, 0, 0), hi=(1, 1, 1, 1))
+    Nz, Nv, Ny, Nx = spec.shape
+    rng = np.random.default_rng(2)
+    f = rng.standard_normal(spec.shape)
+    a = np.zeros((Nz, 5, 5))
+    b = np.zeros_like(a)
+    shifts = [0, 1, -1, 2]
+    for z in range(Nz):
+        a[z] = shifts[z] * spec.h[0]  # integer Courant numbers in x, tau = 1
+    out = oracle.advect_xy(spec, f, a, b, 1.0, 1, 1)
+    for z in range(Nz):
+        ref = np.roll(f[z].reshape(Nv, Ny, 4, 2), shifts[z], axis=2).reshape(Nv, Ny, Nx)
+        assert np.abs(out[z] - ref).max() < 1e-14
+
+
+# ----------------------------------------------------------------- rotation / swirl (accuracy only)
+def _rotation_error(ncell, o, steps):
+    spec = inputs.bumps_grid(ncell, 2, o)
+    f0 = inputs.bumps_initial_f(spec, seed=1)
+    # widen the bumps so that coarse grids resolve them: use sigma from the generator but the test
+    # only compares errors between resolutions
+    a, b = inputs.rotation_velocity(spec)
+    f = f0.copy()
+    m0 = oracle.mass(spec, f)
+    tau = 2 * math.pi / steps
+    for _ in range(steps):
+        f = oracle.advect_xy(spec, f, a, b, tau, 2, 0)
+    return np.abs(f - f0).max() / np.abs(f0).max(), abs(oracle.mass(spec, f) - m0) / abs(m0)
+
+
+def test_rotation_full_period_returns_to_start_with_discretisation_accuracy():
+    """SURVEY.md 8(c)-2 pin (vi): a tolerance test -- refining mesh and time step together, the error
+    after one full period shrinks at about second order.  u = (-y, x) is not periodic on
+    the box, so the upstream mesh does not tile across the wrap seam (reading A15): mass is conserved
+    only up to what the scheme's ripples carry to the seam (<= 1e-11 here); machine-precision mass
+    conservation is pinned by the column-sum identity and the periodic swirl test instead."""
+    e1, m1 = _rotation_error(32, 2, 40)
+    e2, m2 = _rotation_error(64, 2, 80)
+    assert m1 < 1e-10 and m2 < 1e-11
+    assert e2 < 0.2
+    assert e1 / e2 > 2.3
+    e3, _ = _rotation_error(32, 3, 40)
+    assert e3 < 0.5 * e1  # one more node per cell is markedly more accurate on the same mesh
+
+
+def test_swirl_there_and_back_conserves_mass_and_returns():
+    """Swirling deformation (PAPER.md:297-303 shape, config 1 flow): at t = T the exact solution is the
+    initial state; mass error is at machine precision."""
+    spec = inputs.bumps_grid(64, 2, 2)
+    f0 = inputs.bumps_initial_f(spec, seed=1)
+    f = f0.copy()
+    m0 = oracle.mass(spec, f)
+    steps, T = 30, 1.5
+    tau = T / steps
+    for n in range(steps):
+        a, b = inputs.swirl_velocity(spec, (n + 0.5) * tau, period=T)
+        f = oracle.advect_xy(spec, f, a, b, tau, 2, 1)
+        assert abs(oracle.mass(spec, f) - m0) < 1e-13 * abs(m0)
+    assert np.abs(f - f0).max() < 0.25 * np.abs(f0).max()
+
+
+def test_strang_step_composition():
+    """a6: z(dt/2) v(dt/2) xy(dt) v(dt/2) z(dt/2) (Algorithm 1 steps 3,4,6,7,8)."""
+    spec = inputs.itg_grid(6, 6, 4, 6, 2)
+    f = inputs.itg_initial_f(spec)
+    dt = 2.0
+    a, b, Ez, _ = inputs.itg_fields(spec, dt, 0.8)
+    ref = oracle.advect_z(spec, f, dt / 2)
+    ref = oracle.advect_v(spec, ref, Ez, dt / 2)
+    ref = oracle.advect_xy(spec, ref, a, b, dt, 2, 1)
+    ref = oracle.advect_v(spec, ref, Ez, dt / 2)
+    ref = oracle.advect_z(spec, ref, dt / 2)
+    m0 = oracle.mass(spec, f)
+    got = oracle.strang_step(spec, f.copy(), Ez, a, b, dt, 2, 1)
+    assert np.array_equal(got, ref)
+    assert abs(oracle.mass(spec, got) - m0) < 1e-14 * m0
