@@ -1,0 +1,140 @@
+/*
+ * sldg.h -- C-ABI boundary of libsldg: the data-parallel hot path of the drift-kinetic solver of
+ * arxiv 2212.03036 (Einkemmer & Moriggl), i.e. the split semi-Lagrangian discontinuous Galerkin (SLDG)
+ * advection of the 4d distribution f(x,y,z,v) in fp64, as hand-written CUDA for sm_100a (B200).
+ * Citations are PAPER.md:LINE (the paper's text) and SURVEY.md section 8 (the readings taken where the
+ * paper is silent; they are listed in DESIGN.md).
+ *
+ * Conventions
+ *   axes            0:x 1:y 2:z 3:v.  n[d] cells, order[d] Gauss-Legendre nodes per cell,
+ *                   N[d] = n[d]*order[d] degrees of freedom; DOF index = cell*order + node; node
+ *                   coordinate = lo + (cell + xi_node) * h,  h = (hi-lo)/n.  DOFs are point values.
+ *   canonical f     double [Nz][Nv][Ny][Nx]   (x fastest)        -- the layout of import/export
+ *   Ez              double [Nz][Ny][Nx]       speed of the v-advection, Ez = -d(phi)/dz (eq. 5)
+ *   a, b            double [Nz][ny+1][nx+1]   poloidal velocity at the cell vertices (eq. 12)
+ *   rho             double [Nz][Ny][Nx]
+ *   boundary        f is periodic along all four axes (PAPER.md:55 for theta, z, v; SURVEY.md 8(c) A15
+ *                   for the Cartesian x, y).
+ *   memory          every pointer named *_dev is DEVICE memory, *_host is HOST memory.  All device buffers
+ *                   are allocated by the caller and BORROWED: the context owns no device memory except
+ *                   what lives inside `workspace`.  f_a, f_b, workspace must stay valid until
+ *                   sldg_destroy and must be 256-byte aligned.
+ *   state           the library keeps f in an INTERNAL layout (v fastest) inside f_a/f_b and
+ *                   ping-pongs between them; sldg_import_state / sldg_export_state convert.
+ *   stream          every call enqueues on the cudaStream_t given at sldg_create and returns without
+ *                   synchronising, unless stated otherwise.
+ *   errors          return value 0 = success, negative = SLDG_E* below.  Errors detected on the device
+ *                   (geometry) are sticky and reported by sldg_check.  There is no CPU fallback: without
+ *                   a CUDA device every compute call returns SLDG_ECUDA.
+ */
+#ifndef SLDG_H
+#define SLDG_H
+
+#include <stddef.h>
+#include <stdint.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+typedef struct sldg_ctx sldg_ctx; /* opaque */
+
+typedef struct {
+    int32_t n[4];        /* cells in x, y, z, v                                                     */
+    int32_t order[4];    /* nodes per cell per axis, each 1, 2 or 3; order[0] == order[1]
+                            (per-axis degree is in the paper: PAPER.md:396; the paper runs 2)       */
+    double lo[4], hi[4]; /* box                                                                     */
+    int32_t max_stencil; /* largest block of source cells one upstream cell may touch per direction;
+                            must be 3 (the paper's 3x3 assumption)                    */
+    int32_t layout;      /* internal line order: 0 = library default, 1 = z,y,x  2 = y,x,z  3 = y,z,x
+                            (v is always fastest; a tuning knob, results do not depend on it)       */
+} sldg_params;
+
+enum {
+    SLDG_OK = 0,
+    SLDG_EINVAL = -1,   /* bad parameter, null pointer, misaligned or too small buffer               */
+    SLDG_ECUDA = -2,    /* CUDA runtime / launch error, or no device                                  */
+    SLDG_ESTENCIL = -3, /* an upstream cell's bounding box exceeds max_stencil   */
+    SLDG_EGEOM = -4     /* upstream cell not convex / not positively oriented (crossed characteristics,
+                           PAPER.md:190) or a singular Vandermonde system              */
+};
+
+/* Sizes (bytes) of each ping-pong state buffer and of the workspace for these parameters; 0 on
+ * invalid parameters.  Host-only, no device needed. */
+size_t sldg_state_bytes(const sldg_params *p);
+size_t sldg_workspace_bytes(const sldg_params *p);
+
+/* Create a context.  f_a_dev / f_b_dev: the two state buffers (sldg_state_bytes each); workspace_dev:
+ * sldg_workspace_bytes; cuda_stream: a cudaStream_t (NULL = legacy default stream).  The state is
+ * undefined until sldg_import_state.  Fields default to Ez = 0, a = b = 0, trace order 2. */
+int sldg_create(const sldg_params *p, double *f_a_dev, double *f_b_dev, void *workspace_dev,
+                size_t workspace_bytes, void *cuda_stream, sldg_ctx **out);
+int sldg_destroy(sldg_ctx *ctx);
+
+/* State in/out, canonical layout [Nz][Nv][Ny][Nx].  The *_dev calls are asynchronous device-to-device
+ * transposes.  The *_host calls copy through the idle ping-pong buffer and synchronise the stream. */
+int sldg_import_state(sldg_ctx *ctx, const double *f_canonical_dev);
+int sldg_export_state(sldg_ctx *ctx, double *f_canonical_dev);
+int sldg_import_state_host(sldg_ctx *ctx, const double *f_canonical_host);
+int sldg_export_state_host(sldg_ctx *ctx, double *f_canonical_host);
+/* Which of f_a / f_b currently holds the state (internal layout). */
+double *sldg_current(sldg_ctx *ctx);
+
+/* Fields; copied into the workspace, the caller's buffers are free afterwards.
+ * sldg_set_vxy: `periodic` != 0 declares a, b bitwise periodic (a[.., ny, :] == a[.., 0, :] and
+ * a[.., :, nx] == a[.., :, 0]); the half-step point of the second-order tracing (eq. 15) is
+ * then looked up modulo the box so that the upstream mesh tiles across the periodic seam; with
+ * periodic == 0 the cell index is clamped to the box (reading A15). */
+int sldg_set_Ez(sldg_ctx *ctx, const double *Ez_dev);
+int sldg_set_vxy(sldg_ctx *ctx, const double *a_dev, const double *b_dev, int periodic);
+
+/* 1d SLDG sweep along z with speed v (eq. 4; eq. 11): for each v node q,
+ * delta = v_q tau / h_z, s = floor(-delta), alpha = -delta - s, and for every z cell i, node j
+ *   f'[i,j] = sum_m A_jm(alpha) f[(i+s) mod nz, m] + B_jm(alpha) f[(i+s+1) mod nz, m]
+ * with A, B the overlap matrices of eq. (10).  Any tau, any Courant number. */
+int sldg_advect_z(sldg_ctx *ctx, double tau);
+/* 1d SLDG sweep along v with speed Ez(x,y,z) (eq. 5), periodic in v. */
+int sldg_advect_v(sldg_ctx *ctx, double tau);
+/* 2d SLDG step in the poloidal plane (eq. 6, 12-18; Algorithm 3):
+ * per z node the upstream quadrilaterals, adjoint polynomials and Green's-theorem integrals C (18) are
+ * computed once and applied to every v node (17).  trace_order 1: eq. (14); 2: eq. (15) as explicit
+ * midpoint with the one field set by sldg_set_vxy.  Geometry failures are reported
+ * by sldg_check (SLDG_ESTENCIL, SLDG_EGEOM); the state is then unspecified. */
+int sldg_advect_xy(sldg_ctx *ctx, double tau, int trace_order);
+/* rho[z,y,x] = int f dv = h_v sum_{l,q} w_q f[z,(l,q),y,x].  rho_dev: [Nz][Ny][Nx]. */
+int sldg_charge_density(sldg_ctx *ctx, double *rho_dev);
+/* Total mass sum f w_x w_y w_z w_v h_x h_y h_z h_v into one device double. */
+int sldg_mass(sldg_ctx *ctx, double *mass_dev);
+/* One Strang step with the fields currently set (Algorithm 1 steps 3,4,6,7,8; the
+ * source terms vanish for the Cartesian full-f formulation):
+ *   advect_z(dt/2), advect_v(dt/2), advect_xy(dt), advect_v(dt/2), advect_z(dt/2). */
+int sldg_strang_step(sldg_ctx *ctx, double dt);
+int sldg_set_trace_order(sldg_ctx *ctx, int trace_order); /* used by sldg_strang_step; default 2 */
+
+/* The same step driven from HOST buffers (what a host-side field solver sees): copies Ez, a, b from
+ * host to device, runs sldg_strang_step, then the charge density and the mass, copies rho and mass back
+ * to the host, and synchronises the stream.  Pinned host buffers make the copies asynchronous.
+ * Any of Ez_host / a_host+b_host / rho_host / mass_host may be NULL to skip that transfer. */
+int sldg_strang_step_host(sldg_ctx *ctx, double dt, const double *Ez_host, const double *a_host,
+                          const double *b_host, int periodic, double *rho_host, double *mass_host);
+
+/* Synchronises the stream and returns the sticky device error word (0, SLDG_ESTENCIL, SLDG_EGEOM) or
+ * SLDG_ECUDA; clears it. */
+int sldg_check(sldg_ctx *ctx);
+/* Device times (CUDA events on the context's stream) of the last sldg_strang_step, in ms:
+ * ms[0] z  ms[1] v  ms[2] xy geometry  ms[3] xy apply  ms[4] v  ms[5] z  ms[6] (unused, 0)  ms[7] total.
+ * After a single sldg_advect_* call only that entry (and ms[7]) is set.  Synchronises. */
+int sldg_last_timing_ms(sldg_ctx *ctx, float ms[8]);
+/* Number of kernels the library launched on behalf of this context since creation. */
+long long sldg_launch_count(sldg_ctx *ctx);
+/* Debug / test access to the geometry of the last sldg_advect_xy: for z node `z` copies, per target
+ * cell t = j*nx + i, anchor[2t..2t+1] = wrapped source cell of slot (0,0), mask[t] = bitmask over the
+ * 3x3 slots (bit dx + 3 dy), and W[t][slot][m][k] = C^{ij,m}_{rs,k} / W_m (dense, 9*o^4 doubles per cell,
+ * entries of empty slots are unspecified).  Device buffers; asynchronous. */
+int sldg_debug_geometry(sldg_ctx *ctx, int z, int32_t *anchor_dev, int32_t *mask_dev, double *W_dev);
+const char *sldg_strerror(int code);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* SLDG_H */

@@ -1,0 +1,239 @@
+"""ctypes binding of libsldg (include/sldg.h): same names, argument marshalling only.
+
+Every step of the hot path runs inside the CUDA library.  `Sldg` is a small convenience wrapper that
+owns the torch tensors backing the state / workspace and forwards to the C-ABI entry points.
+"""
+from __future__ import annotations
+
+import ctypes as C
+import os
+
+from . import build as _build
+
+_HERE = os.path.dirname(os.path.abspath(__file__))
+_lib = None
+
+SLDG_OK, SLDG_EINVAL, SLDG_ECUDA, SLDG_ESTENCIL, SLDG_EGEOM = 0, -1, -2, -3, -4
+
+EXPORTS = [
+    "sldg_state_bytes", "sldg_workspace_bytes", "sldg_create", "sldg_destroy", "sldg_import_state",
+    "sldg_export_state", "sldg_import_state_host", "sldg_export_state_host", "sldg_current",
+    "sldg_set_Ez", "sldg_set_vxy", "sldg_advect_z", "sldg_advect_v", "sldg_advect_xy",
+    "sldg_charge_density", "sldg_mass", "sldg_strang_step", "sldg_set_trace_order",
+    "sldg_strang_step_host", "sldg_check", "sldg_last_timing_ms", "sldg_launch_count",
+    "sldg_debug_geometry", "sldg_strerror",
+]
+
+
+class SldgParams(C.Structure):
+    _fields_ = [("n", C.c_int32 * 4), ("order", C.c_int32 * 4), ("lo", C.c_double * 4),
+                ("hi", C.c_double * 4), ("max_stencil", C.c_int32), ("layout", C.c_int32)]
+
+
+class SldgError(RuntimeError):
+    def __init__(self, code, what):
+        self.code = code
+        msg = load_library().sldg_strerror(code).decode()
+        super().__init__(f"{what}: {msg} ({code})")
+
+
+def library_path():
+    return os.path.join(_HERE, "libsldg.so")
+
+
+def load_library():
+    """Load libsldg.so (building it with nvcc if the sources are newer).  Raises if unavailable."""
+    global _lib
+    if _lib is not None:
+        return _lib
+    path = library_path()
+    if not os.path.exists(path) or os.environ.get("SLDG_REBUILD"):
+        _build.build()
+    if not os.path.exists(path):
+        raise RuntimeError("libsldg.so is missing and could not be built (nvcc required); "
+                           "there is no CPU fallback")
+    L = C.CDLL(path)
+    vp, dp, ip = C.c_void_p, C.c_void_p, C.c_void_p
+    PP = C.POINTER(SldgParams)
+    L.sldg_state_bytes.argtypes = [PP]
+    L.sldg_state_bytes.restype = C.c_size_t
+    L.sldg_workspace_bytes.argtypes = [PP]
+    L.sldg_workspace_bytes.restype = C.c_size_t
+    L.sldg_create.argtypes = [PP, dp, dp, vp, C.c_size_t, vp, C.POINTER(vp)]
+    L.sldg_destroy.argtypes = [vp]
+    for name in ("sldg_import_state", "sldg_export_state", "sldg_import_state_host",
+                 "sldg_export_state_host", "sldg_set_Ez", "sldg_charge_density", "sldg_mass"):
+        getattr(L, name).argtypes = [vp, dp]
+    L.sldg_current.argtypes = [vp]
+    L.sldg_current.restype = C.c_void_p
+    L.sldg_set_vxy.argtypes = [vp, dp, dp, C.c_int]
+    L.sldg_advect_z.argtypes = [vp, C.c_double]
+    L.sldg_advect_v.argtypes = [vp, C.c_double]
+    L.sldg_advect_xy.argtypes = [vp, C.c_double, C.c_int]
+    L.sldg_strang_step.argtypes = [vp, C.c_double]
+    L.sldg_set_trace_order.argtypes = [vp, C.c_int]
+    L.sldg_strang_step_host.argtypes = [vp, C.c_double, dp, dp, dp, C.c_int, dp, dp]
+    L.sldg_check.argtypes = [vp]
+    L.sldg_last_timing_ms.argtypes = [vp, C.POINTER(C.c_float * 8)]
+    L.sldg_launch_count.argtypes = [vp]
+    L.sldg_launch_count.restype = C.c_longlong
+    L.sldg_debug_geometry.argtypes = [vp, C.c_int, ip, ip, dp]
+    L.sldg_strerror.argtypes = [C.c_int]
+    L.sldg_strerror.restype = C.c_char_p
+    _lib = L
+    return L
+
+
+def make_params(spec, layout=0, max_stencil=3):
+    p = SldgParams()
+    for d in range(4):
+        p.n[d] = int(spec.n[d])
+        p.order[d] = int(spec.order[d])
+        p.lo[d] = float(spec.lo[d])
+        p.hi[d] = float(spec.hi[d])
+    p.max_stencil = max_stencil
+    p.layout = layout
+    return p
+
+
+class Sldg:
+    """One SLDG context on the current CUDA device.  Tensors are torch CUDA tensors (fp64)."""
+
+    def __init__(self, spec, device="cuda", layout=0, stream=None):
+        import torch
+
+        if not torch.cuda.is_available():
+            raise RuntimeError("libsldg needs a CUDA device (sm_100a); there is no CPU fallback")
+        self.torch = torch
+        self.L = load_library()
+        self.spec = spec
+        self.device = torch.device(device)
+        self.params = make_params(spec, layout)
+        sb = self.L.sldg_state_bytes(C.byref(self.params))
+        wb = self.L.sldg_workspace_bytes(C.byref(self.params))
+        if sb == 0 or wb == 0:
+            raise SldgError(SLDG_EINVAL, "sldg_state_bytes")
+        self.state_bytes, self.workspace_bytes = sb, wb
+        self.f_a = torch.empty(sb // 8, dtype=torch.float64, device=self.device)
+        self.f_b = torch.empty(sb // 8, dtype=torch.float64, device=self.device)
+        self.workspace = torch.empty(wb, dtype=torch.uint8, device=self.device)
+        self.stream = stream if stream is not None else torch.cuda.current_stream(self.device)
+        h = C.c_void_p()
+        with torch.cuda.device(self.device):
+            rc = self.L.sldg_create(C.byref(self.params), self.f_a.data_ptr(), self.f_b.data_ptr(),
+                                    self.workspace.data_ptr(), wb, self.stream.cuda_stream, C.byref(h))
+        self._chk(rc, "sldg_create")
+        self.h = h
+
+    def _chk(self, rc, what):
+        if rc != 0:
+            raise SldgError(rc, what)
+
+    def close(self):
+        if getattr(self, "h", None):
+            self.L.sldg_destroy(self.h)
+            self.h = None
+
+    def __del__(self):
+        try:
+            self.close()
+        except Exception:
+            pass
+
+    # ---- state ---------------------------------------------------------------------------------
+    def import_state(self, f_canonical):
+        assert f_canonical.is_cuda and f_canonical.dtype == self.torch.float64 and f_canonical.is_contiguous()
+        assert tuple(f_canonical.shape) == tuple(self.spec.shape)
+        self._chk(self.L.sldg_import_state(self.h, f_canonical.data_ptr()), "sldg_import_state")
+
+    def export_state(self, out=None):
+        if out is None:
+            out = self.torch.empty(self.spec.shape, dtype=self.torch.float64, device=self.device)
+        self._chk(self.L.sldg_export_state(self.h, out.data_ptr()), "sldg_export_state")
+        return out
+
+    def import_state_host(self, f_host):
+        """f_host: numpy array or CPU torch tensor, canonical layout."""
+        ptr = f_host.ctypes.data if hasattr(f_host, "ctypes") else f_host.data_ptr()
+        self._chk(self.L.sldg_import_state_host(self.h, ptr), "sldg_import_state_host")
+
+    def export_state_host(self, f_host):
+        ptr = f_host.ctypes.data if hasattr(f_host, "ctypes") else f_host.data_ptr()
+        self._chk(self.L.sldg_export_state_host(self.h, ptr), "sldg_export_state_host")
+        return f_host
+
+    def current_ptr(self):
+        return self.L.sldg_current(self.h)
+
+    # ---- fields --------------------------------------------------------------------------------
+    def set_Ez(self, Ez):
+        assert Ez.is_cuda and Ez.dtype == self.torch.float64 and Ez.is_contiguous()
+        self._chk(self.L.sldg_set_Ez(self.h, Ez.data_ptr()), "sldg_set_Ez")
+
+    def set_vxy(self, a, b, periodic):
+        for u in (a, b):
+            assert u.is_cuda and u.dtype == self.torch.float64 and u.is_contiguous()
+        self._chk(self.L.sldg_set_vxy(self.h, a.data_ptr(), b.data_ptr(), int(periodic)), "sldg_set_vxy")
+
+    def set_trace_order(self, order):
+        self._chk(self.L.sldg_set_trace_order(self.h, int(order)), "sldg_set_trace_order")
+
+    # ---- substeps ------------------------------------------------------------------------------
+    def advect_z(self, tau):
+        self._chk(self.L.sldg_advect_z(self.h, float(tau)), "sldg_advect_z")
+
+    def advect_v(self, tau):
+        self._chk(self.L.sldg_advect_v(self.h, float(tau)), "sldg_advect_v")
+
+    def advect_xy(self, tau, trace_order=2):
+        self._chk(self.L.sldg_advect_xy(self.h, float(tau), int(trace_order)), "sldg_advect_xy")
+
+    def strang_step(self, dt):
+        self._chk(self.L.sldg_strang_step(self.h, float(dt)), "sldg_strang_step")
+
+    def strang_step_host(self, dt, Ez_host=None, a_host=None, b_host=None, periodic=1, rho_host=None,
+                         mass_host=None):
+        def ptr(x):
+            if x is None:
+                return None
+            return x.ctypes.data if hasattr(x, "ctypes") else x.data_ptr()
+        self._chk(self.L.sldg_strang_step_host(self.h, float(dt), ptr(Ez_host), ptr(a_host), ptr(b_host),
+                                               int(periodic), ptr(rho_host), ptr(mass_host)),
+                  "sldg_strang_step_host")
+
+    def charge_density(self, out=None):
+        Nz, Nv, Ny, Nx = self.spec.shape
+        if out is None:
+            out = self.torch.empty((Nz, Ny, Nx), dtype=self.torch.float64, device=self.device)
+        self._chk(self.L.sldg_charge_density(self.h, out.data_ptr()), "sldg_charge_density")
+        return out
+
+    def mass(self, out=None):
+        if out is None:
+            out = self.torch.empty(1, dtype=self.torch.float64, device=self.device)
+        self._chk(self.L.sldg_mass(self.h, out.data_ptr()), "sldg_mass")
+        return out
+
+    # ---- diagnostics ---------------------------------------------------------------------------
+    def check(self):
+        """Synchronise and raise on a sticky device error."""
+        self._chk(self.L.sldg_check(self.h), "sldg_check")
+
+    def last_timing_ms(self):
+        ms = (C.c_float * 8)()
+        self._chk(self.L.sldg_last_timing_ms(self.h, C.byref(ms)), "sldg_last_timing_ms")
+        return list(ms)
+
+    def launch_count(self):
+        return int(self.L.sldg_launch_count(self.h))
+
+    def debug_geometry(self, z):
+        t = self.torch
+        nx, ny = self.spec.n[0], self.spec.n[1]
+        o4 = self.spec.order[0] ** 4
+        anchor = t.empty((ny * nx, 2), dtype=t.int32, device=self.device)
+        mask = t.empty(ny * nx, dtype=t.int32, device=self.device)
+        W = t.empty((ny * nx, 9, o4), dtype=t.float64, device=self.device)
+        self._chk(self.L.sldg_debug_geometry(self.h, int(z), anchor.data_ptr(), mask.data_ptr(), W.data_ptr()),
+                  "sldg_debug_geometry")
+        return anchor, mask, W

@@ -1,0 +1,541 @@
+// sldg_api.cu -- the C-ABI of libsldg (include/sldg.h): context, host-side tables, orchestration.
+// Product code for sm_100a; no CPU fallback, nothing from oracle/.
+#include <math.h>
+#include <stdio.h>
+#include <stdlib.h>
+#include <string.h>
+
+#include <new>
+#include <vector>
+
+#include "sldg_internal.cuh"
+
+namespace {
+
+size_t align_up(size_t v, size_t a) { return (v + a - 1) / a * a; }
+
+bool params_ok(const sldg_params *p)
+{
+    if (!p) return false;
+    for (int d = 0; d < 4; ++d) {
+        if (p->n[d] < 1 || p->order[d] < 1 || p->order[d] > SLDG_MAXO) return false;
+        if (!(p->hi[d] > p->lo[d])) return false;
+    }
+    if (p->order[0] != p->order[1]) return false;
+    if (p->max_stencil != 3) return false;
+    if (p->layout < 0 || p->layout > 3) return false;
+    return true;
+}
+
+void fill_grid(const sldg_params *p, GridDev *g)
+{
+    for (int d = 0; d < 4; ++d) {
+        g->n[d] = p->n[d];
+        g->o[d] = p->order[d];
+        g->N[d] = p->n[d] * p->order[d];
+        g->lo[d] = p->lo[d];
+        g->h[d] = (p->hi[d] - p->lo[d]) / p->n[d];
+    }
+    g->Pv = (int)align_up((size_t)g->N[3], SLDG_PV_ALIGN);
+    const long long Nx = g->N[0], Ny = g->N[1], Nz = g->N[2], Pv = g->Pv;
+    int layout = p->layout == 0 ? 1 : p->layout;
+    if (layout == 1) {  // z, y, x, v
+        g->sX = Pv; g->sY = Nx * Pv; g->sZ = Ny * Nx * Pv;
+    } else if (layout == 2) {  // y, x, z, v
+        g->sZ = Pv; g->sX = Nz * Pv; g->sY = Nx * Nz * Pv;
+    } else {  // y, z, x, v
+        g->sX = Pv; g->sZ = Nx * Pv; g->sY = Nz * Nx * Pv;
+    }
+    g->lines = Nz * Ny * Nx;
+}
+
+struct WorkspaceMap {
+    size_t Ez, va, vb, anchor, mask, W, partials, rho, scalar, err, total;
+    size_t n_partials;
+};
+
+WorkspaceMap map_workspace(const sldg_params *p)
+{
+    GridDev g;
+    fill_grid(p, &g);
+    WorkspaceMap m;
+    const size_t ncell = (size_t)g.n[0] * g.n[1], Nz = (size_t)g.N[2];
+    const size_t vplane = (size_t)(g.n[0] + 1) * (g.n[1] + 1);
+    const size_t o4 = (size_t)g.o[0] * g.o[0] * g.o[0] * g.o[0];
+    size_t off = 0;
+    auto take = [&](size_t bytes) { size_t at = off; off = align_up(off + bytes, 256); return at; };
+    m.Ez = take((size_t)g.lines * 8);
+    m.va = take(Nz * vplane * 8);
+    m.vb = take(Nz * vplane * 8);
+    m.anchor = take(Nz * ncell * 2 * 4);
+    m.mask = take(Nz * ncell * 4);
+    m.W = take(Nz * ncell * 9 * o4 * 8);
+    m.n_partials = 8192;
+    m.partials = take(m.n_partials * 8);
+    m.rho = take((size_t)g.lines * 8);
+    m.scalar = take(256);
+    m.err = take(256);
+    m.total = off;
+    return m;
+}
+
+// ---- host-side tables (long double) ---------------------------------------------------------------
+typedef std::vector<long double> Poly;
+
+Poly pmul(const Poly &a, const Poly &b)
+{
+    Poly r(a.size() + b.size() - 1, 0.0L);
+    for (size_t i = 0; i < a.size(); ++i)
+        for (size_t j = 0; j < b.size(); ++j) r[i + j] += a[i] * b[j];
+    return r;
+}
+
+long double binom(int n, int k)
+{
+    long double r = 1.0L;
+    for (int i = 1; i <= k; ++i) r = r * (n - k + i) / i;
+    return r;
+}
+
+void gl_nodes(int o, long double *x, long double *w)
+{
+    if (o == 1) {
+        x[0] = 0.5L; w[0] = 1.0L;
+    } else if (o == 2) {
+        long double d = sqrtl(3.0L) / 6.0L;
+        x[0] = 0.5L - d; x[1] = 0.5L + d;
+        w[0] = w[1] = 0.5L;
+    } else if (o == 3) {
+        long double d = sqrtl(15.0L) / 10.0L;
+        x[0] = 0.5L - d; x[1] = 0.5L; x[2] = 0.5L + d;
+        w[0] = w[2] = 5.0L / 18.0L; w[1] = 4.0L / 9.0L;
+    } else {  // o == 5 (edge quadrature only)
+        long double s = sqrtl(10.0L / 7.0L);
+        long double t1 = sqrtl(5.0L - 2.0L * s) / 3.0L, t2 = sqrtl(5.0L + 2.0L * s) / 3.0L;
+        long double w1 = (322.0L + 13.0L * sqrtl(70.0L)) / 900.0L, w2 = (322.0L - 13.0L * sqrtl(70.0L)) / 900.0L;
+        x[0] = 0.5L - 0.5L * t2; x[1] = 0.5L - 0.5L * t1; x[2] = 0.5L; x[3] = 0.5L + 0.5L * t1; x[4] = 0.5L + 0.5L * t2;
+        w[0] = w[4] = 0.5L * w2; w[1] = w[3] = 0.5L * w1; w[2] = 0.5L * 128.0L / 225.0L;
+    }
+}
+
+// monomial coefficients of the Lagrange basis on the o GL nodes
+void lagrange_monomials(int o, const long double *x, long double L[SLDG_MAXO][SLDG_MAXO])
+{
+    for (int j = 0; j < o; ++j) {
+        Poly p(1, 1.0L);
+        for (int i = 0; i < o; ++i)
+            if (i != j) {
+                Poly f(2);
+                f[0] = -x[i] / (x[j] - x[i]);
+                f[1] = 1.0L / (x[j] - x[i]);
+                p = pmul(p, f);
+            }
+        for (int a = 0; a < SLDG_MAXO; ++a) L[j][a] = a < (int)p.size() ? p[a] : 0.0L;
+    }
+}
+
+void fill_basis(const sldg_params *p, Basis *bs)
+{
+    memset(bs, 0, sizeof(*bs));
+    for (int o = 1; o <= SLDG_MAXO; ++o) {
+        long double x[5], w[5], L[SLDG_MAXO][SLDG_MAXO];
+        gl_nodes(o, x, w);
+        lagrange_monomials(o, x, L);
+        for (int j = 0; j < o; ++j) {
+            bs->xi[o][j] = (double)x[j];
+            bs->w[o][j] = (double)w[j];
+            for (int a = 0; a < o; ++a) bs->L[o][j][a] = (double)L[j][a];
+        }
+    }
+    const int nq = 2 * p->order[0] - 1;  // exact for the edge integrand of degree 4o-3
+    long double x[5], w[5];
+    gl_nodes(nq, x, w);
+    bs->nq = nq;
+    for (int k = 0; k < nq; ++k) {
+        bs->qx[k] = (double)x[k];
+        bs->qw[k] = (double)w[k];
+    }
+}
+
+// Polynomial coefficients in alpha of the overlap matrices of eq. (10)-(11):
+//   A_jm(alpha) = (1/w_j) int_0^{1-alpha} l_j(xi) l_m(xi+alpha) dxi
+//   B_jm(alpha) = (1/w_j) int_0^{alpha}   l_j(eta+1-alpha) l_m(eta) deta
+// obtained by expanding the integrals symbolically (binomial theorem), long double arithmetic.
+void fill_shift_poly(int o, ShiftPoly *sp)
+{
+    memset(sp, 0, sizeof(*sp));
+    sp->o = o;
+    long double x[5], w[5], L[SLDG_MAXO][SLDG_MAXO];
+    gl_nodes(o, x, w);
+    lagrange_monomials(o, x, L);
+    const int deg = 2 * o;  // number of coefficients (degree 2o-1)
+    auto one_minus_alpha_pow = [&](int n) {
+        Poly r(n + 1);
+        for (int e = 0; e <= n; ++e) r[e] = binom(n, e) * ((e & 1) ? -1.0L : 1.0L);
+        return r;
+    };
+    auto alpha_pow = [&](int n) {
+        Poly r(n + 1, 0.0L);
+        r[n] = 1.0L;
+        return r;
+    };
+    for (int j = 0; j < o; ++j)
+        for (int m = 0; m < o; ++m) {
+            Poly pa(deg, 0.0L), pb(deg, 0.0L);
+            for (int a = 0; a < o; ++a)
+                for (int b = 0; b < o; ++b) {
+                    // A: l_m(xi+alpha) = sum_b L_m[b] sum_c C(b,c) xi^c alpha^(b-c)
+                    for (int c = 0; c <= b; ++c) {
+                        Poly t = pmul(alpha_pow(b - c), one_minus_alpha_pow(a + c + 1));
+                        long double k = L[j][a] * L[m][b] * binom(b, c) / (a + c + 1);
+                        for (size_t d = 0; d < t.size(); ++d) pa[d] += k * t[d];
+                    }
+                    // B: l_j(eta+1-alpha) = sum_a L_j[a] sum_c C(a,c) eta^c (1-alpha)^(a-c)
+                    for (int c = 0; c <= a; ++c) {
+                        Poly t = pmul(one_minus_alpha_pow(a - c), alpha_pow(b + c + 1));
+                        long double k = L[j][a] * L[m][b] * binom(a, c) / (b + c + 1);
+                        for (size_t d = 0; d < t.size(); ++d) pb[d] += k * t[d];
+                    }
+                }
+            for (int d = 0; d < deg; ++d) {
+                sp->a[j][m][d] = (double)(pa[d] / w[j]);
+                sp->b[j][m][d] = (double)(pb[d] / w[j]);
+            }
+            // A(0) = I and B(0) = 0 hold exactly (orthogonality of the basis): integer Courant numbers
+            // must be bit-exact copies, so the constant terms are set to their exact values.
+            sp->a[j][m][0] = (j == m) ? 1.0 : 0.0;
+            sp->b[j][m][0] = 0.0;
+        }
+}
+
+int cuda_fail(cudaError_t e) { return e == cudaSuccess ? SLDG_OK : SLDG_ECUDA; }
+
+void swap_state(sldg_ctx *c) { c->cur ^= 1; }
+
+}  // namespace
+
+extern "C" {
+
+size_t sldg_state_bytes(const sldg_params *p)
+{
+    if (!params_ok(p)) return 0;
+    GridDev g;
+    fill_grid(p, &g);
+    return (size_t)g.lines * g.Pv * 8;
+}
+
+size_t sldg_workspace_bytes(const sldg_params *p)
+{
+    if (!params_ok(p)) return 0;
+    return map_workspace(p).total;
+}
+
+int sldg_create(const sldg_params *p, double *f_a_dev, double *f_b_dev, void *workspace_dev,
+                size_t workspace_bytes, void *cuda_stream, sldg_ctx **out)
+{
+    if (!out) return SLDG_EINVAL;
+    *out = nullptr;
+    if (!params_ok(p) || !f_a_dev || !f_b_dev || !workspace_dev) return SLDG_EINVAL;
+    if (((uintptr_t)f_a_dev | (uintptr_t)f_b_dev | (uintptr_t)workspace_dev) & 255) return SLDG_EINVAL;
+    WorkspaceMap m = map_workspace(p);
+    if (workspace_bytes < m.total) return SLDG_EINVAL;
+    int dev = 0;
+    if (cudaGetDevice(&dev) != cudaSuccess) return SLDG_ECUDA;
+    sldg_ctx *c = new (std::nothrow) sldg_ctx();
+    if (!c) return SLDG_EINVAL;
+    memset(c, 0, sizeof(*c));
+    c->p = *p;
+    fill_grid(p, &c->g);
+    fill_basis(p, &c->basis);
+    fill_shift_poly(p->order[2], &c->sp_z);
+    fill_shift_poly(p->order[3], &c->sp_v);
+    c->stream = (cudaStream_t)cuda_stream;
+    c->f[0] = f_a_dev;
+    c->f[1] = f_b_dev;
+    c->cur = 0;
+    char *ws = (char *)workspace_dev;
+    c->Ez = (double *)(ws + m.Ez);
+    c->va = (double *)(ws + m.va);
+    c->vb = (double *)(ws + m.vb);
+    c->anchor = (int32_t *)(ws + m.anchor);
+    c->mask = (int32_t *)(ws + m.mask);
+    c->W = (double *)(ws + m.W);
+    c->partials = (double *)(ws + m.partials);
+    c->n_partials = m.n_partials;
+    c->err = (int32_t *)(ws + m.err);
+    c->trace_order = 2;
+    c->vel_periodic = 0;
+    if (cudaDeviceGetAttribute(&c->sm_count, cudaDevAttrMultiProcessorCount, dev) != cudaSuccess) {
+        delete c;
+        return SLDG_ECUDA;
+    }
+    for (int k = 0; k < 8; ++k)
+        if (cudaEventCreate(&c->ev[k]) != cudaSuccess) {
+            delete c;
+            return SLDG_ECUDA;
+        }
+    // fields default to zero, error word cleared
+    cudaError_t e = cudaMemsetAsync(ws + m.Ez, 0, m.anchor - m.Ez, c->stream);
+    if (e == cudaSuccess) e = cudaMemsetAsync(c->err, 0, 256, c->stream);
+    if (e != cudaSuccess) {
+        delete c;
+        return SLDG_ECUDA;
+    }
+    *out = c;
+    return SLDG_OK;
+}
+
+int sldg_destroy(sldg_ctx *c)
+{
+    if (!c) return SLDG_EINVAL;
+    for (int k = 0; k < 8; ++k)
+        if (c->ev[k]) cudaEventDestroy(c->ev[k]);
+    delete c;
+    return SLDG_OK;
+}
+
+double *sldg_current(sldg_ctx *c) { return c ? c->f[c->cur] : nullptr; }
+
+int sldg_import_state(sldg_ctx *c, const double *f_canonical_dev)
+{
+    if (!c || !f_canonical_dev) return SLDG_EINVAL;
+    return cuda_fail(launch_pack(c, f_canonical_dev, c->f[c->cur]));
+}
+
+int sldg_export_state(sldg_ctx *c, double *f_canonical_dev)
+{
+    if (!c || !f_canonical_dev) return SLDG_EINVAL;
+    return cuda_fail(launch_unpack(c, c->f[c->cur], f_canonical_dev));
+}
+
+int sldg_import_state_host(sldg_ctx *c, const double *f_host)
+{
+    if (!c || !f_host) return SLDG_EINVAL;
+    const GridDev &g = c->g;
+    size_t bytes = (size_t)g.lines * g.N[3] * 8;
+    double *stage = c->f[c->cur ^ 1];
+    if (cudaMemcpyAsync(stage, f_host, bytes, cudaMemcpyHostToDevice, c->stream) != cudaSuccess) return SLDG_ECUDA;
+    if (launch_pack(c, stage, c->f[c->cur]) != cudaSuccess) return SLDG_ECUDA;
+    return cuda_fail(cudaStreamSynchronize(c->stream));
+}
+
+int sldg_export_state_host(sldg_ctx *c, double *f_host)
+{
+    if (!c || !f_host) return SLDG_EINVAL;
+    const GridDev &g = c->g;
+    size_t bytes = (size_t)g.lines * g.N[3] * 8;
+    double *stage = c->f[c->cur ^ 1];
+    if (launch_unpack(c, c->f[c->cur], stage) != cudaSuccess) return SLDG_ECUDA;
+    if (cudaMemcpyAsync(f_host, stage, bytes, cudaMemcpyDeviceToHost, c->stream) != cudaSuccess) return SLDG_ECUDA;
+    return cuda_fail(cudaStreamSynchronize(c->stream));
+}
+
+int sldg_set_Ez(sldg_ctx *c, const double *Ez_dev)
+{
+    if (!c || !Ez_dev) return SLDG_EINVAL;
+    return cuda_fail(cudaMemcpyAsync(c->Ez, Ez_dev, (size_t)c->g.lines * 8, cudaMemcpyDeviceToDevice, c->stream));
+}
+
+int sldg_set_vxy(sldg_ctx *c, const double *a_dev, const double *b_dev, int periodic)
+{
+    if (!c || !a_dev || !b_dev) return SLDG_EINVAL;
+    const GridDev &g = c->g;
+    size_t bytes = (size_t)g.N[2] * (g.n[0] + 1) * (g.n[1] + 1) * 8;
+    c->vel_periodic = periodic ? 1 : 0;
+    if (cudaMemcpyAsync(c->va, a_dev, bytes, cudaMemcpyDeviceToDevice, c->stream) != cudaSuccess) return SLDG_ECUDA;
+    return cuda_fail(cudaMemcpyAsync(c->vb, b_dev, bytes, cudaMemcpyDeviceToDevice, c->stream));
+}
+
+int sldg_set_trace_order(sldg_ctx *c, int trace_order)
+{
+    if (!c || (trace_order != 1 && trace_order != 2)) return SLDG_EINVAL;
+    c->trace_order = trace_order;
+    return SLDG_OK;
+}
+
+static int do_z(sldg_ctx *c, double tau)
+{
+    cudaError_t e = launch_advect_z(c, c->f[c->cur], c->f[c->cur ^ 1], tau);
+    if (e != cudaSuccess) return e == cudaErrorInvalidValue ? SLDG_EINVAL : SLDG_ECUDA;
+    swap_state(c);
+    return SLDG_OK;
+}
+
+static int do_v(sldg_ctx *c, double tau)
+{
+    cudaError_t e = launch_advect_v(c, c->f[c->cur], c->f[c->cur ^ 1], tau);
+    if (e != cudaSuccess) return e == cudaErrorInvalidValue ? SLDG_EINVAL : SLDG_ECUDA;
+    swap_state(c);
+    return SLDG_OK;
+}
+
+static int do_xy(sldg_ctx *c, double tau, int trace_order, cudaEvent_t mid)
+{
+    if (launch_xy_geometry(c, tau, trace_order) != cudaSuccess) return SLDG_ECUDA;
+    if (mid) cudaEventRecord(mid, c->stream);
+    if (launch_xy_apply(c, c->f[c->cur], c->f[c->cur ^ 1]) != cudaSuccess) return SLDG_ECUDA;
+    swap_state(c);
+    return SLDG_OK;
+}
+
+int sldg_advect_z(sldg_ctx *c, double tau)
+{
+    if (!c) return SLDG_EINVAL;
+    cudaEventRecord(c->ev[0], c->stream);
+    int rc = do_z(c, tau);
+    cudaEventRecord(c->ev[1], c->stream);
+    c->ev_kind = 2;
+    return rc;
+}
+
+int sldg_advect_v(sldg_ctx *c, double tau)
+{
+    if (!c) return SLDG_EINVAL;
+    cudaEventRecord(c->ev[0], c->stream);
+    int rc = do_v(c, tau);
+    cudaEventRecord(c->ev[1], c->stream);
+    c->ev_kind = 3;
+    return rc;
+}
+
+int sldg_advect_xy(sldg_ctx *c, double tau, int trace_order)
+{
+    if (!c || (trace_order != 1 && trace_order != 2)) return SLDG_EINVAL;
+    cudaEventRecord(c->ev[0], c->stream);
+    int rc = do_xy(c, tau, trace_order, c->ev[1]);
+    cudaEventRecord(c->ev[2], c->stream);
+    c->ev_kind = 4;
+    return rc;
+}
+
+int sldg_charge_density(sldg_ctx *c, double *rho_dev)
+{
+    if (!c || !rho_dev) return SLDG_EINVAL;
+    return cuda_fail(launch_charge_density(c, c->f[c->cur], rho_dev));
+}
+
+int sldg_mass(sldg_ctx *c, double *mass_dev)
+{
+    if (!c || !mass_dev) return SLDG_EINVAL;
+    return cuda_fail(launch_mass(c, c->f[c->cur], mass_dev));
+}
+
+int sldg_strang_step(sldg_ctx *c, double dt)
+{
+    if (!c) return SLDG_EINVAL;
+    int rc;
+    cudaEventRecord(c->ev[0], c->stream);
+    if ((rc = do_z(c, 0.5 * dt))) return rc;
+    cudaEventRecord(c->ev[1], c->stream);
+    if ((rc = do_v(c, 0.5 * dt))) return rc;
+    cudaEventRecord(c->ev[2], c->stream);
+    if ((rc = do_xy(c, dt, c->trace_order, c->ev[3]))) return rc;
+    cudaEventRecord(c->ev[4], c->stream);
+    if ((rc = do_v(c, 0.5 * dt))) return rc;
+    cudaEventRecord(c->ev[5], c->stream);
+    if ((rc = do_z(c, 0.5 * dt))) return rc;
+    cudaEventRecord(c->ev[6], c->stream);
+    c->ev_kind = 1;
+    return SLDG_OK;
+}
+
+int sldg_strang_step_host(sldg_ctx *c, double dt, const double *Ez_host, const double *a_host,
+                          const double *b_host, int periodic, double *rho_host, double *mass_host)
+{
+    if (!c) return SLDG_EINVAL;
+    if ((a_host == nullptr) != (b_host == nullptr)) return SLDG_EINVAL;
+    const GridDev &g = c->g;
+    WorkspaceMap m = map_workspace(&c->p);
+    char *ws = (char *)c->Ez - m.Ez;
+    double *rho_dev = (double *)(ws + m.rho);
+    double *mass_dev = (double *)(ws + m.scalar);
+    if (Ez_host &&
+        cudaMemcpyAsync(c->Ez, Ez_host, (size_t)g.lines * 8, cudaMemcpyHostToDevice, c->stream) != cudaSuccess)
+        return SLDG_ECUDA;
+    if (a_host) {
+        size_t bytes = (size_t)g.N[2] * (g.n[0] + 1) * (g.n[1] + 1) * 8;
+        c->vel_periodic = periodic ? 1 : 0;
+        if (cudaMemcpyAsync(c->va, a_host, bytes, cudaMemcpyHostToDevice, c->stream) != cudaSuccess) return SLDG_ECUDA;
+        if (cudaMemcpyAsync(c->vb, b_host, bytes, cudaMemcpyHostToDevice, c->stream) != cudaSuccess) return SLDG_ECUDA;
+    }
+    int rc = sldg_strang_step(c, dt);
+    if (rc) return rc;
+    if (rho_host) {
+        if (launch_charge_density(c, c->f[c->cur], rho_dev) != cudaSuccess) return SLDG_ECUDA;
+        if (cudaMemcpyAsync(rho_host, rho_dev, (size_t)g.lines * 8, cudaMemcpyDeviceToHost, c->stream) != cudaSuccess)
+            return SLDG_ECUDA;
+    }
+    if (mass_host) {
+        if (launch_mass(c, c->f[c->cur], mass_dev) != cudaSuccess) return SLDG_ECUDA;
+        if (cudaMemcpyAsync(mass_host, mass_dev, 8, cudaMemcpyDeviceToHost, c->stream) != cudaSuccess) return SLDG_ECUDA;
+    }
+    return cuda_fail(cudaStreamSynchronize(c->stream));
+}
+
+int sldg_check(sldg_ctx *c)
+{
+    if (!c) return SLDG_EINVAL;
+    int32_t word = 0;
+    if (cudaMemcpyAsync(&word, c->err, 4, cudaMemcpyDeviceToHost, c->stream) != cudaSuccess) return SLDG_ECUDA;
+    if (cudaStreamSynchronize(c->stream) != cudaSuccess) return SLDG_ECUDA;
+    if (cudaGetLastError() != cudaSuccess) return SLDG_ECUDA;
+    if (word != 0) cudaMemsetAsync(c->err, 0, 4, c->stream);
+    return (int)word;
+}
+
+int sldg_last_timing_ms(sldg_ctx *c, float ms[8])
+{
+    if (!c || !ms) return SLDG_EINVAL;
+    for (int k = 0; k < 8; ++k) ms[k] = 0.0f;
+    if (c->ev_kind == 0) return SLDG_OK;
+    if (cudaStreamSynchronize(c->stream) != cudaSuccess) return SLDG_ECUDA;
+    auto el = [&](int a, int b) {
+        float t = 0.0f;
+        cudaEventElapsedTime(&t, c->ev[a], c->ev[b]);
+        return t;
+    };
+    if (c->ev_kind == 1) {
+        for (int k = 0; k < 6; ++k) ms[k] = el(k, k + 1);
+        ms[7] = el(0, 6);
+    } else if (c->ev_kind == 2) {
+        ms[0] = ms[7] = el(0, 1);
+    } else if (c->ev_kind == 3) {
+        ms[1] = ms[7] = el(0, 1);
+    } else if (c->ev_kind == 4) {
+        ms[2] = el(0, 1);
+        ms[3] = el(1, 2);
+        ms[7] = el(0, 2);
+    }
+    return SLDG_OK;
+}
+
+long long sldg_launch_count(sldg_ctx *c) { return c ? c->launches : 0; }
+
+int sldg_debug_geometry(sldg_ctx *c, int z, int32_t *anchor_dev, int32_t *mask_dev, double *W_dev)
+{
+    if (!c || z < 0 || z >= c->g.N[2]) return SLDG_EINVAL;
+    const size_t ncell = (size_t)c->g.n[0] * c->g.n[1];
+    const size_t o4 = (size_t)c->g.o[0] * c->g.o[0] * c->g.o[0] * c->g.o[0];
+    cudaError_t e = cudaSuccess;
+    if (anchor_dev)
+        e = cudaMemcpyAsync(anchor_dev, c->anchor + (size_t)z * ncell * 2, ncell * 8, cudaMemcpyDeviceToDevice, c->stream);
+    if (e == cudaSuccess && mask_dev)
+        e = cudaMemcpyAsync(mask_dev, c->mask + (size_t)z * ncell, ncell * 4, cudaMemcpyDeviceToDevice, c->stream);
+    if (e == cudaSuccess && W_dev)
+        e = cudaMemcpyAsync(W_dev, c->W + (size_t)z * ncell * 9 * o4, ncell * 9 * o4 * 8, cudaMemcpyDeviceToDevice, c->stream);
+    return cuda_fail(e);
+}
+
+const char *sldg_strerror(int code)
+{
+    switch (code) {
+        case SLDG_OK: return "ok";
+        case SLDG_EINVAL: return "invalid argument";
+        case SLDG_ECUDA: return "CUDA error or no device";
+        case SLDG_ESTENCIL: return "upstream cell exceeds the 3x3 stencil";
+        case SLDG_EGEOM: return "degenerate upstream geometry (crossed characteristics or singular Vandermonde)";
+        default: return "unknown error";
+    }
+}
+
+}  // extern "C"

@@ -1,0 +1,73 @@
+// sldg_internal.cuh -- shared declarations of the CUDA SLDG library (sm_100a).  Product code: shares
+// nothing with oracle/.
+#pragma once
+#include <cuda_runtime.h>
+#include <stdint.h>
+
+#include "sldg.h"
+
+#define SLDG_MAXO 3
+#define SLDG_MAXO2 9
+#define SLDG_MAXQ 5       // quadrature points per edge for the Green's-theorem line integrals (2o-1)
+#define SLDG_PV_ALIGN 16  // internal v-line pitch is a multiple of 16 doubles (128 B)
+
+// Grid description passed by value to kernels (lives in the constant bank).
+struct GridDev {
+    int n[4];   // cells x,y,z,v
+    int o[4];   // nodes per cell
+    int N[4];   // DOFs
+    double lo[4], h[4];
+    // internal layout: element (z,Y,X,v) at  z*sZ + Y*sY + X*sX + v   (doubles), v contiguous, pitch Pv
+    long long sX, sY, sZ;
+    int Pv;
+    long long lines;  // Nz*Ny*Nx
+};
+
+// Gauss-Legendre tables on (0,1) per axis order, Lagrange monomial coefficients, edge quadrature.
+struct Basis {
+    double xi[SLDG_MAXO + 1][SLDG_MAXO];              // xi[o][node]
+    double w[SLDG_MAXO + 1][SLDG_MAXO];               // w[o][node], sums to 1
+    double L[SLDG_MAXO + 1][SLDG_MAXO][SLDG_MAXO];    // l_j(x) = sum_a L[o][j][a] x^a
+    double qx[SLDG_MAXQ], qw[SLDG_MAXQ];              // (2*oxy-1)-point rule for edge integrals
+    int nq;
+};
+
+// A_jm(alpha) = sum_d a[j][m][d] alpha^d,  B likewise; degree 2o-1 (eq. 10-11).
+struct ShiftPoly {
+    double a[SLDG_MAXO][SLDG_MAXO][2 * SLDG_MAXO];
+    double b[SLDG_MAXO][SLDG_MAXO][2 * SLDG_MAXO];
+    int o;
+};
+
+struct sldg_ctx {
+    sldg_params p;
+    GridDev g;
+    Basis basis;
+    ShiftPoly sp_z, sp_v;
+    cudaStream_t stream;
+    double *f[2];
+    int cur;
+    // workspace carve-up
+    double *Ez, *va, *vb;   // fields
+    int32_t *anchor;        // [Nz][ncell][2]
+    int32_t *mask;          // [Nz][ncell]
+    double *W;              // [Nz][ncell][9][o2*o2]  (k-major: W[k*o2+m])
+    double *partials;       // reduction scratch
+    int32_t *err;           // sticky device error word
+    size_t n_partials;
+    int trace_order, vel_periodic;
+    cudaEvent_t ev[8];
+    int ev_kind;            // 0 none, 1 strang, 2 z, 3 v, 4 xy
+    long long launches;
+    int sm_count;
+};
+
+// ---- kernel launchers (each returns cudaGetLastError()) ------------------------------------------
+cudaError_t launch_pack(sldg_ctx *c, const double *canon, double *internal);
+cudaError_t launch_unpack(sldg_ctx *c, const double *internal, double *canon);
+cudaError_t launch_advect_z(sldg_ctx *c, const double *fin, double *fout, double tau);
+cudaError_t launch_advect_v(sldg_ctx *c, const double *fin, double *fout, double tau);
+cudaError_t launch_charge_density(sldg_ctx *c, const double *fin, double *rho);
+cudaError_t launch_mass(sldg_ctx *c, const double *fin, double *mass_out);
+cudaError_t launch_xy_geometry(sldg_ctx *c, double tau, int trace_order);
+cudaError_t launch_xy_apply(sldg_ctx *c, const double *fin, double *fout);

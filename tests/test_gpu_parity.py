@@ -1,0 +1,351 @@
+"""Parity of the CUDA path (libsldg through the C-ABI) against the CPU oracle, element by element on the
+same seeded inputs.  Bar (north_star): relative L-infinity error <= 1e-11, mass conserved to <= 1e-13
+relative; integer/index work (integer Courant numbers, layout transposes) bit-exact."""
+import math
+
+import numpy as np
+import pytest
+
+import oracle
+from paper_2212_03036_b200 import inputs
+from paper_2212_03036_b200.inputs import GridSpec
+
+pytestmark = pytest.mark.gpu
+
+TOL = 1e-11
+
+
+@pytest.fixture(scope="module")
+def torch():
+    import torch as t
+    if not t.cuda.is_available():
+        pytest.skip("needs a CUDA device")
+    return t
+
+
+def _sldg(spec, layout=0):
+    from paper_2212_03036_b200.binding import Sldg
+    return Sldg(spec, layout=layout)
+
+
+def _dev(torch, x):
+    return torch.from_numpy(np.ascontiguousarray(x)).cuda()
+
+
+def _rel(got, ref):
+    return np.abs(got - ref).max() / np.abs(ref).max()
+
+
+SPECS = {
+    "o2_ragged": GridSpec(n=(5, 3, 7, 11), order=(2, 2, 2, 2), lo=(-1, -2, 0, -3.0), hi=(1, 2, 10, 3.5)),
+    "o3_ragged": GridSpec(n=(4, 5, 6, 7), order=(3, 3, 3, 3), lo=(-1, -2, 0, -3.0), hi=(1, 2, 10, 3.5)),
+    "mixed": GridSpec(n=(6, 4, 5, 40), order=(2, 2, 3, 2), lo=(0, 0, 0, -2.0), hi=(1, 1, 5, 2.0)),
+    "o1": GridSpec(n=(6, 4, 9, 70), order=(2, 2, 1, 1), lo=(0, 0, 0, -2.0), hi=(1, 1, 5, 2.0)),
+}
+
+
+@pytest.mark.parametrize("name", list(SPECS))
+@pytest.mark.parametrize("layout", [1, 2, 3])
+def test_pack_unpack_roundtrip_is_bit_exact(torch, name, layout):
+    spec = SPECS[name]
+    rng = np.random.default_rng(1)
+    f = rng.standard_normal(spec.shape)
+    s = _sldg(spec, layout)
+    s.import_state(_dev(torch, f))
+    out = s.export_state().cpu().numpy()
+    s.check()
+    assert np.array_equal(out, f)
+    host = np.empty_like(f)
+    s.import_state_host(f)
+    s.export_state_host(host)
+    assert np.array_equal(host, f)
+
+
+@pytest.mark.parametrize("name", list(SPECS))
+@pytest.mark.parametrize("cfl", [0.3, 20.0])
+def test_advect_z_parity(torch, name, cfl):
+    spec = SPECS[name]
+    rng = np.random.default_rng(2)
+    f = rng.random(spec.shape)
+    tau = inputs.sweeps_dt_z(spec, cfl)
+    ref = oracle.advect_z(spec, f, tau)
+    for layout in (1, 2):
+        s = _sldg(spec, layout)
+        s.import_state(_dev(torch, f))
+        s.advect_z(tau)
+        got = s.export_state().cpu().numpy()
+        s.check()
+        assert _rel(got, ref) <= TOL
+    s.advect_z(-0.37 * tau)
+    ref2 = oracle.advect_z(spec, ref, -0.37 * tau)
+    assert _rel(s.export_state().cpu().numpy(), ref2) <= TOL
+
+
+@pytest.mark.parametrize("name", list(SPECS))
+@pytest.mark.parametrize("cfl", [0.4, 2.5, 40.0])
+def test_advect_v_parity(torch, name, cfl):
+    spec = SPECS[name]
+    rng = np.random.default_rng(3)
+    f = rng.random(spec.shape)
+    Ez = inputs.fourier_Ez(spec, seed=2, modes=3)
+    tau = inputs.sweeps_dt_v(spec, Ez, cfl)
+    ref = oracle.advect_v(spec, f, Ez, tau)
+    for layout in (1, 2):
+        s = _sldg(spec, layout)
+        s.import_state(_dev(torch, f))
+        s.set_Ez(_dev(torch, Ez))
+        s.advect_v(tau)
+        got = s.export_state().cpu().numpy()
+        s.check()
+        assert _rel(got, ref) <= TOL
+
+
+def test_integer_courant_numbers_are_bit_exact(torch):
+    """A(0) = I, B(0) = 0: integer shifts copy the data with wrap, bit for bit (both sweeps)."""
+    spec = GridSpec(n=(3, 2, 6, 8), order=(2, 2, 2, 1), lo=(0, 0, 0.0, -4.0), hi=(1, 1, 6.0, 4.0))
+    rng = np.random.default_rng(4)
+    f = rng.standard_normal(spec.shape)
+    s = _sldg(spec)
+    s.import_state(_dev(torch, f))
+    s.advect_z(2.0)  # v nodes at -3.5..3.5, hz = 1: Courant numbers -7, -5, ..., 7
+    got = s.export_state().cpu().numpy()
+    v = spec.node_coords(3)
+    Nz, Nv, Ny, Nx = spec.shape
+    for V in range(Nv):
+        k = int(round(v[V] * 2.0))
+        ref = np.roll(f[:, V].reshape(6, 2, Ny, Nx), k, axis=0).reshape(Nz, Ny, Nx)
+        assert np.array_equal(got[:, V], ref)
+    # v sweep: Ez * tau / hv integer per line
+    spec = GridSpec(n=(3, 2, 2, 8), order=(2, 2, 1, 2), lo=(0, 0, 0.0, -4.0), hi=(1, 1, 6.0, 4.0))
+    f = rng.standard_normal(spec.shape)
+    Nz, Nv, Ny, Nx = spec.shape
+    k = rng.integers(-11, 12, size=(Nz, Ny, Nx))
+    s = _sldg(spec)
+    s.import_state(_dev(torch, f))
+    s.set_Ez(_dev(torch, k.astype(np.float64)))
+    s.advect_v(1.0)  # hv = 1
+    got = s.export_state().cpu().numpy()
+    s.check()
+    for z in range(Nz):
+        for y in range(Ny):
+            for x in range(Nx):
+                ref = np.roll(f[z, :, y, x].reshape(8, 2), k[z, y, x], axis=0).reshape(-1)
+                assert np.array_equal(got[z, :, y, x], ref)
+
+
+@pytest.mark.parametrize("name", list(SPECS))
+def test_charge_density_and_mass_parity(torch, name):
+    spec = SPECS[name]
+    rng = np.random.default_rng(5)
+    f = rng.random(spec.shape)
+    s = _sldg(spec)
+    s.import_state(_dev(torch, f))
+    rho = s.charge_density().cpu().numpy()
+    m = float(s.mass().cpu()[0])
+    s.check()
+    assert _rel(rho, oracle.charge_density(spec, f)) <= 1e-13
+    assert abs(m - oracle.mass(spec, f)) <= 1e-13 * abs(m)
+
+
+def _periodic_velocity(spec, seed, cfl, tau, Nz, wobble=0.12):
+    """Bitwise-periodic smooth flow: a mean drift (sets the Courant number, so upstream cells land up to
+    `cfl` cells away) plus a few low Fourier modes that deform them moderately (the upstream cells must
+    stay convex: PAPER.md:190 'stability problems might appear if the approximated characteristics
+    cross')."""
+    nx, ny = spec.n[0], spec.n[1]
+    rng = np.random.default_rng(seed)
+    X, Y = np.meshgrid(np.arange(nx) / nx, np.arange(ny) / ny, indexing="xy")
+    a = np.zeros((Nz, ny + 1, nx + 1))
+    b = np.zeros_like(a)
+    for z in range(Nz):
+        ua = np.full((ny, nx), rng.uniform(-1, 1))
+        ub = np.full((ny, nx), rng.uniform(-1, 1))
+        for _ in range(4):
+            kx, ky = rng.integers(0, 3, size=2)
+            ua += wobble * rng.uniform(-1, 1) * np.cos(2 * np.pi * (kx * X + ky * Y) + rng.uniform(0, 6.28))
+            ub += wobble * rng.uniform(-1, 1) * np.cos(2 * np.pi * (kx * X + ky * Y) + rng.uniform(0, 6.28))
+        sc = cfl / max(np.abs(ua).max() * tau / spec.h[0], np.abs(ub).max() * tau / spec.h[1])
+        for dst, src in ((a[z], ua), (b[z], ub)):
+            dst[:ny, :nx] = sc * src
+            dst[ny, :nx] = dst[0, :nx]
+            dst[:, nx] = dst[:, 0]
+    return a, b
+
+
+@pytest.mark.parametrize("o", [2, 3])
+@pytest.mark.parametrize("trace_order", [1, 2])
+def test_xy_geometry_matches_oracle_coefficients(torch, o, trace_order):
+    """Green's-theorem weights (GPU) vs clipped-polygon Gauss quadrature (oracle), block by block, plus the
+    column-sum identity (mass conservation) evaluated on the GPU weights alone."""
+    spec = GridSpec(n=(9, 7, 2, 3), order=(o, o, 1, 1), lo=(0, 0, 0, 0), hi=(1.8, 2.1, 1, 1))
+    nx, ny = spec.n[0], spec.n[1]
+    tau = 0.05
+    a, b = _periodic_velocity(spec, 5, 0.9, tau, 2)
+    s = _sldg(spec)
+    s.import_state(_dev(torch, np.zeros(spec.shape)))
+    s.set_vxy(_dev(torch, a), _dev(torch, b), 1)
+    s.advect_xy(tau, trace_order)
+    s.check()
+    _, wg = oracle.gl(o)
+    Wm = np.array([wg[m % o] * wg[m // o] for m in range(o * o)])
+    for z in range(2):
+        anchor, mask, W = (t.cpu().numpy() for t in s.debug_geometry(z))
+        offs, er, es, eC = oracle.xy_plane_geometry(spec, a[z], b[z], tau, trace_order, 1)
+        col = np.zeros((ny, nx, o * o))
+        worst, scale = 0.0, 1.0
+        for t in range(nx * ny):
+            seen = 0
+            for e in range(offs[t], offs[t + 1]):
+                r, c = er[e] % nx, es[e] % ny
+                dx, dy = (r - anchor[t, 0]) % nx, (c - anchor[t, 1]) % ny
+                assert dx < 3 and dy < 3
+                slot = dx + 3 * dy
+                ref = (eC[e] / Wm[:, None]).T.reshape(-1)  # k-major [k][m]
+                if (mask[t] >> slot) & 1:
+                    seen |= 1 << slot
+                    worst = max(worst, np.abs(W[t, slot] - ref).max())
+                    scale = max(scale, np.abs(ref).max())
+                    col[c, r] += (W[t, slot].reshape(o * o, o * o) * Wm[None, :]).sum(axis=1)
+                else:
+                    assert np.abs(ref).max() < 1e-13  # empty on the GPU <=> zero-area piece
+            assert seen == mask[t]
+        assert worst < 1e-12 * scale
+        assert np.abs(col - Wm).max() < 5e-14
+
+
+def _xy_case(torch, spec, f, a, b, tau, trace_order, periodic, steps=1):
+    s = _sldg(spec)
+    s.import_state(_dev(torch, f))
+    s.set_vxy(_dev(torch, a), _dev(torch, b), periodic)
+    ref = f
+    for _ in range(steps):
+        s.advect_xy(tau, trace_order)
+        ref = oracle.advect_xy(spec, ref, a, b, tau, trace_order, periodic)
+    got = s.export_state().cpu().numpy()
+    s.check()
+    return got, ref, s
+
+
+@pytest.mark.parametrize("o", [2, 3])
+@pytest.mark.parametrize("trace_order", [1, 2])
+@pytest.mark.parametrize("cfl", [0.5, 1.7])
+def test_advect_xy_parity_random_periodic_flow(torch, o, trace_order, cfl):
+    spec = GridSpec(n=(11, 9, 3, 13), order=(o, o, 1, 2), lo=(0, 0, 0, 0), hi=(2.2, 1.8, 1, 1))
+    rng = np.random.default_rng(6)
+    f = rng.random(spec.shape)
+    tau = 0.1
+    a, b = _periodic_velocity(spec, 8, cfl, tau, spec.shape[0])
+    got, ref, s = _xy_case(torch, spec, f, a, b, tau, trace_order, 1, steps=2)
+    assert _rel(got, ref) <= TOL
+    m0, m1 = oracle.mass(spec, f), float(s.mass().cpu()[0])
+    assert abs(m1 - m0) <= 1e-13 * abs(m0)
+
+
+@pytest.mark.parametrize("o", [2, 3])
+def test_advect_xy_parity_rotation_and_swirl(torch, o):
+    """Config 1 shapes at a size the oracle finishes in seconds: 48x48 cells, 40 planes."""
+    spec = inputs.bumps_grid(48, 40, o)
+    f = inputs.bumps_initial_f(spec, seed=1)
+    a, b = inputs.rotation_velocity(spec)
+    got, ref, _ = _xy_case(torch, spec, f, a, b, 2 * math.pi / 40, 2, 0, steps=3)
+    assert _rel(got, ref) <= TOL
+    tau = 0.05
+    a, b = inputs.swirl_velocity(spec, 0.5 * tau)
+    got, ref, s = _xy_case(torch, spec, f, a, b, tau, 2, 1, steps=2)
+    assert _rel(got, ref) <= TOL
+    m0, m1 = oracle.mass(spec, f), float(s.mass().cpu()[0])
+    assert abs(m1 - m0) <= 1e-13 * abs(m0)
+
+
+def test_zero_and_constant_velocity(torch):
+    spec = GridSpec(n=(6, 5, 1, 4), order=(2, 2, 1, 2), lo=(0, 0, 0, 0), hi=(3.0, 2.5, 1, 1))
+    rng = np.random.default_rng(9)
+    f = rng.standard_normal(spec.shape)
+    z = np.zeros((1, 6, 7))
+    got, ref, _ = _xy_case(torch, spec, f, z, z, 0.3, 2, 1)
+    assert np.abs(got - f).max() < 1e-14
+    # integer Courant numbers in x and y: pure roll of cells (to round-off)
+    a = np.full((1, 6, 7), 2 * spec.h[0])
+    b = np.full((1, 6, 7), -1 * spec.h[1])
+    got, ref, _ = _xy_case(torch, spec, f, a, b, 1.0, 1, 1)
+    Nz, Nv, Ny, Nx = spec.shape
+    roll = np.roll(np.roll(f.reshape(Nz, Nv, 5, 2, 6, 2), 2, axis=4), -1, axis=2).reshape(spec.shape)
+    assert np.abs(got - roll).max() < 1e-13
+    assert _rel(got, ref) <= TOL
+
+
+def test_config0_tiny_itg_20_strang_steps(torch):
+    """BASELINE.json configs[0]: 16x16x8x16 cells, o=2, dt=2, 20 Strang steps; parity and mass."""
+    spec = inputs.itg_grid(16, 16, 8, 16, 2)
+    f = inputs.itg_initial_f(spec)
+    dt = 2.0
+    a, b, Ez, _ = inputs.itg_fields(spec, dt, 0.8)
+    s = _sldg(spec)
+    s.import_state(_dev(torch, f))
+    s.set_Ez(_dev(torch, Ez))
+    s.set_vxy(_dev(torch, a), _dev(torch, b), 1)
+    ref = f.copy()
+    m0 = oracle.mass(spec, f)
+    assert abs(float(s.mass().cpu()[0]) - m0) <= 1e-14 * m0
+    for n in range(20):
+        s.strang_step(dt)
+        oracle.strang_step(spec, ref, Ez, a, b, dt, 2, 1)
+        m = float(s.mass().cpu()[0])
+        assert abs(m - m0) <= 1e-13 * m0, (n, m, m0)
+    got = s.export_state().cpu().numpy()
+    s.check()
+    assert _rel(got, ref) <= TOL
+    rho = s.charge_density().cpu().numpy()
+    assert _rel(rho, oracle.charge_density(spec, ref)) <= TOL
+    ms = s.last_timing_ms()
+    assert all(t > 0 for t in ms[:6]) and ms[7] >= max(ms[:6])
+    assert s.launch_count() >= 20 * 6
+
+
+def test_layouts_agree_bitwise_on_a_strang_step(torch):
+    spec = inputs.itg_grid(8, 8, 4, 8, 2)
+    f = inputs.itg_initial_f(spec)
+    a, b, Ez, _ = inputs.itg_fields(spec, 2.0, 0.8)
+    outs = []
+    for layout in (1, 2, 3):
+        s = _sldg(spec, layout)
+        s.import_state(_dev(torch, f))
+        s.set_Ez(_dev(torch, Ez))
+        s.set_vxy(_dev(torch, a), _dev(torch, b), 1)
+        s.strang_step(2.0)
+        outs.append(s.export_state().cpu().numpy())
+        s.check()
+    assert np.array_equal(outs[0], outs[1]) and np.array_equal(outs[0], outs[2])
+
+
+def test_strang_step_host_entry_point(torch):
+    spec = inputs.itg_grid(8, 8, 4, 8, 2)
+    f = inputs.itg_initial_f(spec)
+    a, b, Ez, _ = inputs.itg_fields(spec, 2.0, 0.8)
+    s = _sldg(spec)
+    s.import_state_host(f)
+    rho = np.empty((spec.shape[0], spec.shape[2], spec.shape[3]))
+    mass = np.empty(1)
+    s.strang_step_host(2.0, Ez, a, b, 1, rho, mass)
+    ref = oracle.strang_step(spec, f.copy(), Ez, a, b, 2.0, 2, 1)
+    assert _rel(rho, oracle.charge_density(spec, ref)) <= TOL
+    assert abs(mass[0] - oracle.mass(spec, ref)) <= 1e-13 * abs(mass[0])
+    out = np.empty_like(f)
+    s.export_state_host(out)
+    assert _rel(out, ref) <= TOL
+
+
+def test_geometry_error_words(torch):
+    from paper_2212_03036_b200.binding import SLDG_ESTENCIL, SldgError
+    spec = GridSpec(n=(8, 8, 1, 2), order=(2, 2, 1, 1), lo=(0, 0, 0, 0), hi=(1, 1, 1, 1))
+    s = _sldg(spec)
+    s.import_state(_dev(torch, np.zeros(spec.shape)))
+    # a shear so strong that upstream cells span more than three source cells
+    a = np.zeros((1, 9, 9))
+    a[0] = (np.arange(9)[:, None] * 5.0) * spec.h[0]
+    s.set_vxy(_dev(torch, a), _dev(torch, np.zeros((1, 9, 9))), 0)
+    s.advect_xy(1.0, 1)
+    with pytest.raises(SldgError) as ei:
+        s.check()
+    assert ei.value.code == SLDG_ESTENCIL
+    s.check()  # cleared
