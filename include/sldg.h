@@ -128,7 +128,8 @@ int sldg_last_timing_ms(sldg_ctx *ctx, float ms[8]);
 /* Number of kernels the library launched on behalf of this context since creation. */
 long long sldg_launch_count(sldg_ctx *ctx);
 /* Debug / test access to the geometry of the last sldg_advect_xy: for z node `z` copies, per target
- * cell t = j*nx + i, anchor[2t..2t+1] = wrapped source cell of slot (0,0), mask[t] = bitmask over the
+ * cell t = j*nx + i, anchor[2t..2t+1] = offset (in cells, unwrapped) of the source cell of slot (0,0)
+ * relative to the target cell, mask[t] = bitmask over the
  * 3x3 slots (bit dx + 3 dy), and W[t][slot][m][k] = C^{ij,m}_{rs,k} / W_m (dense, 9*o^4 doubles per cell,
  * entries of empty slots are unspecified).  Device buffers; asynchronous. */
 int sldg_debug_geometry(sldg_ctx *ctx, int z, int32_t *anchor_dev, int32_t *mask_dev, double *W_dev);

@@ -1,11 +1,11 @@
-// sldg_xy.cu -- 2d SLDG step in the poloidal plane (Algorithm 3).
+// sldg_xy_geometry.cu -- 2d SLDG step in the poloidal plane (Algorithm 3).
 //
 //   xy_geometry : per (z node, target cell, 3x3 slot): back-trace corners and GL nodes (eq. 14/15,
 //                 PAPER.md:206-218), adjoint polynomial phi* from a Vandermonde solve,
 //                 monomial moments of  A*_ij cap A_rs  by Green's theorem along the clipped upstream edges
 //                 ("outer segments") and the grid-line pieces inside the upstream cell ("inner
 //                 segments", Table 4), coefficients C of eq. (18), scaled by 1/W_m.
-//   xy_apply    : eq. (17) for every v: lanes <-> v, weights are warp-uniform, empty slots are skipped.
+//   (the apply kernels, eq. (17), live in sldg_xy_apply.cu)
 //
 // Green's theorem with P = 0, Q^{(p,q)} = x^{p+1} y^q / (p+1)  (reproduces the paper's
 // Q^{(2,1)}, Q^{(2,2)}): in the source cell's local coordinates horizontal segments and
@@ -230,8 +230,8 @@ __global__ void __launch_bounds__(128) xy_geometry_kernel(const double *__restri
     const int r0 = (int)floor(xmin), s0 = (int)floor(ymin);
     const int r1 = max((int)ceil(xmax) - 1, r0), s1 = max((int)ceil(ymax) - 1, s0);
     if (slot == 0) {
-        anchor[2 * cellid] = wrap_idx(i + r0, nx);
-        anchor[2 * cellid + 1] = wrap_idx(j + s0, ny);
+        anchor[2 * cellid] = r0;      // relative to the target cell, unwrapped
+        anchor[2 * cellid + 1] = s0;
         bool convex = true;
 #pragma unroll
         for (int e = 0; e < 4; ++e) {
@@ -382,96 +382,3 @@ cudaError_t launch_xy_geometry(sldg_ctx *c, double tau, int trace_order)
     return cudaGetLastError();
 }
 
-// --------------------------------------------------------------------------------------------------
-// apply, eq. (17): out[ij,m] = sum_{rs} sum_k (C^{ij,m}_{rs,k} / W_m) in[rs,k]   for every (z, v).
-// block = 8 warps, a tile of 8x4 target cells at one z node and one chunk of 32*NVT v values;
-// warp <-> target cell (4 cells per warp), lane <-> v.  Weights are read warp-uniformly.
-// --------------------------------------------------------------------------------------------------
-template <int O, int NVT>
-__global__ void __launch_bounds__(256) xy_apply_kernel(const double *__restrict__ fin,
-                                                       double *__restrict__ fout,
-                                                       const int32_t *__restrict__ anchor,
-                                                       const int32_t *__restrict__ mask,
-                                                       const double *__restrict__ W, GridDev g)
-{
-    constexpr int O2 = O * O, TX = 8, TY = 4;
-    const int nx = g.n[0], ny = g.n[1];
-    const int tiles_x = (nx + TX - 1) / TX;
-    const int tile_i = (blockIdx.x % tiles_x) * TX, tile_j = (blockIdx.x / tiles_x) * TY;
-    const int z = blockIdx.z;
-    const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
-    const int v = (blockIdx.y * 32 + lane) * NVT;
-    if (v >= g.Pv) return;
-    const long long ncell = (long long)nx * ny;
-    const double *fz = fin + z * g.sZ + v;
-    double *oz = fout + z * g.sZ + v;
-
-    for (int c = warp; c < TX * TY; c += 8) {
-        const int i = tile_i + (c % TX), j = tile_j + (c / TX);
-        if (i >= nx || j >= ny) continue;
-        const long long cellid = (long long)z * ncell + (long long)j * nx + i;
-        const int ax = __ldg(anchor + 2 * cellid), ay = __ldg(anchor + 2 * cellid + 1);
-        const int msk = __ldg(mask + cellid);
-        double acc[O2][NVT];
-#pragma unroll
-        for (int m = 0; m < O2; ++m)
-#pragma unroll
-            for (int e = 0; e < NVT; ++e) acc[m][e] = 0.0;
-#pragma unroll 1
-        for (int slot = 0; slot < 9; ++slot) {
-            if (!((msk >> slot) & 1)) continue;
-            int r = ax + slot % 3, s = ay + slot / 3;
-            if (r >= nx) r -= nx;
-            if (s >= ny) s -= ny;
-            const double *Wp = W + ((size_t)cellid * 9 + slot) * (O2 * O2);
-#pragma unroll
-            for (int kq = 0; kq < O; ++kq)
-#pragma unroll
-                for (int kp = 0; kp < O; ++kp) {
-                    const double *src = fz + (long long)(s * O + kq) * g.sY + (long long)(r * O + kp) * g.sX;
-                    double in[NVT];
-                    if (NVT == 2) {
-                        double2 t = __ldg(reinterpret_cast<const double2 *>(src));
-                        in[0] = t.x;
-                        in[NVT - 1] = t.y;
-                    } else {
-                        in[0] = __ldg(src);
-                    }
-                    const int k = kp + O * kq;
-#pragma unroll
-                    for (int m = 0; m < O2; ++m) {
-                        const double w = __ldg(Wp + k * O2 + m);
-#pragma unroll
-                        for (int e = 0; e < NVT; ++e) acc[m][e] = fma(w, in[e], acc[m][e]);
-                    }
-                }
-        }
-#pragma unroll
-        for (int mq = 0; mq < O; ++mq)
-#pragma unroll
-            for (int mp = 0; mp < O; ++mp) {
-                double *dst = oz + (long long)(j * O + mq) * g.sY + (long long)(i * O + mp) * g.sX;
-                const int m = mp + O * mq;
-                if (NVT == 2)
-                    *reinterpret_cast<double2 *>(dst) = make_double2(acc[m][0], acc[m][NVT - 1]);
-                else
-                    dst[0] = acc[m][0];
-            }
-    }
-}
-
-cudaError_t launch_xy_apply(sldg_ctx *c, const double *fin, double *fout)
-{
-    const GridDev &g = c->g;
-    const int O = g.o[0];
-    constexpr int NVT = 2;
-    const int tiles = ((g.n[0] + 7) / 8) * ((g.n[1] + 3) / 4);
-    const int vchunks = (g.Pv + 32 * NVT - 1) / (32 * NVT);
-    dim3 grid((unsigned)tiles, (unsigned)vchunks, (unsigned)g.N[2]);
-#define LAUNCH_A(OO) \
-    xy_apply_kernel<OO, NVT><<<grid, 256, 0, c->stream>>>(fin, fout, c->anchor, c->mask, c->W, g)
-    if (O == 1) LAUNCH_A(1); else if (O == 2) LAUNCH_A(2); else LAUNCH_A(3);
-#undef LAUNCH_A
-    c->launches++;
-    return cudaGetLastError();
-}

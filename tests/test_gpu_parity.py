@@ -197,7 +197,7 @@ def test_xy_geometry_matches_oracle_coefficients(torch, o, trace_order):
             seen = 0
             for e in range(offs[t], offs[t + 1]):
                 r, c = er[e] % nx, es[e] % ny
-                dx, dy = (r - anchor[t, 0]) % nx, (c - anchor[t, 1]) % ny
+                dx, dy = (r - (t % nx + anchor[t, 0])) % nx, (c - (t // nx + anchor[t, 1])) % ny
                 assert dx < 3 and dy < 3
                 slot = dx + 3 * dy
                 ref = (eC[e] / Wm[:, None]).T.reshape(-1)  # k-major [k][m]
@@ -209,7 +209,9 @@ def test_xy_geometry_matches_oracle_coefficients(torch, o, trace_order):
                 else:
                     assert np.abs(ref).max() < 1e-13  # empty on the GPU <=> zero-area piece
             assert seen == mask[t]
-        assert worst < 1e-12 * scale
+        # Green boundary integrals lose ~1e-16 absolute per O(1) edge term; times the adjoint coefficients and
+        # 1/W_m (up to 13 at o=3) this is a few 1e-12 per block at o=3, ~1e-14 at o=2 (tolerances)
+        assert worst < (1e-13 if o == 2 else 5e-12) * scale, (worst, scale)
         assert np.abs(col - Wm).max() < 5e-14
 
 
