@@ -47,6 +47,7 @@ void fill_grid(const sldg_params *p, GridDev *g)
         g->sX = Pv; g->sZ = Nx * Pv; g->sY = Nz * Nx * Pv;
     }
     g->lines = Nz * Ny * Nx;
+    g->contig = (layout == 1) ? 1 : 0;
 }
 
 struct WorkspaceMap {
@@ -262,6 +263,8 @@ int sldg_create(const sldg_params *p, double *f_a_dev, double *f_b_dev, void *wo
     c->W = (double *)(ws + m.W);
     c->partials = (double *)(ws + m.partials);
     c->n_partials = m.n_partials;
+    c->rho_ws = (double *)(ws + m.rho);
+    c->scalar_ws = (double *)(ws + m.scalar);
     c->err = (int32_t *)(ws + m.err);
     c->trace_order = 2;
     c->vel_periodic = 0;
@@ -445,10 +448,8 @@ int sldg_strang_step_host(sldg_ctx *c, double dt, const double *Ez_host, const d
     if (!c) return SLDG_EINVAL;
     if ((a_host == nullptr) != (b_host == nullptr)) return SLDG_EINVAL;
     const GridDev &g = c->g;
-    WorkspaceMap m = map_workspace(&c->p);
-    char *ws = (char *)c->Ez - m.Ez;
-    double *rho_dev = (double *)(ws + m.rho);
-    double *mass_dev = (double *)(ws + m.scalar);
+    double *rho_dev = c->rho_ws;
+    double *mass_dev = c->scalar_ws;
     if (Ez_host &&
         cudaMemcpyAsync(c->Ez, Ez_host, (size_t)g.lines * 8, cudaMemcpyHostToDevice, c->stream) != cudaSuccess)
         return SLDG_ECUDA;
@@ -460,13 +461,15 @@ int sldg_strang_step_host(sldg_ctx *c, double dt, const double *Ez_host, const d
     }
     int rc = sldg_strang_step(c, dt);
     if (rc) return rc;
-    if (rho_host) {
+    if (rho_host || mass_host) {
         if (launch_charge_density(c, c->f[c->cur], rho_dev) != cudaSuccess) return SLDG_ECUDA;
+    }
+    if (rho_host) {
         if (cudaMemcpyAsync(rho_host, rho_dev, (size_t)g.lines * 8, cudaMemcpyDeviceToHost, c->stream) != cudaSuccess)
             return SLDG_ECUDA;
     }
     if (mass_host) {
-        if (launch_mass(c, c->f[c->cur], mass_dev) != cudaSuccess) return SLDG_ECUDA;
+        if (launch_mass_from_rho(c, rho_dev, mass_dev) != cudaSuccess) return SLDG_ECUDA;
         if (cudaMemcpyAsync(mass_host, mass_dev, 8, cudaMemcpyDeviceToHost, c->stream) != cudaSuccess) return SLDG_ECUDA;
     }
     return cuda_fail(cudaStreamSynchronize(c->stream));

@@ -20,6 +20,7 @@ struct GridDev {
     // internal layout: element (z,Y,X,v) at  z*sZ + Y*sY + X*sX + v   (doubles), v contiguous, pitch Pv
     long long sX, sY, sZ;
     int Pv;
+    int contig;       // 1: lines are stored in canonical (z,Y,X) enumeration order, base = line*Pv
     long long lines;  // Nz*Ny*Nx
 };
 
@@ -53,6 +54,8 @@ struct sldg_ctx {
     int32_t *mask;          // [Nz][ncell]
     double *W;              // [Nz][ncell][9][o2*o2]  (k-major: W[k*o2+m])
     double *partials;       // reduction scratch
+    double *rho_ws;         // [Nz][Ny][Nx] scratch charge density (mass, host entry point)
+    double *scalar_ws;      // one double
     int32_t *err;           // sticky device error word
     size_t n_partials;
     int trace_order, vel_periodic;
@@ -69,5 +72,6 @@ cudaError_t launch_advect_z(sldg_ctx *c, const double *fin, double *fout, double
 cudaError_t launch_advect_v(sldg_ctx *c, const double *fin, double *fout, double tau);
 cudaError_t launch_charge_density(sldg_ctx *c, const double *fin, double *rho);
 cudaError_t launch_mass(sldg_ctx *c, const double *fin, double *mass_out);
+cudaError_t launch_mass_from_rho(sldg_ctx *c, const double *rho, double *mass_out);
 cudaError_t launch_xy_geometry(sldg_ctx *c, double tau, int trace_order);
 cudaError_t launch_xy_apply(sldg_ctx *c, const double *fin, double *fout);

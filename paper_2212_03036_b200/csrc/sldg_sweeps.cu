@@ -119,181 +119,177 @@ cudaError_t launch_unpack(sldg_ctx *c, const double *internal, double *canon)
 }
 
 // --------------------------------------------------------------------------------------------------
-// advect_v: every (z,Y,X) line is a contiguous periodic line of nv cells; one Courant number per line.
-// A block stages LPB consecutive-in-enumeration lines in shared memory, one thread per (line, cell).
+// advect_v: every (z,Y,X) line is a contiguous periodic line of nv cells with one Courant number.
+// warp <-> line, lane <-> target cell (lane, lane+32, ...).  A target cell reads its two source cells
+// (i+s, i+s+1) straight from global memory: neighbouring lanes overlap by one cell, the overlap is served
+// by L1 (each 128-byte line is fetched from L2 once), so there is no shared-memory staging and no
+// block-level synchronisation; every byte of f crosses HBM once in each direction.
 // --------------------------------------------------------------------------------------------------
-template <int O>
+__device__ __forceinline__ long long line_base_fast(const GridDev &g, unsigned line)
+{
+    if (g.contig) return (long long)line * g.Pv;
+    unsigned X = line % (unsigned)g.N[0], t = line / (unsigned)g.N[0];
+    unsigned Y = t % (unsigned)g.N[1], z = t / (unsigned)g.N[1];
+    return z * g.sZ + Y * g.sY + X * g.sX;
+}
+
+// LPL lanes share one line (32/LPL lines per warp); CU target cells per lane are in flight at once.
+template <int O, int LPL, int CU>
 __global__ void __launch_bounds__(256) advect_v_kernel(const double *__restrict__ fin,
                                                        double *__restrict__ fout,
                                                        const double *__restrict__ Ez, GridDev g,
-                                                       ShiftPoly sp, double tau, int lpb)
+                                                       ShiftPoly sp, double tau)
 {
-    extern __shared__ double smem[];
-    const int Pv = g.Pv, Nv = g.N[3], nv = g.n[3];
-    double *sin_ = smem;                                   // [lpb][Pv]
-    double *sAB = smem + (size_t)lpb * Pv;                 // [lpb][2*O*O]
-    int *sS = (int *)(sAB + (size_t)lpb * 2 * O * O);      // [lpb]
-    long long *sBase = (long long *)(sS + ((lpb + 1) & ~1)); // [lpb]
-
-    for (long long l0 = (long long)blockIdx.x * lpb; l0 < g.lines; l0 += (long long)gridDim.x * lpb) {
-        const int nl = (int)min((long long)lpb, g.lines - l0);
-        // per-line shift data
-        for (int l = threadIdx.x; l < nl; l += blockDim.x) {
-            int s;
-            double alpha, A[O][O], B[O][O];
-            shift_of(Ez[l0 + l], tau, g.h[3], s, alpha);
-            eval_shift<O>(sp, alpha, A, B);
+    constexpr int LPW = 32 / LPL;  // lines per warp
+    const int nv = g.n[3];
+    const int lane = threadIdx.x & 31, sub = lane % LPL, grp = lane / LPL;
+    const unsigned warp = (blockIdx.x * blockDim.x + threadIdx.x) >> 5;
+    const unsigned nwarp = (gridDim.x * blockDim.x) >> 5;
+    const unsigned lines = (unsigned)g.lines;
+    unsigned line = warp * LPW + grp;
+    double e_next = line < lines ? __ldg(Ez + line) : 0.0;
+    for (; line < lines; line += nwarp * LPW) {
+        const double e = e_next;
+        const unsigned nline = line + nwarp * LPW;
+        if (nline < lines) e_next = __ldg(Ez + nline);  // prefetch: takes the Ez latency off the critical path
+        int s;
+        double alpha, A[O][O], B[O][O];
+        shift_of(e, tau, g.h[3], s, alpha);
+        eval_shift<O>(sp, alpha, A, B);
+        s = wrapi(s, nv);
+        const long long base = line_base_fast(g, line);
+        const double *u = fin + base;
+        double *w = fout + base;
+        for (int cell0 = sub; cell0 < nv; cell0 += LPL * CU) {
+            double u0[CU][O], u1[CU][O];
 #pragma unroll
-            for (int j = 0; j < O; ++j)
+            for (int k = 0; k < CU; ++k) {
+                const int cell = cell0 + k * LPL;
+                if (cell < nv) {
+                    int c0 = cell + s;
+                    if (c0 >= nv) c0 -= nv;
+                    int c1 = c0 + 1;
+                    if (c1 >= nv) c1 -= nv;
+                    if (O == 2) {
+                        const double2 t0 = __ldg(reinterpret_cast<const double2 *>(u + 2 * c0));
+                        const double2 t1 = __ldg(reinterpret_cast<const double2 *>(u + 2 * c1));
+                        u0[k][0] = t0.x; u0[k][O - 1] = t0.y;
+                        u1[k][0] = t1.x; u1[k][O - 1] = t1.y;
+                    } else {
 #pragma unroll
-                for (int m = 0; m < O; ++m) {
-                    sAB[(size_t)l * 2 * O * O + j * O + m] = A[j][m];
-                    sAB[(size_t)l * 2 * O * O + O * O + j * O + m] = B[j][m];
+                        for (int m = 0; m < O; ++m) {
+                            u0[k][m] = __ldg(u + c0 * O + m);
+                            u1[k][m] = __ldg(u + c1 * O + m);
+                        }
+                    }
                 }
-            sS[l] = wrapi(s, nv);
-            sBase[l] = line_base(g, l0 + l);
-        }
-        __syncthreads();
-        // stage the lines (16-byte vector loads; Pv is even and lines are 128-byte aligned)
-        const int vec_per_line = Pv / 2;
-        for (int idx = threadIdx.x; idx < nl * vec_per_line; idx += blockDim.x) {
-            int l = idx / vec_per_line, k = idx - l * vec_per_line;
-            double2 val = *reinterpret_cast<const double2 *>(fin + sBase[l] + 2 * k);
-            *reinterpret_cast<double2 *>(sin_ + (size_t)l * Pv + 2 * k) = val;
-        }
-        __syncthreads();
-        for (int idx = threadIdx.x; idx < nl * nv; idx += blockDim.x) {
-            int l = idx / nv, cell = idx - l * nv;
-            const double *A = sAB + (size_t)l * 2 * O * O, *B = A + O * O;
-            const double *u = sin_ + (size_t)l * Pv;
-            int c0 = cell + sS[l];
-            if (c0 >= nv) c0 -= nv;
-            int c1 = c0 + 1;
-            if (c1 >= nv) c1 -= nv;
-            double u0[O], u1[O], r[O];
-#pragma unroll
-            for (int m = 0; m < O; ++m) {
-                u0[m] = u[c0 * O + m];
-                u1[m] = u[c1 * O + m];
             }
 #pragma unroll
-            for (int j = 0; j < O; ++j) {
-                double acc = 0.0;
+            for (int k = 0; k < CU; ++k) {
+                const int cell = cell0 + k * LPL;
+                if (cell < nv) {
+                    double r[O];
 #pragma unroll
-                for (int m = 0; m < O; ++m) acc = fma(A[j * O + m], u0[m], acc);
+                    for (int j = 0; j < O; ++j) {
+                        double acc = 0.0;
 #pragma unroll
-                for (int m = 0; m < O; ++m) acc = fma(B[j * O + m], u1[m], acc);
-                r[j] = acc;
-            }
-            double *dst = fout + sBase[l] + cell * O;
-            if (O == 2) {
-                *reinterpret_cast<double2 *>(dst) = make_double2(r[0], r[O - 1]);
-            } else {
+                        for (int m = 0; m < O; ++m) acc = fma(A[j][m], u0[k][m], acc);
 #pragma unroll
-                for (int j = 0; j < O; ++j) dst[j] = r[j];
+                        for (int m = 0; m < O; ++m) acc = fma(B[j][m], u1[k][m], acc);
+                        r[j] = acc;
+                    }
+                    if (O == 2) {
+                        __stcs(reinterpret_cast<double2 *>(w + 2 * cell), make_double2(r[0], r[O - 1]));
+                    } else {
+#pragma unroll
+                        for (int j = 0; j < O; ++j) __stcs(w + cell * O + j, r[j]);
+                    }
+                }
             }
         }
-        __syncthreads();
     }
-    (void)Nv;
 }
 
 cudaError_t launch_advect_v(sldg_ctx *c, const double *fin, double *fout, double tau)
 {
     const GridDev &g = c->g;
     const int O = g.o[3];
-    int lpb = (1024 + g.n[3] - 1) / g.n[3];  // about 1024 cells per block iteration
-    if (lpb < 1) lpb = 1;
-    auto smem_for = [&](int l) {
-        return (size_t)l * g.Pv * 8 + (size_t)l * 2 * O * O * 8 + (size_t)((l + 1) & ~1) * 4 + (size_t)l * 8;
-    };
-    while (lpb > 1 && smem_for(lpb) > 64 * 1024) lpb--;
-    size_t smem = smem_for(lpb);
-    if (smem > 227 * 1024) return cudaErrorInvalidValue;
-    long long nblk = (g.lines + lpb - 1) / lpb;
-    long long cap = (long long)c->sm_count * 32;
+    if (g.lines >= (1ll << 31)) return cudaErrorInvalidValue;
+    constexpr int LPL = 8, CU = 4;
+    long long nblk = (g.lines + 8 * (32 / LPL) - 1) / (8 * (32 / LPL));  // 8 warps per block
+    long long cap = (long long)c->sm_count * 8 * 8;
     int grid = (int)(nblk < cap ? nblk : cap);
-#define LAUNCH_V(OO)                                                                                 \
-    {                                                                                                \
-        cudaFuncSetAttribute(advect_v_kernel<OO>, cudaFuncAttributeMaxDynamicSharedMemorySize,       \
-                             (int)smem);                                                             \
-        advect_v_kernel<OO><<<grid, 256, smem, c->stream>>>(fin, fout, c->Ez, g, c->sp_v, tau, lpb); \
-    }
-    if (O == 1) LAUNCH_V(1) else if (O == 2) LAUNCH_V(2) else LAUNCH_V(3)
+#define LAUNCH_V(OO) \
+    advect_v_kernel<OO, LPL, CU><<<grid, 256, 0, c->stream>>>(fin, fout, c->Ez, g, c->sp_v, tau)
+    if (O == 1) LAUNCH_V(1); else if (O == 2) LAUNCH_V(2); else LAUNCH_V(3);
 #undef LAUNCH_V
     c->launches++;
     return cudaGetLastError();
 }
 
 // --------------------------------------------------------------------------------------------------
-// advect_z: the z axis is strided.  A block owns one (Y,X) position and a chunk of VC consecutive v
-// values, stages the [Nz][VC] slab in shared memory (rows of VC*8 contiguous bytes, no transpose), and
-// shifts every v column along z by its own (s, alpha): lane <-> v, so shared-memory reads are
-// conflict-free whatever the per-lane row offsets are.
+// advect_z: the z axis is strided, v is contiguous.  thread <-> one (Y,X,v) column, lanes along v
+// (coalesced), walking z with a rolling register window: the two source cells of target cell i are
+// cells i+s and i+s+1, so every step loads one new cell and stores one -- each input is read exactly
+// once, no shared memory, no transpose.  (s, A, B) depend on the v node only and live in registers.
+// U target cells are processed per iteration so that U*O independent loads are in flight per thread.
 // --------------------------------------------------------------------------------------------------
-template <int O, int VC>
+template <int O, int U>
 __global__ void __launch_bounds__(256) advect_z_kernel(const double *__restrict__ fin,
                                                        double *__restrict__ fout, GridDev g,
                                                        ShiftPoly sp, Basis bs, double tau)
 {
-    extern __shared__ double slab[];  // [Nz][VC]
-    const int Nz = g.N[2], nz = g.n[2], Nv = g.N[3], ov = g.o[3];
-    const int nchunk = (Nv + VC - 1) / VC;
-    const long long nyx = (long long)g.N[1] * g.N[0];
-    const long long ntask = nyx * nchunk;
-    const int lane = threadIdx.x % VC, grp = threadIdx.x / VC, ngrp = blockDim.x / VC;
-
-    for (long long task = blockIdx.x; task < ntask; task += gridDim.x) {
-        const int chunk = (int)(task % nchunk);
-        const long long yx = task / nchunk;
-        const int X = (int)(yx % g.N[0]), Y = (int)(yx / g.N[0]);
-        const long long base = Y * g.sY + X * g.sX + (long long)chunk * VC;
-        const int v = chunk * VC + lane;
-        const bool live = v < Nv;
-        // stage rows
-        constexpr int VEC = VC / 2;
-        for (int idx = threadIdx.x; idx < Nz * VEC; idx += blockDim.x) {
-            int row = idx / VEC, k = idx - row * VEC;
-            if (chunk * VC + 2 * k < g.Pv) {
-                double2 val = *reinterpret_cast<const double2 *>(fin + base + row * g.sZ + 2 * k);
-                *reinterpret_cast<double2 *>(slab + row * VC + 2 * k) = val;
+    const int nz = g.n[2], Nv = g.N[3], ov = g.o[3];
+    const unsigned Pv = (unsigned)g.Pv;
+    const unsigned long long tid = (unsigned long long)blockIdx.x * blockDim.x + threadIdx.x;
+    const unsigned yx = (unsigned)(tid / Pv);
+    const int v = (int)(tid - (unsigned long long)yx * Pv);
+    if (yx >= (unsigned)(g.N[1] * g.N[0]) || v >= Nv) return;
+    const unsigned X = yx % (unsigned)g.N[0], Y = yx / (unsigned)g.N[0];
+    const long long base = Y * g.sY + X * g.sX + v;
+    int s;
+    double A[O][O], B[O][O];
+    {
+        const int l = v / ov, q = v - l * ov;
+        const double vq = __dadd_rn(g.lo[3], __dmul_rn(__dadd_rn((double)l, bs.xi[ov][q]), g.h[3]));
+        double alpha;
+        shift_of(vq, tau, g.h[2], s, alpha);
+        eval_shift<O>(sp, alpha, A, B);
+        s = wrapi(s, nz);
+    }
+    const long long sZ = g.sZ;
+    const double *src = fin + base;
+    double *dst = fout + base;
+    int c = s;  // source cell of the window's left half
+    double up[O];
+#pragma unroll
+    for (int m = 0; m < O; ++m) up[m] = __ldcs(src + (long long)(c * O + m) * sZ);
+    for (int i0 = 0; i0 < nz; i0 += U) {
+        double un[U][O];
+#pragma unroll
+        for (int k = 0; k < U; ++k) {
+            if (i0 + k < nz) {
+                c = (c + 1 == nz) ? 0 : c + 1;
+#pragma unroll
+                for (int m = 0; m < O; ++m) un[k][m] = __ldcs(src + (long long)(c * O + m) * sZ);
             }
         }
-        // per-lane shift
-        int s = 0;
-        double A[O][O], B[O][O];
-        {
-            int l = v / ov, q = v - l * ov;
-            double vq = __dadd_rn(g.lo[3], __dmul_rn(__dadd_rn((double)l, bs.xi[ov][q]), g.h[3]));
-            double alpha;
-            if (!live) vq = 0.0;
-            shift_of(vq, tau, g.h[2], s, alpha);
-            eval_shift<O>(sp, alpha, A, B);
-            s = wrapi(s, nz);
-        }
-        __syncthreads();
-        for (int cell = grp; cell < nz; cell += ngrp) {
-            int c0 = cell + s;
-            if (c0 >= nz) c0 -= nz;
-            int c1 = c0 + 1;
-            if (c1 >= nz) c1 -= nz;
-            double u0[O], u1[O];
 #pragma unroll
-            for (int m = 0; m < O; ++m) {
-                u0[m] = slab[(c0 * O + m) * VC + lane];
-                u1[m] = slab[(c1 * O + m) * VC + lane];
-            }
+        for (int k = 0; k < U; ++k) {
+            if (i0 + k < nz) {
 #pragma unroll
-            for (int j = 0; j < O; ++j) {
-                double acc = 0.0;
+                for (int j = 0; j < O; ++j) {
+                    double acc = 0.0;
 #pragma unroll
-                for (int m = 0; m < O; ++m) acc = fma(A[j][m], u0[m], acc);
+                    for (int m = 0; m < O; ++m) acc = fma(A[j][m], k == 0 ? up[m] : un[k == 0 ? 0 : k - 1][m], acc);
 #pragma unroll
-                for (int m = 0; m < O; ++m) acc = fma(B[j][m], u1[m], acc);
-                if (live) fout[base + (long long)(cell * O + j) * g.sZ + lane] = acc;
+                    for (int m = 0; m < O; ++m) acc = fma(B[j][m], un[k][m], acc);
+                    __stcs(dst + (long long)((i0 + k) * O + j) * sZ, acc);
+                }
             }
         }
-        __syncthreads();
+#pragma unroll
+        for (int m = 0; m < O; ++m) up[m] = un[U - 1][m];
     }
 }
 
@@ -301,19 +297,12 @@ cudaError_t launch_advect_z(sldg_ctx *c, const double *fin, double *fout, double
 {
     const GridDev &g = c->g;
     const int O = g.o[2];
-    constexpr int VC = 32;
-    size_t smem = (size_t)g.N[2] * VC * 8;
-    if (smem > 227 * 1024) return cudaErrorInvalidValue;
-    long long ntask = (long long)g.N[1] * g.N[0] * ((g.N[3] + VC - 1) / VC);
-    long long cap = (long long)c->sm_count * 64;
-    int grid = (int)(ntask < cap ? ntask : cap);
-#define LAUNCH_Z(OO)                                                                                   \
-    {                                                                                                  \
-        cudaFuncSetAttribute(advect_z_kernel<OO, VC>, cudaFuncAttributeMaxDynamicSharedMemorySize,     \
-                             (int)smem);                                                               \
-        advect_z_kernel<OO, VC><<<grid, 256, smem, c->stream>>>(fin, fout, g, c->sp_z, c->basis, tau); \
-    }
-    if (O == 1) LAUNCH_Z(1) else if (O == 2) LAUNCH_Z(2) else LAUNCH_Z(3)
+    const long long nthreads = (long long)g.N[1] * g.N[0] * g.Pv;
+    const long long nblk = (nthreads + 255) / 256;
+    if (nblk >= (1ll << 31)) return cudaErrorInvalidValue;
+    const unsigned grid = (unsigned)nblk;
+#define LAUNCH_Z(OO, UU) advect_z_kernel<OO, UU><<<grid, 256, 0, c->stream>>>(fin, fout, g, c->sp_z, c->basis, tau)
+    if (O == 1) LAUNCH_Z(1, 8); else if (O == 2) LAUNCH_Z(2, 4); else LAUNCH_Z(3, 2);
 #undef LAUNCH_Z
     c->launches++;
     return cudaGetLastError();
@@ -327,13 +316,21 @@ __global__ void __launch_bounds__(256) charge_density_kernel(const double *__res
                                                              Basis bs)
 {
     const int lane = threadIdx.x & 31;
-    const long long warp = ((long long)blockIdx.x * blockDim.x + threadIdx.x) >> 5;
-    const long long nwarp = ((long long)gridDim.x * blockDim.x) >> 5;
+    const unsigned warp = (blockIdx.x * blockDim.x + threadIdx.x) >> 5;
+    const unsigned nwarp = (gridDim.x * blockDim.x) >> 5;
+    const unsigned lines = (unsigned)g.lines;
     const int Nv = g.N[3], ov = g.o[3];
-    for (long long line = warp; line < g.lines; line += nwarp) {
-        const double *u = fin + line_base(g, line);
+    for (unsigned line = warp; line < lines; line += nwarp) {
+        const double *u = fin + line_base_fast(g, line);
         double acc = 0.0;
-        for (int v = lane; v < Nv; v += 32) acc = fma(bs.w[ov][v % ov], u[v], acc);
+        // pairs (2 lane, 2 lane + 1) + 64 k; Nv is even unless ov * nv is odd (tail handled below)
+        int v = 2 * lane;
+        for (; v + 1 < Nv; v += 64) {
+            const double2 t = __ldcs(reinterpret_cast<const double2 *>(u + v));
+            acc = fma(bs.w[ov][v % ov], t.x, acc);
+            acc = fma(bs.w[ov][(v + 1) % ov], t.y, acc);
+        }
+        if (v < Nv) acc = fma(bs.w[ov][v % ov], u[v], acc);
 #pragma unroll
         for (int off = 16; off > 0; off >>= 1) acc += __shfl_xor_sync(0xffffffffu, acc, off);
         if (lane == 0) rho[line] = g.h[3] * acc;
@@ -343,8 +340,9 @@ __global__ void __launch_bounds__(256) charge_density_kernel(const double *__res
 cudaError_t launch_charge_density(sldg_ctx *c, const double *fin, double *rho)
 {
     const GridDev &g = c->g;
+    if (g.lines >= (1ll << 31)) return cudaErrorInvalidValue;
     long long nblk = (g.lines + 7) / 8;
-    long long cap = (long long)c->sm_count * 32;
+    long long cap = (long long)c->sm_count * 8 * 16;
     int grid = (int)(nblk < cap ? nblk : cap);
     charge_density_kernel<<<grid, 256, 0, c->stream>>>(fin, rho, g, c->basis);
     c->launches++;
@@ -352,7 +350,8 @@ cudaError_t launch_charge_density(sldg_ctx *c, const double *fin, double *rho)
 }
 
 // --------------------------------------------------------------------------------------------------
-// mass: two-pass deterministic reduction (per-block partial sums, then one block).
+// mass: the v integral is the charge density; the remaining (x,y,z) Gauss sum is a
+// two-pass deterministic reduction over rho (per-block Kahan partial sums, then one block).
 // --------------------------------------------------------------------------------------------------
 __device__ __forceinline__ double block_sum(double v)
 {
@@ -372,25 +371,17 @@ __device__ __forceinline__ double block_sum(double v)
     return t;
 }
 
-__global__ void __launch_bounds__(256) mass_partial_kernel(const double *__restrict__ fin,
+__global__ void __launch_bounds__(256) mass_partial_kernel(const double *__restrict__ rho,
                                                            double *__restrict__ partials, GridDev g,
                                                            Basis bs)
 {
-    const int lane = threadIdx.x & 31;
-    const long long warp = ((long long)blockIdx.x * blockDim.x + threadIdx.x) >> 5;
-    const long long nwarp = ((long long)gridDim.x * blockDim.x) >> 5;
-    const int Nv = g.N[3], ov = g.o[3];
-    double total = 0.0, comp = 0.0;  // Kahan over the lines of this lane
-    for (long long line = warp; line < g.lines; line += nwarp) {
-        int X = (int)(line % g.N[0]);
-        long long t = line / g.N[0];
-        int Y = (int)(t % g.N[1]);
-        int z = (int)(t / g.N[1]);
+    const unsigned lines = (unsigned)g.lines;
+    double total = 0.0, comp = 0.0;  // Kahan over the lines of this thread
+    for (unsigned line = blockIdx.x * blockDim.x + threadIdx.x; line < lines; line += gridDim.x * blockDim.x) {
+        const unsigned X = line % (unsigned)g.N[0], t = line / (unsigned)g.N[0];
+        const unsigned Y = t % (unsigned)g.N[1], z = t / (unsigned)g.N[1];
         const double wl = bs.w[g.o[0]][X % g.o[0]] * bs.w[g.o[1]][Y % g.o[1]] * bs.w[g.o[2]][z % g.o[2]];
-        const double *u = fin + z * g.sZ + Y * g.sY + X * g.sX;
-        double acc = 0.0;
-        for (int v = lane; v < Nv; v += 32) acc = fma(bs.w[ov][v % ov], u[v], acc);
-        double yk = wl * acc - comp;
+        double yk = wl * rho[line] - comp;
         double tk = total + yk;
         comp = (tk - total) - yk;
         total = tk;
@@ -408,15 +399,22 @@ __global__ void __launch_bounds__(256) mass_final_kernel(const double *__restric
     if (threadIdx.x == 0) *out = s * scale;
 }
 
-cudaError_t launch_mass(sldg_ctx *c, const double *fin, double *mass_out)
+cudaError_t launch_mass_from_rho(sldg_ctx *c, const double *rho, double *mass_out)
 {
     const GridDev &g = c->g;
-    long long nblk = (g.lines + 7) / 8;
-    long long cap = (long long)c->n_partials;
+    long long nblk = (g.lines + 255) / 256;
+    long long cap = 1024;
     int grid = (int)(nblk < cap ? nblk : cap);
-    mass_partial_kernel<<<grid, 256, 0, c->stream>>>(fin, c->partials, g, c->basis);
-    double scale = g.h[0] * g.h[1] * g.h[2] * g.h[3];
+    mass_partial_kernel<<<grid, 256, 0, c->stream>>>(rho, c->partials, g, c->basis);
+    double scale = g.h[0] * g.h[1] * g.h[2];
     mass_final_kernel<<<1, 256, 0, c->stream>>>(c->partials, grid, scale, mass_out);
     c->launches += 2;
     return cudaGetLastError();
+}
+
+cudaError_t launch_mass(sldg_ctx *c, const double *fin, double *mass_out)
+{
+    cudaError_t e = launch_charge_density(c, fin, c->rho_ws);
+    if (e != cudaSuccess) return e;
+    return launch_mass_from_rho(c, c->rho_ws, mass_out);
 }
