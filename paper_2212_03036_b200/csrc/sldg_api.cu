@@ -51,7 +51,7 @@ void fill_grid(const sldg_params *p, GridDev *g)
 }
 
 struct WorkspaceMap {
-    size_t Ez, va, vb, anchor, mask, W, partials, rho, scalar, err, total;
+    size_t Ez, va, vb, hdr, W, partials, rho, scalar, err, total;
     size_t n_partials;
 };
 
@@ -68,8 +68,7 @@ WorkspaceMap map_workspace(const sldg_params *p)
     m.Ez = take((size_t)g.lines * 8);
     m.va = take(Nz * vplane * 8);
     m.vb = take(Nz * vplane * 8);
-    m.anchor = take(Nz * ncell * 2 * 4);
-    m.mask = take(Nz * ncell * 4);
+    m.hdr = take(Nz * ncell * 16);
     m.W = take(Nz * ncell * 9 * o4 * 8);
     m.n_partials = 8192;
     m.partials = take(m.n_partials * 8);
@@ -258,8 +257,7 @@ int sldg_create(const sldg_params *p, double *f_a_dev, double *f_b_dev, void *wo
     c->Ez = (double *)(ws + m.Ez);
     c->va = (double *)(ws + m.va);
     c->vb = (double *)(ws + m.vb);
-    c->anchor = (int32_t *)(ws + m.anchor);
-    c->mask = (int32_t *)(ws + m.mask);
+    c->hdr = (int4 *)(ws + m.hdr);
     c->W = (double *)(ws + m.W);
     c->partials = (double *)(ws + m.partials);
     c->n_partials = m.n_partials;
@@ -278,7 +276,7 @@ int sldg_create(const sldg_params *p, double *f_a_dev, double *f_b_dev, void *wo
             return SLDG_ECUDA;
         }
     // fields default to zero, error word cleared
-    cudaError_t e = cudaMemsetAsync(ws + m.Ez, 0, m.anchor - m.Ez, c->stream);
+    cudaError_t e = cudaMemsetAsync(ws + m.Ez, 0, m.hdr - m.Ez, c->stream);
     if (e == cudaSuccess) e = cudaMemsetAsync(c->err, 0, 256, c->stream);
     if (e != cudaSuccess) {
         delete c;
@@ -517,16 +515,7 @@ long long sldg_launch_count(sldg_ctx *c) { return c ? c->launches : 0; }
 int sldg_debug_geometry(sldg_ctx *c, int z, int32_t *anchor_dev, int32_t *mask_dev, double *W_dev)
 {
     if (!c || z < 0 || z >= c->g.N[2]) return SLDG_EINVAL;
-    const size_t ncell = (size_t)c->g.n[0] * c->g.n[1];
-    const size_t o4 = (size_t)c->g.o[0] * c->g.o[0] * c->g.o[0] * c->g.o[0];
-    cudaError_t e = cudaSuccess;
-    if (anchor_dev)
-        e = cudaMemcpyAsync(anchor_dev, c->anchor + (size_t)z * ncell * 2, ncell * 8, cudaMemcpyDeviceToDevice, c->stream);
-    if (e == cudaSuccess && mask_dev)
-        e = cudaMemcpyAsync(mask_dev, c->mask + (size_t)z * ncell, ncell * 4, cudaMemcpyDeviceToDevice, c->stream);
-    if (e == cudaSuccess && W_dev)
-        e = cudaMemcpyAsync(W_dev, c->W + (size_t)z * ncell * 9 * o4, ncell * 9 * o4 * 8, cudaMemcpyDeviceToDevice, c->stream);
-    return cuda_fail(e);
+    return cuda_fail(launch_geometry_expand(c, z, anchor_dev, mask_dev, W_dev));
 }
 
 const char *sldg_strerror(int code)

@@ -50,9 +50,8 @@ struct sldg_ctx {
     int cur;
     // workspace carve-up
     double *Ez, *va, *vb;   // fields
-    int32_t *anchor;        // [Nz][ncell][2]
-    int32_t *mask;          // [Nz][ncell]
-    double *W;              // [Nz][ncell][9][o2*o2]  (k-major: W[k*o2+m])
+    int4 *hdr;              // [Nz][ncell] {anchor x, anchor y, slot mask, number of blocks}
+    double *W;              // [Nz][ncell][9][o2*o2]  (k-major: W[k*o2+m]), `count` blocks packed from 0
     double *partials;       // reduction scratch
     double *rho_ws;         // [Nz][Ny][Nx] scratch charge density (mass, host entry point)
     double *scalar_ws;      // one double
@@ -74,4 +73,5 @@ cudaError_t launch_charge_density(sldg_ctx *c, const double *fin, double *rho);
 cudaError_t launch_mass(sldg_ctx *c, const double *fin, double *mass_out);
 cudaError_t launch_mass_from_rho(sldg_ctx *c, const double *rho, double *mass_out);
 cudaError_t launch_xy_geometry(sldg_ctx *c, double tau, int trace_order);
+cudaError_t launch_geometry_expand(sldg_ctx *c, int z, int32_t *anchor, int32_t *mask, double *Wd);
 cudaError_t launch_xy_apply(sldg_ctx *c, const double *fin, double *fout);

@@ -96,8 +96,8 @@ struct StreamSmem {
 
 template <int RWC, int NR, int NW, int WCAP>
 __global__ void __launch_bounds__(STREAM_THREADS) xy_apply_stream_kernel(
-    const double *__restrict__ fin, double *__restrict__ fout, const int32_t *__restrict__ anchor,
-    const int32_t *__restrict__ mask, const double *__restrict__ W, GridDev g, int L)
+    const double *__restrict__ fin, double *__restrict__ fout, const int4 *__restrict__ hdrg,
+    const double *__restrict__ W, GridDev g, int L)
 {
     constexpr int TX = STREAM_TX;
     using SM = StreamSmem<RWC, NR, NW, WCAP>;
@@ -134,9 +134,7 @@ __global__ void __launch_bounds__(STREAM_THREADS) xy_apply_stream_kernel(
         int4 h = make_int4(0, 0, 0, 0);
         if (i0 + ci < nx) {
             const long long cellid = zc + (long long)(j0 + jr) * nx + i0 + ci;
-            h.x = __ldg(anchor + 2 * cellid);
-            h.y = __ldg(anchor + 2 * cellid + 1);
-            h.z = __ldg(mask + cellid);
+            h = __ldg(hdrg + cellid);
         }
         hdr[tid] = h;
         if (h.z) {
@@ -169,6 +167,7 @@ __global__ void __launch_bounds__(STREAM_THREADS) xy_apply_stream_kernel(
             const int gx = wrap_idx(i + h.x, nx), gy = wrap_idx(j + h.y, ny);
             for (int v = 2 * lane; v < VL; v += 64) {
                 double acc[4][2] = {};
+                int nb = 0;
 #pragma unroll 1
                 for (int slot = 0; slot < 9; ++slot) {
                     if (!((h.z >> slot) & 1)) continue;
@@ -180,7 +179,7 @@ __global__ void __launch_bounds__(STREAM_THREADS) xy_apply_stream_kernel(
                     for (int k = 0; k < 4; ++k)
                         in[k] = __ldg(reinterpret_cast<const double2 *>(
                             fz + (long long)(2 * s + (k >> 1)) * g.sY + (long long)(2 * r + (k & 1)) * g.sX + v));
-                    fma_block_o2(acc, in, W + ((size_t)cellid * 9 + slot) * 16);
+                    fma_block_o2(acc, in, W + ((size_t)cellid * 9 + nb++) * 16);
                 }
 #pragma unroll
                 for (int m = 0; m < 4; ++m)
@@ -233,19 +232,17 @@ __global__ void __launch_bounds__(STREAM_THREADS) xy_apply_stream_kernel(
             if (jr >= 0 && jr < rows) {
                 const int ws = jr % NW;
                 if (jr >= NW) mbar_wait(&wempty[ws], ((jr / NW) & 1) ^ 1);
-                const int ci = lane >> 3, n = lane & 7;   // 4 cells x 8 candidate blocks
-                const int4 h = hdr[jr * TX + ci];
-                const int cnt = __popc(h.z);
+                const int ci = lane;                      // one packed run of weight blocks per cell
+                const int cnt = ci < TX ? hdr[jr * TX + ci].w : 0;
                 int tot = cnt;
-                tot += __shfl_xor_sync(0xffffffffu, tot, 8);
-                tot += __shfl_xor_sync(0xffffffffu, tot, 16);
+#pragma unroll
+                for (int off = 1; off < TX; off <<= 1) tot += __shfl_xor_sync(0xffffffffu, tot, off);
                 if (lane == 0) mbar_arrive_expect_tx(&wfull[ws], (uint32_t)(tot * 128));
                 __syncwarp();
-                if (n < cnt) {
-                    const int slot = __fns(h.z, 0, n + 1);
+                if (cnt > 0) {
                     const long long cellid = zc + (long long)(j0 + jr) * nx + i0 + ci;
-                    bulk_g2s(wring + ((size_t)(ws * TX + ci) * WCAP + n) * 16, W + ((size_t)cellid * 9 + slot) * 16, 128,
-                             &wfull[ws]);
+                    bulk_g2s(wring + (size_t)(ws * TX + ci) * WCAP * 16, W + (size_t)cellid * 9 * 16,
+                             (uint32_t)(cnt * 128), &wfull[ws]);
                 }
             }
         }
@@ -305,8 +302,7 @@ __global__ void __launch_bounds__(STREAM_THREADS) xy_apply_stream_kernel(
 template <int O, int NVT>
 __global__ void __launch_bounds__(256) xy_apply_direct_kernel(const double *__restrict__ fin,
                                                               double *__restrict__ fout,
-                                                              const int32_t *__restrict__ anchor,
-                                                              const int32_t *__restrict__ mask,
+                                                              const int4 *__restrict__ hdrg,
                                                               const double *__restrict__ W, GridDev g)
 {
     constexpr int O2 = O * O, TX = 8, TY = 4;
@@ -325,9 +321,11 @@ __global__ void __launch_bounds__(256) xy_apply_direct_kernel(const double *__re
         const int i = tile_i + (c % TX), j = tile_j + (c / TX);
         if (i >= nx || j >= ny) continue;
         const long long cellid = (long long)z * ncell + (long long)j * nx + i;
-        const int ax = wrap_idx(i + __ldg(anchor + 2 * cellid), nx);
-        const int ay = wrap_idx(j + __ldg(anchor + 2 * cellid + 1), ny);
-        const int msk = __ldg(mask + cellid);
+        const int4 h = __ldg(hdrg + cellid);
+        const int ax = wrap_idx(i + h.x, nx);
+        const int ay = wrap_idx(j + h.y, ny);
+        const int msk = h.z;
+        int nb = 0;
         double acc[O2][NVT];
 #pragma unroll
         for (int m = 0; m < O2; ++m)
@@ -339,7 +337,7 @@ __global__ void __launch_bounds__(256) xy_apply_direct_kernel(const double *__re
             int r = ax + slot % 3, s = ay + slot / 3;
             if (r >= nx) r -= nx;
             if (s >= ny) s -= ny;
-            const double *Wp = W + ((size_t)cellid * 9 + slot) * (O2 * O2);
+            const double *Wp = W + ((size_t)cellid * 9 + nb++) * (O2 * O2);
 #pragma unroll
             for (int kq = 0; kq < O; ++kq)
 #pragma unroll
@@ -388,7 +386,7 @@ cudaError_t launch_xy_apply(sldg_ctx *c, const double *fin, double *fout)
         const int L = g.n[1] < STREAM_LMAX ? g.n[1] : STREAM_LMAX;
         const int strips = (g.n[0] + STREAM_TX - 1) / STREAM_TX, segs = (g.n[1] + L - 1) / L;
         dim3 grid((unsigned)(strips * segs), (unsigned)((g.Pv + STREAM_VMAX - 1) / STREAM_VMAX), (unsigned)g.N[2]);
-        kern<<<grid, STREAM_THREADS, SM::total, c->stream>>>(fin, fout, c->anchor, c->mask, c->W, g, L);
+        kern<<<grid, STREAM_THREADS, SM::total, c->stream>>>(fin, fout, c->hdr, c->W, g, L);
         c->launches++;
         return cudaGetLastError();
     }
@@ -397,7 +395,7 @@ cudaError_t launch_xy_apply(sldg_ctx *c, const double *fin, double *fout)
     const int vchunks = (g.Pv + 32 * NVT - 1) / (32 * NVT);
     dim3 grid((unsigned)tiles, (unsigned)vchunks, (unsigned)g.N[2]);
 #define LAUNCH_A(OO) \
-    xy_apply_direct_kernel<OO, NVT><<<grid, 256, 0, c->stream>>>(fin, fout, c->anchor, c->mask, c->W, g)
+    xy_apply_direct_kernel<OO, NVT><<<grid, 256, 0, c->stream>>>(fin, fout, c->hdr, c->W, g)
     if (O == 1) LAUNCH_A(1); else if (O == 2) LAUNCH_A(2); else LAUNCH_A(3);
 #undef LAUNCH_A
     c->launches++;

@@ -1,20 +1,32 @@
-// sldg_xy_geometry.cu -- 2d SLDG step in the poloidal plane (Algorithm 3).
+// sldg_xy_geometry.cu -- geometry of the 2d SLDG step in the poloidal plane (Algorithm 3
+// PAPER.md:287-293): everything of eq. (14)-(18) that does not depend on v.
 //
-//   xy_geometry : per (z node, target cell, 3x3 slot): back-trace corners and GL nodes (eq. 14/15,
-//                 PAPER.md:206-218), adjoint polynomial phi* from a Vandermonde solve,
-//                 monomial moments of  A*_ij cap A_rs  by Green's theorem along the clipped upstream edges
-//                 ("outer segments") and the grid-line pieces inside the upstream cell ("inner
-//                 segments", Table 4), coefficients C of eq. (18), scaled by 1/W_m.
+//   thread <-> one (z node, target cell).  Per cell, once:
+//     step 1  back-trace the four corners (eq. 14/15) -> upstream quadrilateral, its
+//             bounding box -> anchor (r0,s0) and the candidate source cells (Table 4 step 1);
+//     step 4  back-trace the o^2 Gauss-Legendre nodes, invert the Vandermonde matrix in centred
+//             coordinates -> adjoint polynomials phi*_m (Table 4 step 4);
+//   then per candidate source cell (<= 3x3):
+//     steps 2,3,5  monomial moments of  A*_ij cap A_rs  by Green's theorem along the clipped upstream
+//             edges ("outer segments") and the piece of the cell's right edge inside the upstream cell
+//             ("inner segments", Table 4 steps 2,3,5), contracted with the Lagrange basis
+//             and phi* into the coefficients C of eq. (18), stored as W = C / W_m.
 //   (the apply kernels, eq. (17), live in sldg_xy_apply.cu)
 //
-// Green's theorem with P = 0, Q^{(p,q)} = x^{p+1} y^q / (p+1)  (reproduces the paper's
+// Green's theorem with P = 0, Q^{(p,q)} = x^{p+1} y^q / (p+1)  (R7; reproduces the paper's
 // Q^{(2,1)}, Q^{(2,2)}): in the source cell's local coordinates horizontal segments and
 // segments on the cell's left edge x=0 contribute nothing; only the upstream edges and the pieces of the
 // cell's right edge x=1 inside the upstream cell do.
 //
 // All geometry is done in cell units relative to the target cell (the target is [0,1]^2), the integrals
-// in the source cell's own local coordinates.
+// in the source cell's own local coordinates (R10).
+//
+// Output per (z node, cell): header int4 {ax, ay, mask, count} (anchor = offset of slot (0,0) relative to
+// the target cell, unwrapped; mask over the 3x3 slots, bit dx + 3 dy) and `count` weight blocks of o^4
+// doubles, k-major (W[k*o2+m]), packed in increasing slot order at W[cell][0..count).
 #include "sldg_internal.cuh"
+
+namespace {
 
 __device__ __forceinline__ int wrap_idx(int i, int n)
 {
@@ -22,7 +34,7 @@ __device__ __forceinline__ int wrap_idx(int i, int n)
     return r < 0 ? r + n : r;
 }
 
-// piecewise-bilinear velocity of cell (ci,cj) at local (xi,eta), scaled to Courant units
+// piecewise-bilinear velocity of cell (ci,cj) at local (xi,eta)
 __device__ __forceinline__ void bilinear_vel(const double *__restrict__ a, const double *__restrict__ b,
                                              int pitch, int ci, int cj, double xi, double eta,
                                              double &ua, double &ub)
@@ -112,54 +124,57 @@ __device__ __forceinline__ double gauss_jordan(double (&V)[N][N], double (&X)[N]
     return minpiv;
 }
 
-// Monomial moments M[p][q] = int x^p y^q over (upstream quadrilateral) cap (unit cell), by Green's theorem.
-// (X,Y): quadrilateral corners counter-clockwise in the source cell's local coordinates.
-// inner_right: the grid line x_local = 1 lies strictly inside the quadrilateral's x-extent.
+// Per-cell description of the upstream quadrilateral's edges (corners counter-clockwise, target-cell
+// units): start point, direction and the reciprocals of the direction components (0 when the component is 0).
+struct QuadEdges {
+    double x0[4], y0[4], dx[4], dy[4], idx[4], idy[4];
+};
+
+// Monomial moments M[p][q] = int x^p y^q over (upstream quadrilateral) cap (source cell (r,s)), in that
+// cell's local coordinates, by Green's theorem.  inner_right: the grid line x_local = 1 lies inside the
+// quadrilateral's bounding box (r < r1).
 template <int O>
-__device__ __forceinline__ void piece_moments(const double (&X)[4], const double (&Y)[4],
-                                              bool inner_right, const Basis &bs,
-                                              double (&M)[2 * O - 1][2 * O - 1])
+__device__ __forceinline__ void piece_moments(const QuadEdges &q, double offx, double offy, bool inner_right,
+                                              const Basis &bs, double (&M)[2 * O - 1][2 * O - 1])
 {
     constexpr int NM = 2 * O - 1;
 #pragma unroll
     for (int p = 0; p < NM; ++p)
 #pragma unroll
-        for (int q = 0; q < NM; ++q) M[p][q] = 0.0;
+        for (int qq = 0; qq < NM; ++qq) M[p][qq] = 0.0;
     double ylo = 1e300, yhi = -1e300;
 #pragma unroll
     for (int e = 0; e < 4; ++e) {
-        const double x0 = X[e], y0 = Y[e], x1 = X[(e + 1) & 3], y1 = Y[(e + 1) & 3];
-        const double dx = x1 - x0, dy = y1 - y0;
-        // crossing with the line x = 1 (for the inner segment)
+        const double x0 = q.x0[e] - offx, y0 = q.y0[e] - offy;
+        const double dx = q.dx[e], dy = q.dy[e];
+        // crossing with the line x = 1 (for the inner segment); decided from the actual end points
+        const double x1 = q.x0[(e + 1) & 3] - offx;
         if (inner_right && dx != 0.0 && (x0 - 1.0) * (x1 - 1.0) <= 0.0) {
-            double yc = fma((1.0 - x0) / dx, dy, y0);
+            const double yc = fma(fmin(fmax((1.0 - x0) * q.idx[e], 0.0), 1.0), dy, y0);
             ylo = fmin(ylo, yc);
             yhi = fmax(yhi, yc);
         }
         // outer segment: Liang-Barsky clip of the edge against the closed unit square
         double t0 = 0.0, t1 = 1.0;
-        bool ok = true;
-        {
-            const double pp[4] = {-dx, dx, -dy, dy};
-            const double qq[4] = {x0, 1.0 - x0, y0, 1.0 - y0};
-#pragma unroll
-            for (int k = 0; k < 4; ++k) {
-                if (pp[k] == 0.0) {
-                    if (qq[k] < 0.0) ok = false;
-                } else {
-                    double r = qq[k] / pp[k];
-                    if (pp[k] < 0.0)
-                        t0 = fmax(t0, r);
-                    else
-                        t1 = fmin(t1, r);
-                }
-            }
+        bool ok = dy != 0.0;  // horizontal edges contribute nothing (dy = 0 in the line integral)
+        if (dx == 0.0) {
+            ok = ok && x0 >= 0.0 && x0 <= 1.0;
+        } else {
+            const double ta = -x0 * q.idx[e], tb = (1.0 - x0) * q.idx[e];
+            t0 = fmax(t0, fmin(ta, tb));
+            t1 = fmin(t1, fmax(ta, tb));
         }
-        if (ok && t1 > t0 && dy != 0.0) {
+        {
+            const double ta = -y0 * q.idy[e], tb = (1.0 - y0) * q.idy[e];
+            t0 = fmax(t0, fmin(ta, tb));
+            t1 = fmin(t1, fmax(ta, tb));
+        }
+        if (ok && t1 > t0) {
             const double xa = fmin(fmax(fma(t0, dx, x0), 0.0), 1.0), ya = fmin(fmax(fma(t0, dy, y0), 0.0), 1.0);
             const double xb = fmin(fmax(fma(t1, dx, x0), 0.0), 1.0), yb = fmin(fmax(fma(t1, dy, y0), 0.0), 1.0);
             const double ex = xb - xa, ey = yb - ya;
-            for (int gq = 0; gq < bs.nq; ++gq) {
+#pragma unroll
+            for (int gq = 0; gq < NM; ++gq) {  // (2o-1)-point Gauss rule: exact for degree 4o-3
                 const double t = bs.qx[gq];
                 const double x = fma(t, ex, xa), y = fma(t, ey, ya);
                 const double wgt = bs.qw[gq] * ey;
@@ -168,8 +183,8 @@ __device__ __forceinline__ void piece_moments(const double (&X)[4], const double
                 for (int p = 0; p < NM; ++p) {
                     double term = wgt * xp * (1.0 / (p + 1));
 #pragma unroll
-                    for (int q = 0; q < NM; ++q) {
-                        M[p][q] += term;
+                    for (int qq = 0; qq < NM; ++qq) {
+                        M[p][qq] += term;
                         term *= y;
                     }
                     xp *= x;
@@ -182,10 +197,10 @@ __device__ __forceinline__ void piece_moments(const double (&X)[4], const double
         if (yb > ya) {
             double pa = ya, pb = yb;  // y^{q+1}
 #pragma unroll
-            for (int q = 0; q < NM; ++q) {
-                const double seg = (pb - pa) * (1.0 / (q + 1));
+            for (int qq = 0; qq < NM; ++qq) {
+                const double seg = (pb - pa) * (1.0 / (qq + 1));
 #pragma unroll
-                for (int p = 0; p < NM; ++p) M[p][q] += seg * (1.0 / (p + 1));
+                for (int p = 0; p < NM; ++p) M[p][qq] += seg * (1.0 / (p + 1));
                 pa *= ya;
                 pb *= yb;
             }
@@ -194,24 +209,20 @@ __device__ __forceinline__ void piece_moments(const double (&X)[4], const double
 }
 
 template <int O>
-__global__ void __launch_bounds__(128) xy_geometry_kernel(const double *__restrict__ va,
-                                                          const double *__restrict__ vb,
-                                                          int32_t *__restrict__ anchor,
-                                                          int32_t *__restrict__ mask,
-                                                          double *__restrict__ W, int32_t *err,
-                                                          GridDev g, Basis bs, double tau, int order,
-                                                          int periodic)
+__global__ void __launch_bounds__(O == 3 ? 64 : 128) xy_geometry_kernel(const double *__restrict__ va,
+                                                                         const double *__restrict__ vb,
+                                                                         int4 *__restrict__ hdr,
+                                                                         double *__restrict__ W, int32_t *err,
+                                                                         GridDev g, Basis bs, double tau, int order,
+                                                                         int periodic)
 {
     constexpr int O2 = O * O, NM = 2 * O - 1;
     const int nx = g.n[0], ny = g.n[1];
-    const long long ncell = (long long)nx * ny;
-    const long long total = (long long)g.N[2] * ncell * 9;
-    const long long gid = (long long)blockIdx.x * blockDim.x + threadIdx.x;
-    if (gid >= total) return;
-    const int slot = (int)(gid % 9);
-    const long long cellid = gid / 9;
-    const int z = (int)(cellid / ncell);
-    const int t = (int)(cellid % ncell);
+    const int ncell = nx * ny;
+    const int t = blockIdx.x * blockDim.x + threadIdx.x;
+    if (t >= ncell) return;
+    const int z = blockIdx.y;
+    const long long cellid = (long long)z * ncell + t;
     const int i = t % nx, j = t / nx;
     const long long vplane = (long long)(ny + 1) * (nx + 1);
     const double *a = va + z * vplane, *b = vb + z * vplane;
@@ -224,161 +235,230 @@ __global__ void __launch_bounds__(128) xy_geometry_kernel(const double *__restri
     trace_point(a, b, nx, ny, tx, ty, i, j, 1.0, 1.0, order, periodic, cx[2], cy[2]);
     trace_point(a, b, nx, ny, tx, ty, i, j, 0.0, 1.0, order, periodic, cx[3], cy[3]);
     const double xmin = fmin(fmin(cx[0], cx[1]), fmin(cx[2], cx[3]));
-    const double xmax = fmax(fmax(cx[0], cx[1]), fmax(cx[2], cx[3]));
     const double ymin = fmin(fmin(cy[0], cy[1]), fmin(cy[2], cy[3]));
-    const double ymax = fmax(fmax(cy[0], cy[1]), fmax(cy[2], cy[3]));
     const int r0 = (int)floor(xmin), s0 = (int)floor(ymin);
-    const int r1 = max((int)ceil(xmax) - 1, r0), s1 = max((int)ceil(ymax) - 1, s0);
-    if (slot == 0) {
-        anchor[2 * cellid] = r0;      // relative to the target cell, unwrapped
-        anchor[2 * cellid + 1] = s0;
+    int nr, ns;  // the bounding box covers source cells r0 .. r0+nr, s0 .. s0+ns
+    QuadEdges q;
+    {
+        // Corners relative to the anchor cell (keeps |coordinates| <= 4).  Everything below -- edge
+        // directions, clip parameters, crossings -- is derived from these rounded coordinates only, so
+        // that the clipped pieces of neighbouring source cells fit together exactly.
+#pragma unroll
+        for (int e = 0; e < 4; ++e) {
+            q.x0[e] = cx[e] - r0;
+            q.y0[e] = cy[e] - s0;
+        }
         bool convex = true;
 #pragma unroll
         for (int e = 0; e < 4; ++e) {
-            double e1x = cx[(e + 1) & 3] - cx[e], e1y = cy[(e + 1) & 3] - cy[e];
-            double e2x = cx[(e + 2) & 3] - cx[(e + 1) & 3], e2y = cy[(e + 2) & 3] - cy[(e + 1) & 3];
+            const double e1x = q.x0[(e + 1) & 3] - q.x0[e], e1y = q.y0[(e + 1) & 3] - q.y0[e];
+            const double e2x = q.x0[(e + 2) & 3] - q.x0[(e + 1) & 3], e2y = q.y0[(e + 2) & 3] - q.y0[(e + 1) & 3];
             if (!(e1x * e2y - e1y * e2x > 0.0)) convex = false;
+            q.dx[e] = e1x;
+            q.dy[e] = e1y;
+            q.idx[e] = e1x != 0.0 ? 1.0 / e1x : 0.0;
+            q.idy[e] = e1y != 0.0 ? 1.0 / e1y : 0.0;
         }
         if (!convex) atomicMin(err, SLDG_EGEOM);
-        if (r1 - r0 > 2 || s1 - s0 > 2) atomicMin(err, SLDG_ESTENCIL);
-    }
-    const int dr = slot % 3, ds = slot / 3;
-    if (dr > r1 - r0 || ds > s1 - s0) return;
-    const int r = r0 + dr, s = s0 + ds;
-
-    // moments of the piece in the source cell's local coordinates
-    double X[4], Y[4];
-#pragma unroll
-    for (int k = 0; k < 4; ++k) {
-        X[k] = cx[k] - r;
-        Y[k] = cy[k] - s;
-    }
-    double M[NM][NM];
-    piece_moments<O>(X, Y, r < r1, bs, M);
-    if (!(M[0][0] > 0.0)) return;  // empty intersection
-
-    // step 2: node feet and adjoint polynomial (centred monomials, then shifted to local monomials)
-    double fx[O2], fy[O2], xc = 0.0, yc = 0.0;
-#pragma unroll
-    for (int q = 0; q < O; ++q)
-#pragma unroll
-        for (int p = 0; p < O; ++p) {
-            double px, py;
-            trace_point(a, b, nx, ny, tx, ty, i, j, bs.xi[O][p], bs.xi[O][q], order, periodic, px, py);
-            fx[p + O * q] = px - r;
-            fy[p + O * q] = py - s;
-            xc += px - r;
-            yc += py - s;
+        // half-open bounding box, taken from the same rounded coordinates (a foot exactly on a grid line
+        // does not add a zero-area column, R12)
+        const double xmax = fmax(fmax(q.x0[0], q.x0[1]), fmax(q.x0[2], q.x0[3]));
+        const double ymax = fmax(fmax(q.y0[0], q.y0[1]), fmax(q.y0[2], q.y0[3]));
+        nr = max((int)ceil(xmax) - 1, 0);
+        ns = max((int)ceil(ymax) - 1, 0);
+        if (nr > 2 || ns > 2) {
+            atomicMin(err, SLDG_ESTENCIL);
+            nr = min(nr, 2);
+            ns = min(ns, 2);
         }
-    xc *= 1.0 / O2;
-    yc *= 1.0 / O2;
-    double V[O2][O2], Vi[O2][O2];
-#pragma unroll
-    for (int m = 0; m < O2; ++m) {
-        double py = 1.0;
-#pragma unroll
-        for (int bq = 0; bq < O; ++bq) {
-            double px = 1.0;
-#pragma unroll
-            for (int bp = 0; bp < O; ++bp) {
-                V[m][bp + O * bq] = px * py;
-                px *= fx[m] - xc;
-            }
-            py *= fy[m] - yc;
-        }
-#pragma unroll
-        for (int k = 0; k < O2; ++k) Vi[m][k] = (m == k) ? 1.0 : 0.0;
     }
-    const double minpiv = gauss_jordan<O2>(V, Vi);  // Vi[ab][m]: phi*_m = sum_ab Vi[ab][m] (x-xc)^a (y-yc)^b
-    if (!(minpiv > 1e-10)) atomicMin(err, SLDG_EGEOM);
-    // shift to monomials x^a y^b of the source cell: (x-xc)^a = sum_a' binom(a,a') (-xc)^(a-a') x^a'
-    double cf[O2][O2];  // cf[a'+O b'][m]
+
+    // step 4: node feet and adjoint polynomials in centred coordinates (relative to the anchor cell)
+    double Vi[O2][O2], xc = 0.0, yc = 0.0;
     {
-        double sxp[O][O], syp[O][O];  // sxp[a][a'] = binom(a,a') (-xc)^(a-a')
+        double fx[O2], fy[O2];
 #pragma unroll
-        for (int aa = 0; aa < O; ++aa)
+        for (int qn = 0; qn < O; ++qn)
 #pragma unroll
-            for (int ap = 0; ap < O; ++ap) {
-                double bin = (ap > aa) ? 0.0 : ((aa == 2 && ap == 1) ? 2.0 : 1.0);
-                double px = 1.0, py = 1.0;
-                for (int e = 0; e < aa - ap; ++e) {
-                    px *= -xc;
-                    py *= -yc;
+            for (int p = 0; p < O; ++p) {
+                double px, py;
+                trace_point(a, b, nx, ny, tx, ty, i, j, bs.xi[O][p], bs.xi[O][qn], order, periodic, px, py);
+                fx[p + O * qn] = px - r0;
+                fy[p + O * qn] = py - s0;
+                xc += px - r0;
+                yc += py - s0;
+            }
+        xc *= 1.0 / O2;
+        yc *= 1.0 / O2;
+        double V[O2][O2];
+#pragma unroll
+        for (int m = 0; m < O2; ++m) {
+            double py = 1.0;
+#pragma unroll
+            for (int bq = 0; bq < O; ++bq) {
+                double px = 1.0;
+#pragma unroll
+                for (int bp = 0; bp < O; ++bp) {
+                    V[m][bp + O * bq] = px * py;
+                    px *= fx[m] - xc;
                 }
-                sxp[aa][ap] = bin * px;
-                syp[aa][ap] = bin * py;
+                py *= fy[m] - yc;
             }
 #pragma unroll
-        for (int m = 0; m < O2; ++m)
-#pragma unroll
-            for (int bp_ = 0; bp_ < O; ++bp_)
-#pragma unroll
-                for (int ap = 0; ap < O; ++ap) {
-                    double acc = 0.0;
-#pragma unroll
-                    for (int bb = bp_; bb < O; ++bb)
-#pragma unroll
-                        for (int aa = ap; aa < O; ++aa) acc = fma(Vi[aa + O * bb][m], sxp[aa][ap] * syp[bb][bp_], acc);
-                    cf[ap + O * bp_][m] = acc;
-                }
-    }
-    // G[k][a'+O b'] = int phi_k x^a' y^b' = sum_{p',q'} L[kp][p'] L[kq][q'] M[p'+a'][q'+b']  (separable)
-    double T[O][O][NM];  // T[kp][a'][q] = sum_p' L[kp][p'] M[p'+a'][q]
-#pragma unroll
-    for (int kp = 0; kp < O; ++kp)
-#pragma unroll
-        for (int ap = 0; ap < O; ++ap)
-#pragma unroll
-            for (int q = 0; q < NM; ++q) {
-                double acc = 0.0;
-#pragma unroll
-                for (int pp = 0; pp < O; ++pp) acc = fma(bs.L[O][kp][pp], M[pp + ap][q], acc);
-                T[kp][ap][q] = acc;
-            }
-    double *Wout = W + ((size_t)cellid * 9 + slot) * (O2 * O2);
-#pragma unroll
-    for (int kq = 0; kq < O; ++kq)
-#pragma unroll
-        for (int kp = 0; kp < O; ++kp) {
-            double G[O2];
-#pragma unroll
-            for (int bp_ = 0; bp_ < O; ++bp_)
-#pragma unroll
-                for (int ap = 0; ap < O; ++ap) {
-                    double acc = 0.0;
-#pragma unroll
-                    for (int qq = 0; qq < O; ++qq) acc = fma(bs.L[O][kq][qq], T[kp][ap][qq + bp_], acc);
-                    G[ap + O * bp_] = acc;
-                }
-            const int k = kp + O * kq;
-#pragma unroll
-            for (int m = 0; m < O2; ++m) {
-                double acc = 0.0;
-#pragma unroll
-                for (int ab = 0; ab < O2; ++ab) acc = fma(cf[ab][m], G[ab], acc);
-                Wout[k * O2 + m] = acc / (bs.w[O][m % O] * bs.w[O][m / O]);
-            }
+            for (int k = 0; k < O2; ++k) Vi[m][k] = (m == k) ? 1.0 : 0.0;
         }
-    atomicOr(&mask[cellid], 1 << slot);
+        const double minpiv = gauss_jordan<O2>(V, Vi);  // phi*_m = sum_ab Vi[ab][m] (x-xc)^a (y-yc)^b
+        if (!(minpiv > 1e-10)) atomicMin(err, SLDG_EGEOM);
+    }
+    double iw[O2];
+#pragma unroll
+    for (int m = 0; m < O2; ++m) iw[m] = 1.0 / (bs.w[O][m % O] * bs.w[O][m / O]);
+
+    // steps 2, 3, 5: one candidate source cell at a time
+    int msk = 0, cnt = 0;
+    double *Wcell = W + (size_t)cellid * 9 * (O2 * O2);
+#pragma unroll 1
+    for (int ds = 0; ds <= ns; ++ds)
+#pragma unroll 1
+        for (int dr = 0; dr <= nr; ++dr) {
+            double M[NM][NM];
+            piece_moments<O>(q, (double)dr, (double)ds, dr < nr, bs, M);
+            if (!(M[0][0] > 0.0)) continue;  // empty intersection
+            // phi*_m in the source cell's monomials: (x-xc)^a = sum_a' binom(a,a') (-xc)^(a-a') x^a'
+            const double lxc = xc - dr, lyc = yc - ds;
+            double cf[O2][O2];  // cf[a'+O b'][m]
+            {
+                double sxp[O][O], syp[O][O];  // sxp[a][a'] = binom(a,a') (-lxc)^(a-a')
+#pragma unroll
+                for (int aa = 0; aa < O; ++aa)
+#pragma unroll
+                    for (int ap = 0; ap < O; ++ap) {
+                        const double bin = (ap > aa) ? 0.0 : ((aa == 2 && ap == 1) ? 2.0 : 1.0);
+                        double px = 1.0, py = 1.0;
+#pragma unroll
+                        for (int e = 0; e < O; ++e)
+                            if (e < aa - ap) {
+                                px *= -lxc;
+                                py *= -lyc;
+                            }
+                        sxp[aa][ap] = bin * px;
+                        syp[aa][ap] = bin * py;
+                    }
+#pragma unroll
+                for (int m = 0; m < O2; ++m)
+#pragma unroll
+                    for (int bp_ = 0; bp_ < O; ++bp_)
+#pragma unroll
+                        for (int ap = 0; ap < O; ++ap) {
+                            double acc = 0.0;
+#pragma unroll
+                            for (int bb = bp_; bb < O; ++bb)
+#pragma unroll
+                                for (int aa = ap; aa < O; ++aa)
+                                    acc = fma(Vi[aa + O * bb][m], sxp[aa][ap] * syp[bb][bp_], acc);
+                            cf[ap + O * bp_][m] = acc;
+                        }
+            }
+            // G[k][a'+O b'] = int phi_k x^a' y^b' = sum_{p',q'} L[kp][p'] L[kq][q'] M[p'+a'][q'+b']  (separable)
+            double T[O][O][NM];  // T[kp][a'][q] = sum_p' L[kp][p'] M[p'+a'][q]
+#pragma unroll
+            for (int kp = 0; kp < O; ++kp)
+#pragma unroll
+                for (int ap = 0; ap < O; ++ap)
+#pragma unroll
+                    for (int qq = 0; qq < NM; ++qq) {
+                        double acc = 0.0;
+#pragma unroll
+                        for (int pp = 0; pp < O; ++pp) acc = fma(bs.L[O][kp][pp], M[pp + ap][qq], acc);
+                        T[kp][ap][qq] = acc;
+                    }
+            double *Wout = Wcell + (size_t)cnt * (O2 * O2);
+#pragma unroll
+            for (int kq = 0; kq < O; ++kq)
+#pragma unroll
+                for (int kp = 0; kp < O; ++kp) {
+                    double G[O2];
+#pragma unroll
+                    for (int bp_ = 0; bp_ < O; ++bp_)
+#pragma unroll
+                        for (int ap = 0; ap < O; ++ap) {
+                            double acc = 0.0;
+#pragma unroll
+                            for (int qq = 0; qq < O; ++qq) acc = fma(bs.L[O][kq][qq], T[kp][ap][qq + bp_], acc);
+                            G[ap + O * bp_] = acc;
+                        }
+                    const int k = kp + O * kq;
+                    double out[O2];
+#pragma unroll
+                    for (int m = 0; m < O2; ++m) {
+                        double acc = 0.0;
+#pragma unroll
+                        for (int ab = 0; ab < O2; ++ab) acc = fma(cf[ab][m], G[ab], acc);
+                        out[m] = acc * iw[m];
+                    }
+                    if (O == 2) {
+                        reinterpret_cast<double2 *>(Wout + k * O2)[0] = make_double2(out[0], out[1]);
+                        reinterpret_cast<double2 *>(Wout + k * O2)[1] = make_double2(out[O2 - 2], out[O2 - 1]);
+                    } else {
+#pragma unroll
+                        for (int m = 0; m < O2; ++m) Wout[k * O2 + m] = out[m];
+                    }
+                }
+            msk |= 1 << (dr + 3 * ds);
+            ++cnt;
+        }
+    hdr[cellid] = make_int4(r0, s0, msk, cnt);
 }
+
+// debug/test helper: expand the packed weight blocks of one z plane to the dense [cell][slot] form
+__global__ void geometry_expand_kernel(const int4 *__restrict__ hdr, const double *__restrict__ W, int ncell, int o4,
+                                       int32_t *__restrict__ anchor, int32_t *__restrict__ mask,
+                                       double *__restrict__ Wd)
+{
+    const int t = blockIdx.x;
+    const int4 h = hdr[t];
+    if (threadIdx.x == 0) {
+        if (anchor) {
+            anchor[2 * t] = h.x;
+            anchor[2 * t + 1] = h.y;
+        }
+        if (mask) mask[t] = h.z;
+    }
+    if (!Wd) return;
+    int n = 0;
+    for (int slot = 0; slot < 9; ++slot) {
+        if (!((h.z >> slot) & 1)) continue;
+        for (int e = threadIdx.x; e < o4; e += blockDim.x)
+            Wd[((size_t)t * 9 + slot) * o4 + e] = W[((size_t)t * 9 + n) * o4 + e];
+        ++n;
+    }
+}
+
+}  // namespace
 
 cudaError_t launch_xy_geometry(sldg_ctx *c, double tau, int trace_order)
 {
     const GridDev &g = c->g;
-    const long long ncell = (long long)g.n[0] * g.n[1];
-    const long long total = (long long)g.N[2] * ncell * 9;
-    cudaError_t e = cudaMemsetAsync(c->mask, 0, sizeof(int32_t) * (size_t)g.N[2] * ncell, c->stream);
-    if (e != cudaSuccess) return e;
-    const int threads = 128;
-    const unsigned grid = (unsigned)((total + threads - 1) / threads);
+    const int ncell = g.n[0] * g.n[1];
     const int O = g.o[0];
-#define LAUNCH_G(OO)                                                                                 \
-    xy_geometry_kernel<OO><<<grid, threads, 0, c->stream>>>(c->va, c->vb, c->anchor, c->mask, c->W, \
-                                                            c->err, g, c->basis, tau, trace_order,  \
-                                                            c->vel_periodic)
+    const int threads = O == 3 ? 64 : 128;
+    dim3 grid((unsigned)((ncell + threads - 1) / threads), (unsigned)g.N[2]);
+#define LAUNCH_G(OO)                                                                                         \
+    xy_geometry_kernel<OO><<<grid, threads, 0, c->stream>>>(c->va, c->vb, c->hdr, c->W, c->err, g, c->basis, \
+                                                            tau, trace_order, c->vel_periodic)
     if (O == 1) LAUNCH_G(1); else if (O == 2) LAUNCH_G(2); else LAUNCH_G(3);
 #undef LAUNCH_G
     c->launches++;
     return cudaGetLastError();
 }
 
+cudaError_t launch_geometry_expand(sldg_ctx *c, int z, int32_t *anchor, int32_t *mask, double *Wd)
+{
+    const GridDev &g = c->g;
+    const int ncell = g.n[0] * g.n[1];
+    const int o4 = g.o[0] * g.o[0] * g.o[0] * g.o[0];
+    geometry_expand_kernel<<<ncell, 32, 0, c->stream>>>(c->hdr + (size_t)z * ncell, c->W + (size_t)z * ncell * 9 * o4,
+                                                        ncell, o4, anchor, mask, Wd);
+    c->launches++;
+    return cudaGetLastError();
+}

@@ -215,6 +215,37 @@ def test_xy_geometry_matches_oracle_coefficients(torch, o, trace_order):
         assert np.abs(col - Wm).max() < 5e-14
 
 
+@pytest.mark.parametrize("o,ncell", [(2, 128), (3, 96)])
+def test_geometry_column_sums_at_bench_size(torch, o, ncell):
+    """Property that holds at any size (mass conservation, SURVEY.md 8(c)-2 pin (i)): on the ITG field of
+    the headline config (full nx x ny plane, a few z nodes) every source DOF's weights sum to W_k.  The ITG
+    field decays to ~1e-18 away from the annulus, which produces upstream cells whose corners sit within
+    rounding of grid lines (zero-area slivers) -- the degenerate cases of the clipping."""
+    spec = inputs.itg_grid(ncell, ncell, 2, 1, o)
+    a, b, _, _ = inputs.itg_fields(spec, 4.0, 0.8)
+    s = _sldg(spec)
+    s.import_state(_dev(torch, np.zeros(spec.shape)))
+    s.set_vxy(_dev(torch, a), _dev(torch, b), 1)
+    s.advect_xy(4.0, 2)
+    s.check()
+    _, wg = oracle.gl(o)
+    Wm = torch.tensor([wg[m % o] * wg[m // o] for m in range(o * o)], dtype=torch.float64, device="cuda")
+    nx = ny = ncell
+    t = torch.arange(nx * ny, device="cuda")
+    ti, tj = t % nx, t // nx
+    for z in range(spec.shape[0]):
+        anchor, mask, W = s.debug_geometry(z)
+        anchor, mask = anchor.long(), mask.long()
+        col = torch.zeros(ny * nx, o * o, dtype=torch.float64, device="cuda")
+        for slot in range(9):
+            on = ((mask >> slot) & 1).bool()
+            r = (ti + anchor[:, 0] + slot % 3) % nx
+            c = (tj + anchor[:, 1] + slot // 3) % ny
+            w = W[on, slot].reshape(-1, o * o, o * o) * Wm[None, None, :]  # [k][m]
+            col.index_add_(0, (c * nx + r)[on], w.sum(dim=2))
+        assert float((col - Wm[None, :]).abs().max()) < 5e-14
+
+
 def _xy_case(torch, spec, f, a, b, tau, trace_order, periodic, steps=1):
     s = _sldg(spec)
     s.import_state(_dev(torch, f))
