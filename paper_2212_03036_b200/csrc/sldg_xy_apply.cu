@@ -6,17 +6,18 @@
 // warp-uniform, the control flow over the (up to 3x3) non-empty source cells is warp-uniform, and empty
 // source cells cost nothing.
 //
-//   xy_apply_stream_kernel (o = 2, the default): a streaming stencil.  A block owns a strip of TX = 4
-//     target cells in x, a segment of L target rows in y, one z node and one chunk of <= 128 v values.
-//     It first reads the segment's headers and takes the bounds of the anchors; they fix a static
-//     schedule: target row j needs source rows j+aymin .. j+aymax and the x window
-//     [axmin, TX-1+axmax].  A producer warp streams the source rows (each row = the window's lines, all
-//     v of the chunk) and each target row's weight blocks into shared-memory rings with cp.async.bulk
-//     copies completing on mbarriers; eight consumer warps (cell x half of the v chunk) wait on the
-//     rows they need, apply, store 512-byte output rows straight to global memory and release the
-//     oldest source row.  Every input line is fetched once per strip (x halo: window/TX), weights once,
-//     several rows are always in flight, no registers are held by loads in flight.
-//     Segments whose anchors vary too much for the rings fall back to direct global loads.
+//   xy_apply_stream_kernel (o = 2, the default): a streaming stencil in SOURCE-row order.  A block owns a
+//     strip of TX = 8 target cells in x, a segment of up to 128 target rows in y, one z node and one chunk
+//     of <= 128 v values.  The prologue reads the segment's headers and takes the bounds of the anchors;
+//     they fix a static schedule: target row j uses source rows j+aymin .. j+aymin+2 and the x window
+//     [axmin, TX-1+axmax].  A producer warp streams the source rows (each row = the window's lines, all v
+//     of the chunk, 40 KB) and each target row's packed weight blocks into shared-memory rings with
+//     cp.async.bulk copies completing on mbarriers.  Sixteen consumer warps (cell x half of the v chunk)
+//     wait for ONE source row at a time, add its contributions to the (up to three) target rows that
+//     use it -- their partial sums live in registers -- release the row at once, and store a target row
+//     when its last source row has been applied.  Because a source row is never held while others arrive,
+//     all but one ring slot are in flight.  Every input line is fetched once per strip (x halo:
+//     window/TX = 10/8), weights once.  Segments whose anchors vary too much fall back to direct loads.
 //   xy_apply_direct_kernel (any o): warp <-> target cell, inputs through L1.
 #include <stdlib.h>
 
@@ -80,34 +81,32 @@ __device__ __forceinline__ void fma_block_o2(double (&acc)[4][2], const double2 
     }
 }
 
-constexpr int STREAM_TX = 4;      // target cells per strip
-constexpr int STREAM_LMAX = 32;   // target rows per segment
-constexpr int STREAM_VMAX = 128;  // v values per chunk
-constexpr int STREAM_THREADS = 288;
+constexpr int STREAM_TX = 8;        // target cells per strip
+constexpr int STREAM_LMAX = 128;    // target rows per segment
+constexpr int STREAM_VMAX = 128;    // v values per chunk
+constexpr int STREAM_CWARPS = 16;   // consumer warps: cell x v half
+constexpr int STREAM_THREADS = 32 * (STREAM_CWARPS + 1);
+constexpr int STREAM_NRMAX = 8;     // ring slots (barrier arrays)
+constexpr int STREAM_NW = 5;        // weight stages (target rows)
+constexpr int STREAM_WROW = 48;     // weight blocks per target row stage (8 cells, <= 9 each, typically 35)
+constexpr int STREAM_NACC = 3;      // source rows per target row handled by the register accumulators
+constexpr size_t STREAM_RING_BYTES = 160 * 1024;
+constexpr size_t STREAM_WRING_BYTES = (size_t)STREAM_NW * STREAM_WROW * 128;
+constexpr size_t STREAM_HDR_BYTES = (size_t)STREAM_LMAX * STREAM_TX * 16;
+constexpr size_t STREAM_SMEM = STREAM_RING_BYTES + STREAM_WRING_BYTES + STREAM_HDR_BYTES + 512;
 
-template <int RWC, int NR, int NW, int WCAP>
-struct StreamSmem {
-    static constexpr size_t ring = (size_t)NR * 2 * 2 * RWC * STREAM_VMAX * 8;
-    static constexpr size_t wring = (size_t)NW * STREAM_TX * WCAP * 16 * 8;
-    static constexpr size_t hdr = (size_t)STREAM_LMAX * STREAM_TX * 16;
-    static constexpr size_t misc = 64 + (size_t)(2 * NR + 2 * NW) * 8;
-    static constexpr size_t total = ring + wring + hdr + misc;
-};
-
-template <int RWC, int NR, int NW, int WCAP>
-__global__ void __launch_bounds__(STREAM_THREADS) xy_apply_stream_kernel(
+__global__ void __launch_bounds__(STREAM_THREADS, 1) xy_apply_stream_kernel(
     const double *__restrict__ fin, double *__restrict__ fout, const int4 *__restrict__ hdrg,
     const double *__restrict__ W, GridDev g, int L)
 {
-    constexpr int TX = STREAM_TX;
-    using SM = StreamSmem<RWC, NR, NW, WCAP>;
+    constexpr int TX = STREAM_TX, NW = STREAM_NW, NACC = STREAM_NACC;
     extern __shared__ __align__(128) unsigned char smem_raw[];
-    double *ring = reinterpret_cast<double *>(smem_raw);                 // [NR][2 kq][2*RWC xdof][VL]
-    double *wring = reinterpret_cast<double *>(smem_raw + SM::ring);     // [NW][TX][WCAP][16]
-    int4 *hdr = reinterpret_cast<int4 *>(smem_raw + SM::ring + SM::wring);  // [L][TX] (ax, ay, mask, -)
-    int *bnd = reinterpret_cast<int *>(smem_raw + SM::ring + SM::wring + SM::hdr);  // bounds
+    double *ring = reinterpret_cast<double *>(smem_raw);                                  // [NR][2 kq][2*RW][VL]
+    double *wring = reinterpret_cast<double *>(smem_raw + STREAM_RING_BYTES);             // [NW][WROW][16]
+    int4 *hdr = reinterpret_cast<int4 *>(smem_raw + STREAM_RING_BYTES + STREAM_WRING_BYTES);  // [L][TX]
+    int *bnd = reinterpret_cast<int *>(smem_raw + STREAM_RING_BYTES + STREAM_WRING_BYTES + STREAM_HDR_BYTES);
     uint64_t *full = reinterpret_cast<uint64_t *>(bnd + 16);
-    uint64_t *empty = full + NR, *wfull = empty + NR, *wempty = wfull + NW;
+    uint64_t *empty = full + STREAM_NRMAX, *wfull = empty + STREAM_NRMAX, *wempty = wfull + NW;
 
     const int nx = g.n[0], ny = g.n[1];
     const int strips = (nx + TX - 1) / TX;
@@ -121,22 +120,19 @@ __global__ void __launch_bounds__(STREAM_THREADS) xy_apply_stream_kernel(
     const long long ncell = (long long)nx * ny;
     const long long zc = (long long)z * ncell;
 
-    // ---- prologue: headers of the segment, anchor bounds ---------------------------------------------
+    // ---- prologue: headers of the segment, anchor bounds, per-row packing of the weight blocks -----------
     if (tid == 0) {
         bnd[0] = 1 << 30; bnd[1] = -(1 << 30); bnd[2] = 1 << 30; bnd[3] = -(1 << 30); bnd[4] = 0;
-        for (int s = 0; s < NR; ++s) { mbar_init(&full[s], 1); mbar_init(&empty[s], 8); }
-        for (int s = 0; s < NW; ++s) { mbar_init(&wfull[s], 1); mbar_init(&wempty[s], 8); }
+        for (int s = 0; s < STREAM_NRMAX; ++s) { mbar_init(&full[s], 1); mbar_init(&empty[s], STREAM_CWARPS); }
+        for (int s = 0; s < NW; ++s) { mbar_init(&wfull[s], 1); mbar_init(&wempty[s], STREAM_CWARPS); }
         mbar_fence_init();
     }
     __syncthreads();
-    if (tid < rows * TX) {
-        const int jr = tid / TX, ci = tid % TX;
+    for (int c = tid; c < rows * TX; c += STREAM_THREADS) {
+        const int jr = c / TX, ci = c % TX;
         int4 h = make_int4(0, 0, 0, 0);
-        if (i0 + ci < nx) {
-            const long long cellid = zc + (long long)(j0 + jr) * nx + i0 + ci;
-            h = __ldg(hdrg + cellid);
-        }
-        hdr[tid] = h;
+        if (i0 + ci < nx) h = __ldg(hdrg + zc + (long long)(j0 + jr) * nx + i0 + ci);
+        hdr[c] = h;
         if (h.z) {
             const int wx = (h.z & 0x124) ? 3 : ((h.z & 0x092) ? 2 : 1);
             const int wy = (h.z & 0x1c0) ? 3 : ((h.z & 0x038) ? 2 : 1);
@@ -144,15 +140,29 @@ __global__ void __launch_bounds__(STREAM_THREADS) xy_apply_stream_kernel(
             atomicMax(&bnd[1], h.x + wx - 1);
             atomicMin(&bnd[2], h.y);
             atomicMax(&bnd[3], h.y + wy - 1);
-            atomicMax(&bnd[4], __popc(h.z));
         }
     }
     __syncthreads();
+    // per target row: exclusive prefix of the block counts -> hdr.w = offset of the cell's first block
+    for (int jr = tid; jr < rows; jr += STREAM_THREADS) {
+        int off = 0;
+#pragma unroll
+        for (int ci = 0; ci < TX; ++ci) {
+            const int n = hdr[jr * TX + ci].w;
+            hdr[jr * TX + ci].w = off;
+            off += n;
+        }
+        atomicMax(&bnd[4], off);
+    }
+    __syncthreads();
+    if (bnd[4] == 0) return;                 // nothing to do (no valid cell)
     const int axmin = bnd[0], aymin = bnd[2];
     const int RW = TX + bnd[1] - axmin;      // window width in cells
     const int S = bnd[3] - aymin + 1;        // source rows per target row
-    if (bnd[4] == 0) return;                 // nothing to do (no valid cell)
-    const bool staged = RW <= RWC && S <= NR && bnd[4] <= WCAP;
+    const size_t stage_doubles = (size_t)2 * 2 * RW * VL;
+    int NR = (int)(STREAM_RING_BYTES / (stage_doubles * 8));
+    NR = NR > STREAM_NRMAX ? STREAM_NRMAX : NR;
+    const bool staged = NR >= 2 && S <= NACC && bnd[4] <= STREAM_WROW;
     const double *fz = fin + z * g.sZ + v0;
     double *oz = fout + z * g.sZ + v0;
 
@@ -192,14 +202,13 @@ __global__ void __launch_bounds__(STREAM_THREADS) xy_apply_stream_kernel(
     }
 
     const int nsrc = rows + S - 1;  // source rows y' = 0 .. nsrc-1, Y = j0 + aymin + y'
-    const size_t stage_doubles = (size_t)2 * 2 * RWC * VL;
 
-    if (warp == 8) {
+    if (warp == STREAM_CWARPS) {
         // ---------------- producer warp -------------------------------------------------------------------
         const int wx0 = wrap_idx(i0 + axmin, nx);       // first cell of the x window (wrapped)
         const int n1 = min(RW, nx - wx0);               // cells before the periodic seam
-        const bool runs = (g.sX == (long long)VL);      // window lines contiguous in memory (z,y,x order)
-        const uint32_t row_bytes = (uint32_t)(2 * 2 * RW * VL * 8);
+        const bool runs = (g.sX == (long long)VL) && RW <= nx;  // window lines contiguous in memory (z,y,x order)
+        const uint32_t row_bytes = (uint32_t)(stage_doubles * 8);
         for (int k = 0; k < nsrc; ++k) {
             const int st = k % NR;
             if (k >= NR) mbar_wait(&empty[st], ((k / NR) & 1) ^ 1);
@@ -213,35 +222,38 @@ __global__ void __launch_bounds__(STREAM_THREADS) xy_apply_stream_kernel(
                     const int kq = lane & 1, part = lane >> 1;
                     const int c0 = part ? 0 : wx0, nc = part ? RW - n1 : n1, off = part ? n1 : 0;
                     if (nc > 0)
-                        bulk_g2s(dst + ((size_t)kq * 2 * RWC + 2 * off) * VL,
+                        bulk_g2s(dst + ((size_t)kq * 2 * RW + 2 * off) * VL,
                                  fz + (long long)(2 * sY + kq) * g.sY + (long long)(2 * c0) * g.sX,
                                  (uint32_t)(2 * nc * VL * 8), &full[st]);
                 }
             } else {
                 for (int l = lane; l < 4 * RW; l += 32) {
                     const int kq = l / (2 * RW), xd = l - kq * 2 * RW;
-                    int r = wx0 + (xd >> 1);
-                    if (r >= nx) r -= nx;
-                    bulk_g2s(dst + ((size_t)kq * 2 * RWC + xd) * VL,
+                    const int r = (wx0 + (xd >> 1)) % nx;  // the window may be wider than the periodic box
+                    bulk_g2s(dst + ((size_t)kq * 2 * RW + xd) * VL,
                              fz + (long long)(2 * sY + kq) * g.sY + (long long)(2 * r + (xd & 1)) * g.sX,
                              (uint32_t)(VL * 8), &full[st]);
                 }
             }
-            // weights of the target row whose last source row this is
-            const int jr = k - (S - 1);
-            if (jr >= 0 && jr < rows) {
-                const int ws = jr % NW;
-                if (jr >= NW) mbar_wait(&wempty[ws], ((jr / NW) & 1) ^ 1);
+            // weights of target row k (first used with source row k)
+            if (k < rows) {
+                const int ws = k % NW;
+                if (k >= NW) mbar_wait(&wempty[ws], ((k / NW) & 1) ^ 1);
                 const int ci = lane;                      // one packed run of weight blocks per cell
-                const int cnt = ci < TX ? hdr[jr * TX + ci].w : 0;
+                int cnt = 0, off = 0;
+                if (ci < TX) {
+                    const int4 h = hdr[k * TX + ci];
+                    cnt = __popc(h.z);
+                    off = h.w;
+                }
                 int tot = cnt;
 #pragma unroll
-                for (int off = 1; off < TX; off <<= 1) tot += __shfl_xor_sync(0xffffffffu, tot, off);
+                for (int o = 1; o < TX; o <<= 1) tot += __shfl_xor_sync(0xffffffffu, tot, o);
                 if (lane == 0) mbar_arrive_expect_tx(&wfull[ws], (uint32_t)(tot * 128));
                 __syncwarp();
                 if (cnt > 0) {
-                    const long long cellid = zc + (long long)(j0 + jr) * nx + i0 + ci;
-                    bulk_g2s(wring + (size_t)(ws * TX + ci) * WCAP * 16, W + (size_t)cellid * 9 * 16,
+                    const long long cellid = zc + (long long)(j0 + k) * nx + i0 + ci;
+                    bulk_g2s(wring + ((size_t)ws * STREAM_WROW + off) * 16, W + (size_t)cellid * 9 * 16,
                              (uint32_t)(cnt * 128), &wfull[ws]);
                 }
             }
@@ -253,44 +265,71 @@ __global__ void __launch_bounds__(STREAM_THREADS) xy_apply_stream_kernel(
     const int ci = warp >> 1, vh = warp & 1;
     const int v = vh * 64 + 2 * lane;
     const bool live = (i0 + ci < nx) && (v < VL);
-    for (int jr = 0; jr < rows; ++jr) {
-        const int ws = jr % NW;
-        mbar_wait(&wfull[ws], (jr / NW) & 1);
-        for (int y = jr; y < jr + S; ++y) mbar_wait(&full[y % NR], (y / NR) & 1);
-        const int4 h = hdr[jr * TX + ci];
-        if (live && h.z) {
-            double acc[4][2] = {};
-            const int bx = ci + h.x - axmin, by = jr + h.y - aymin;
-            const double *Wp = wring + (size_t)(ws * TX + ci) * WCAP * 16;
-#pragma unroll 1
-            for (int dy = 0; dy < 3; ++dy) {
-                const int mrow = (h.z >> (3 * dy)) & 7;
-                if (!mrow) continue;
-                const double *srow = ring + (size_t)((by + dy) % NR) * stage_doubles + v;
+    double acc[NACC][4][2];
 #pragma unroll
-                for (int dx = 0; dx < 3; ++dx) {
-                    if (!((mrow >> dx) & 1)) continue;
-                    const double *src = srow + (size_t)(2 * (bx + dx)) * VL;
-                    double2 in[4];
-                    in[0] = *reinterpret_cast<const double2 *>(src);
-                    in[1] = *reinterpret_cast<const double2 *>(src + VL);
-                    in[2] = *reinterpret_cast<const double2 *>(src + (size_t)2 * RWC * VL);
-                    in[3] = *reinterpret_cast<const double2 *>(src + (size_t)2 * RWC * VL + VL);
-                    fma_block_o2(acc, in, Wp);
-                    Wp += 16;
+    for (int a = 0; a < NACC; ++a)
+#pragma unroll
+        for (int m = 0; m < 4; ++m) acc[a][m][0] = acc[a][m][1] = 0.0;
+
+    // one step: source row k; target rows k, k-1, k-2 (accumulator sets are indexed by row mod 3, static
+    // because the step loop is unrolled by 3)
+    for (int kb = 0; kb < rows + NACC - 1; kb += NACC) {
+#pragma unroll
+        for (int u = 0; u < NACC; ++u) {
+            const int k = kb + u;
+            if (k >= rows + NACC - 1) break;
+            if (k < rows) mbar_wait(&wfull[k % NW], (k / NW) & 1);
+            if (k < nsrc) {
+                const int st = k % NR;
+                mbar_wait(&full[st], (k / NR) & 1);
+                const double *srow = ring + (size_t)st * stage_doubles + v;
+#pragma unroll
+                for (int d = 0; d < NACC; ++d) {
+                    const int jr = k - d;
+                    if (jr < 0 || jr >= rows) continue;
+                    const int4 h = hdr[jr * TX + ci];
+                    const int dy = d - (h.y - aymin);
+                    if (!live || dy < 0 || dy > 2) continue;
+                    const int mrow = (h.z >> (3 * dy)) & 7;
+                    if (!mrow) continue;
+                    const double *Wp = wring + ((size_t)(jr % NW) * STREAM_WROW + h.w +
+                                                __popc(h.z & ((1 << (3 * dy)) - 1))) * 16;
+                    const int bx = ci + h.x - axmin;
+#pragma unroll
+                    for (int dx = 0; dx < 3; ++dx) {
+                        if (!((mrow >> dx) & 1)) continue;
+                        const double *src = srow + (size_t)(2 * (bx + dx)) * VL;
+                        double2 in[4];
+                        in[0] = *reinterpret_cast<const double2 *>(src);
+                        in[1] = *reinterpret_cast<const double2 *>(src + VL);
+                        in[2] = *reinterpret_cast<const double2 *>(src + (size_t)2 * RW * VL);
+                        in[3] = *reinterpret_cast<const double2 *>(src + (size_t)2 * RW * VL + VL);
+                        fma_block_o2(acc[(u - d + NACC) % NACC], in, Wp);
+                        Wp += 16;
+                    }
                 }
+                __syncwarp();
+                if (lane == 0) mbar_arrive(&empty[st]);
             }
-            const int i = i0 + ci, j = j0 + jr;
+            // target row k - 2 has seen all its source rows
+            const int jd = k - (NACC - 1);
+            if (jd >= 0 && jd < rows) {
+                constexpr int unused = 0;
+                (void)unused;
+                double(&a)[4][2] = acc[(u + 1) % NACC];  // (u - 2 + 3) % 3
+                if (live && hdr[jd * TX + ci].z) {
+                    const int i = i0 + ci, j = j0 + jd;
 #pragma unroll
-            for (int m = 0; m < 4; ++m)
-                *reinterpret_cast<double2 *>(oz + (long long)(2 * j + (m >> 1)) * g.sY +
-                                             (long long)(2 * i + (m & 1)) * g.sX + v) =
-                    make_double2(acc[m][0], acc[m][1]);
-        }
-        __syncwarp();
-        if (lane == 0) {
-            mbar_arrive(&wempty[ws]);
-            mbar_arrive(&empty[jr % NR]);  // source row y' = jr is not needed by later target rows
+                    for (int m = 0; m < 4; ++m)
+                        __stcs(reinterpret_cast<double2 *>(oz + (long long)(2 * j + (m >> 1)) * g.sY +
+                                                           (long long)(2 * i + (m & 1)) * g.sX + v),
+                               make_double2(a[m][0], a[m][1]));
+                }
+#pragma unroll
+                for (int m = 0; m < 4; ++m) a[m][0] = a[m][1] = 0.0;
+                __syncwarp();
+                if (lane == 0) mbar_arrive(&wempty[jd % NW]);
+            }
         }
     }
 }
@@ -379,14 +418,12 @@ cudaError_t launch_xy_apply(sldg_ctx *c, const double *fin, double *fout)
     const GridDev &g = c->g;
     const int O = g.o[0];
     if (O == 2 && !getenv("SLDG_APPLY_DIRECT")) {
-        constexpr int RWC = 6, NR = 4, NW = 3, WCAP = 6;
-        using SM = StreamSmem<RWC, NR, NW, WCAP>;
-        auto kern = xy_apply_stream_kernel<RWC, NR, NW, WCAP>;
-        cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)SM::total);
+        auto kern = xy_apply_stream_kernel;
+        cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)STREAM_SMEM);
         const int L = g.n[1] < STREAM_LMAX ? g.n[1] : STREAM_LMAX;
         const int strips = (g.n[0] + STREAM_TX - 1) / STREAM_TX, segs = (g.n[1] + L - 1) / L;
         dim3 grid((unsigned)(strips * segs), (unsigned)((g.Pv + STREAM_VMAX - 1) / STREAM_VMAX), (unsigned)g.N[2]);
-        kern<<<grid, STREAM_THREADS, SM::total, c->stream>>>(fin, fout, c->hdr, c->W, g, L);
+        kern<<<grid, STREAM_THREADS, STREAM_SMEM, c->stream>>>(fin, fout, c->hdr, c->W, g, L);
         c->launches++;
         return cudaGetLastError();
     }
