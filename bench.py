@@ -52,6 +52,20 @@ def measured_peak():
         return 6650.0, "fallback (B200_PROFILING.md: 6.65 TB/s)"
 
 
+def ncu_traffic(kernel, workload):
+    """dram__bytes_read.sum + dram__bytes_write.sum per launch from the committed ncu --set full capture
+    (profiles/ncu_traffic.csv: workload,kernel,read_bytes,write_bytes); None if there is no capture."""
+    try:
+        with open(os.path.join(ROOT, "profiles", "ncu_traffic.csv")) as fh:
+            for row in fh:
+                p = [x.strip() for x in row.split(",")]
+                if len(p) >= 4 and p[0] == workload and p[1] == kernel:
+                    return float(p[2]) + float(p[3])
+    except OSError:
+        pass
+    return None
+
+
 class ClockSampler:
     """Samples nvidia-smi SM clocks and throttle reasons during the timed region."""
 
@@ -229,24 +243,28 @@ def run_ours(args):
     sub = {
         "advect_z_gbs": gbs(2 * nbytes, 0.5 * (med[0] + med[5])),
         "advect_v_gbs": gbs(2 * nbytes, 0.5 * (med[1] + med[4])),
-        "advect_xy_gbs": gbs(2 * nbytes, med[2] + med[3]),
-        "xy_geometry_ms": float(med[2]), "xy_apply_ms": float(med[3]),
-        "xy_apply_only_gbs": gbs(2 * nbytes, med[3]),
+        "advect_xy_gbs": gbs(2 * nbytes, med[3]),
+        "xy_ms": float(med[3]), "xy_geometry_kernel_ms": float(med[2]),
+        "xy_geometry_overlapped_with_apply": bool(med[6] > 0.5),
         "charge_density_gbs": gbs(nbytes, rho_ms),
-        "ms": [float(x) for x in med[:6]],
+        "xy_apply_direct_path_blocks_total": s.debug_counter(0),
+        "ms": {"z": float(med[0]), "v": float(med[1]), "xy": float(med[3]), "v2": float(med[4]), "z2": float(med[5])},
     }
     for k in ("advect_z_gbs", "advect_v_gbs", "advect_xy_gbs"):
         sub[k.replace("_gbs", "_frac_of_8TBs")] = sub[k] / NOMINAL_PEAK_GBS
     # dominant kernel = the one with the largest share of the step
-    shares = {"advect_z": med[0] + med[5], "advect_v": med[1] + med[4], "xy_geometry": med[2], "xy_apply": med[3]}
+    shares = {"advect_z": med[0] + med[5], "advect_v": med[1] + med[4], "xy_apply": med[3]}
     dom = max(shares, key=shares.get)
-    dom_ms = {"advect_z": 0.5 * (med[0] + med[5]), "advect_v": 0.5 * (med[1] + med[4]), "xy_geometry": med[2],
-              "xy_apply": med[3]}[dom]
+    dom_ms = {"advect_z": 0.5 * (med[0] + med[5]), "advect_v": 0.5 * (med[1] + med[4]), "xy_apply": med[3]}[dom]
     achieved = gbs(2 * nbytes, dom_ms)
     roofline = {"kernel": dom, "bound": "hbm", "achieved": achieved, "peak": peak, "unit": "GB/s",
-                "frac": achieved / peak, "traffic": None, "peak_source": peak_src,
+                "frac": achieved / peak, "traffic": ncu_traffic(dom, args.workload), "peak_source": peak_src,
                 "algorithmic_bytes_per_launch": 2 * nbytes, "launch_ms": float(dom_ms),
-                "share_of_step": float(shares[dom] / med[7])}
+                "share_of_step": float(shares[dom] / med[7]),
+                "all": {k: {"achieved": gbs(2 * nbytes, t), "frac": gbs(2 * nbytes, t) / peak,
+                            "traffic": ncu_traffic(k, args.workload)}
+                        for k, t in (("advect_z", 0.5 * (med[0] + med[5])), ("advect_v", 0.5 * (med[1] + med[4])),
+                                     ("xy_apply", med[3]))}}
 
     # ---------------- end-to-end leg: host buffers through the C-ABI --------------------------------
     Ez_h, a_h, b_h = (torch.from_numpy(x).pin_memory() for x in (Ez, a, b))

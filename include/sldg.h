@@ -22,7 +22,8 @@
  *   state           the library keeps f in an INTERNAL layout (v fastest) inside f_a/f_b and
  *                   ping-pongs between them; sldg_import_state / sldg_export_state convert.
  *   stream          every call enqueues on the cudaStream_t given at sldg_create and returns without
- *                   synchronising, unless stated otherwise.
+ *                   synchronising, unless stated otherwise.  (Inside sldg_advect_xy the geometry kernel runs on
+ *                   an internal stream that forks from and joins that stream; invisible to the caller.)
  *   errors          return value 0 = success, negative = SLDG_E* below.  Errors detected on the device
  *                   (geometry) are sticky and reported by sldg_check.  There is no CPU fallback: without
  *                   a CUDA device every compute call returns SLDG_ECUDA.
@@ -121,8 +122,11 @@ int sldg_strang_step_host(sldg_ctx *ctx, double dt, const double *Ez_host, const
 /* Synchronises the stream and returns the sticky device error word (0, SLDG_ESTENCIL, SLDG_EGEOM) or
  * SLDG_ECUDA; clears it. */
 int sldg_check(sldg_ctx *ctx);
-/* Device times (CUDA events on the context's stream) of the last sldg_strang_step, in ms:
- * ms[0] z  ms[1] v  ms[2] xy geometry  ms[3] xy apply  ms[4] v  ms[5] z  ms[6] (unused, 0)  ms[7] total.
+/* Device times (CUDA events) of the last sldg_strang_step, in ms:
+ * ms[0] z  ms[1] v  ms[3] the WHOLE xy substep (geometry + apply, first launch to last)  ms[4] v  ms[5] z
+ * ms[7] total -- all on the context's stream; ms[2] = duration of the geometry kernel alone on the library's
+ * internal stream (it is part of ms[3], not in addition to it); ms[6] = 1 if that kernel ran concurrently
+ * with the apply (o = 2), 0 if the apply waited for it.
  * After a single sldg_advect_* call only that entry (and ms[7]) is set.  Synchronises. */
 int sldg_last_timing_ms(sldg_ctx *ctx, float ms[8]);
 /* Number of kernels the library launched on behalf of this context since creation. */
@@ -133,6 +137,10 @@ long long sldg_launch_count(sldg_ctx *ctx);
  * 3x3 slots (bit dx + 3 dy), and W[t][slot][m][k] = C^{ij,m}_{rs,k} / W_m (dense, 9*o^4 doubles per cell,
  * entries of empty slots are unspecified).  Device buffers; asynchronous. */
 int sldg_debug_geometry(sldg_ctx *ctx, int z, int32_t *anchor_dev, int32_t *mask_dev, double *W_dev);
+/* Diagnostic counter `which` since creation, into *value_host; synchronises the stream.
+ *   0: blocks of the 2d apply kernel that could not use the staged (shared-memory ring) path and fell back to
+ *      direct global loads (windows too wide for the ring, more than 3 source rows per target row). */
+int sldg_debug_counter(sldg_ctx *ctx, int which, long long *value_host);
 const char *sldg_strerror(int code);
 
 #ifdef __cplusplus

@@ -51,7 +51,7 @@ void fill_grid(const sldg_params *p, GridDev *g)
 }
 
 struct WorkspaceMap {
-    size_t Ez, va, vb, hdr, W, partials, rho, scalar, err, total;
+    size_t Ez, va, vb, hdr, W, partials, rho, scalar, err, zflag, total;
     size_t n_partials;
 };
 
@@ -75,6 +75,7 @@ WorkspaceMap map_workspace(const sldg_params *p)
     m.rho = take((size_t)g.lines * 8);
     m.scalar = take(256);
     m.err = take(256);
+    m.zflag = take(Nz * 8);
     m.total = off;
     return m;
 }
@@ -264,6 +265,9 @@ int sldg_create(const sldg_params *p, double *f_a_dev, double *f_b_dev, void *wo
     c->rho_ws = (double *)(ws + m.rho);
     c->scalar_ws = (double *)(ws + m.scalar);
     c->err = (int32_t *)(ws + m.err);
+    c->zflag = (unsigned long long *)(ws + m.zflag);
+    c->xy_epoch = 0;
+    c->overlap = getenv("SLDG_XY_OVERLAP") ? 1 : 0;  // experimental: co-running the two kernels is slower today
     c->trace_order = 2;
     c->vel_periodic = 0;
     if (cudaDeviceGetAttribute(&c->sm_count, cudaDevAttrMultiProcessorCount, dev) != cudaSuccess) {
@@ -272,14 +276,26 @@ int sldg_create(const sldg_params *p, double *f_a_dev, double *f_b_dev, void *wo
     }
     for (int k = 0; k < 8; ++k)
         if (cudaEventCreate(&c->ev[k]) != cudaSuccess) {
-            delete c;
+            sldg_destroy(c);
             return SLDG_ECUDA;
         }
+    {
+        // the geometry kernel runs on an internal stream of the highest priority, concurrently with the apply
+        int lo_pri = 0, hi_pri = 0;
+        cudaDeviceGetStreamPriorityRange(&lo_pri, &hi_pri);
+        bool ok = cudaStreamCreateWithPriority(&c->gstream, cudaStreamNonBlocking, hi_pri) == cudaSuccess;
+        for (int k = 0; k < 4 && ok; ++k) ok = cudaEventCreate(&c->gev[k]) == cudaSuccess;
+        if (!ok) {
+            sldg_destroy(c);
+            return SLDG_ECUDA;
+        }
+    }
     // fields default to zero, error word cleared
     cudaError_t e = cudaMemsetAsync(ws + m.Ez, 0, m.hdr - m.Ez, c->stream);
     if (e == cudaSuccess) e = cudaMemsetAsync(c->err, 0, 256, c->stream);
+    if (e == cudaSuccess) e = cudaMemsetAsync(c->zflag, 0, (size_t)c->g.N[2] * 8, c->stream);
     if (e != cudaSuccess) {
-        delete c;
+        sldg_destroy(c);
         return SLDG_ECUDA;
     }
     *out = c;
@@ -289,8 +305,12 @@ int sldg_create(const sldg_params *p, double *f_a_dev, double *f_b_dev, void *wo
 int sldg_destroy(sldg_ctx *c)
 {
     if (!c) return SLDG_EINVAL;
+    if (c->gstream) cudaStreamSynchronize(c->gstream);
     for (int k = 0; k < 8; ++k)
         if (c->ev[k]) cudaEventDestroy(c->ev[k]);
+    for (int k = 0; k < 4; ++k)
+        if (c->gev[k]) cudaEventDestroy(c->gev[k]);
+    if (c->gstream) cudaStreamDestroy(c->gstream);
     delete c;
     return SLDG_OK;
 }
@@ -370,11 +390,24 @@ static int do_v(sldg_ctx *c, double tau)
     return SLDG_OK;
 }
 
-static int do_xy(sldg_ctx *c, double tau, int trace_order, cudaEvent_t mid)
+// The geometry (once per z node) and the apply (every v) of one 2d step.  The geometry runs on the
+// internal stream: it starts when everything enqueued before this call has finished (fields set, previous
+// apply done with the weights) and publishes one counter per z node; the apply, on the caller's stream, starts
+// at the same time and each of its blocks waits for its z node's counter -- the ALU-bound geometry is hidden
+// under the bandwidth-bound apply.  Without overlap (o != 2, SLDG_NO_OVERLAP) the apply waits for the whole
+// geometry kernel.
+static int do_xy(sldg_ctx *c, double tau, int trace_order)
 {
-    if (launch_xy_geometry(c, tau, trace_order) != cudaSuccess) return SLDG_ECUDA;
-    if (mid) cudaEventRecord(mid, c->stream);
-    if (launch_xy_apply(c, c->f[c->cur], c->f[c->cur ^ 1]) != cudaSuccess) return SLDG_ECUDA;
+    const bool overlap = c->overlap && xy_apply_can_overlap(c);
+    c->xy_epoch++;
+    cudaEventRecord(c->gev[0], c->stream);
+    cudaStreamWaitEvent(c->gstream, c->gev[0], 0);
+    cudaEventRecord(c->gev[1], c->gstream);
+    if (launch_xy_geometry(c, c->gstream, tau, trace_order) != cudaSuccess) return SLDG_ECUDA;
+    cudaEventRecord(c->gev[2], c->gstream);
+    if (!overlap) cudaStreamWaitEvent(c->stream, c->gev[2], 0);
+    if (launch_xy_apply(c, c->f[c->cur], c->f[c->cur ^ 1], overlap) != cudaSuccess) return SLDG_ECUDA;
+    if (overlap) cudaStreamWaitEvent(c->stream, c->gev[2], 0);  // join (the geometry has long finished)
     swap_state(c);
     return SLDG_OK;
 }
@@ -403,8 +436,8 @@ int sldg_advect_xy(sldg_ctx *c, double tau, int trace_order)
 {
     if (!c || (trace_order != 1 && trace_order != 2)) return SLDG_EINVAL;
     cudaEventRecord(c->ev[0], c->stream);
-    int rc = do_xy(c, tau, trace_order, c->ev[1]);
-    cudaEventRecord(c->ev[2], c->stream);
+    int rc = do_xy(c, tau, trace_order);
+    cudaEventRecord(c->ev[1], c->stream);
     c->ev_kind = 4;
     return rc;
 }
@@ -430,12 +463,12 @@ int sldg_strang_step(sldg_ctx *c, double dt)
     cudaEventRecord(c->ev[1], c->stream);
     if ((rc = do_v(c, 0.5 * dt))) return rc;
     cudaEventRecord(c->ev[2], c->stream);
-    if ((rc = do_xy(c, dt, c->trace_order, c->ev[3]))) return rc;
-    cudaEventRecord(c->ev[4], c->stream);
+    if ((rc = do_xy(c, dt, c->trace_order))) return rc;
+    cudaEventRecord(c->ev[3], c->stream);
     if ((rc = do_v(c, 0.5 * dt))) return rc;
-    cudaEventRecord(c->ev[5], c->stream);
+    cudaEventRecord(c->ev[4], c->stream);
     if ((rc = do_z(c, 0.5 * dt))) return rc;
-    cudaEventRecord(c->ev[6], c->stream);
+    cudaEventRecord(c->ev[5], c->stream);
     c->ev_kind = 1;
     return SLDG_OK;
 }
@@ -495,17 +528,25 @@ int sldg_last_timing_ms(sldg_ctx *c, float ms[8])
         cudaEventElapsedTime(&t, c->ev[a], c->ev[b]);
         return t;
     };
+    auto geom = [&]() {
+        float t = 0.0f;
+        cudaEventSynchronize(c->gev[2]);
+        cudaEventElapsedTime(&t, c->gev[1], c->gev[2]);
+        return t;
+    };
     if (c->ev_kind == 1) {
-        for (int k = 0; k < 6; ++k) ms[k] = el(k, k + 1);
-        ms[7] = el(0, 6);
+        ms[0] = el(0, 1); ms[1] = el(1, 2); ms[3] = el(2, 3); ms[4] = el(3, 4); ms[5] = el(4, 5);
+        ms[2] = geom();
+        ms[6] = (c->overlap && xy_apply_can_overlap(c)) ? 1.0f : 0.0f;
+        ms[7] = el(0, 5);
     } else if (c->ev_kind == 2) {
         ms[0] = ms[7] = el(0, 1);
     } else if (c->ev_kind == 3) {
         ms[1] = ms[7] = el(0, 1);
     } else if (c->ev_kind == 4) {
-        ms[2] = el(0, 1);
-        ms[3] = el(1, 2);
-        ms[7] = el(0, 2);
+        ms[2] = geom();
+        ms[3] = ms[7] = el(0, 1);
+        ms[6] = (c->overlap && xy_apply_can_overlap(c)) ? 1.0f : 0.0f;
     }
     return SLDG_OK;
 }
@@ -516,6 +557,16 @@ int sldg_debug_geometry(sldg_ctx *c, int z, int32_t *anchor_dev, int32_t *mask_d
 {
     if (!c || z < 0 || z >= c->g.N[2]) return SLDG_EINVAL;
     return cuda_fail(launch_geometry_expand(c, z, anchor_dev, mask_dev, W_dev));
+}
+
+int sldg_debug_counter(sldg_ctx *c, int which, long long *value_host)
+{
+    if (!c || !value_host || which != 0) return SLDG_EINVAL;
+    int32_t word = 0;
+    if (cudaMemcpyAsync(&word, c->err + 1 + which, 4, cudaMemcpyDeviceToHost, c->stream) != cudaSuccess) return SLDG_ECUDA;
+    if (cudaStreamSynchronize(c->stream) != cudaSuccess) return SLDG_ECUDA;
+    *value_host = word;
+    return SLDG_OK;
 }
 
 const char *sldg_strerror(int code)

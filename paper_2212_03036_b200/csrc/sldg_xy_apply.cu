@@ -12,8 +12,8 @@
 //     they fix a static schedule: target row j uses source rows j+aymin .. j+aymin+2 and the x window
 //     [axmin, TX-1+axmax].  A producer warp streams the source rows (each row = the window's lines, all v
 //     of the chunk, 40 KB) and each target row's packed weight blocks into shared-memory rings with
-//     cp.async.bulk copies completing on mbarriers.  Sixteen consumer warps (cell x half of the v chunk)
-//     wait for ONE source row at a time, add its contributions to the (up to three) target rows that
+//     cp.async.bulk copies completing on mbarriers.  Eight consumer warps (one per target cell, four v values
+//     per lane) wait for ONE source row at a time, add its contributions to the (up to three) target rows that
 //     use it -- their partial sums live in registers -- release the row at once, and store a target row
 //     when its last source row has been applied.  Because a source row is never held while others arrive,
 //     all but one ring slot are in flight.  Every input line is fetched once per strip (x halo:
@@ -63,8 +63,39 @@ __device__ __forceinline__ void mbar_wait(uint64_t *bar, uint32_t parity)
     } while (!ok);
 }
 
-// One source cell's contribution for two v values per lane: 4 inputs (k), 16 weights W[k][m] (o = 2).
-__device__ __forceinline__ void fma_block_o2(double (&acc)[4][2], const double2 (&in)[4], const double *Wp)
+// One source cell's contribution for NP v pairs per lane (pair p at v = 64 p + 2 lane): 4 inputs (k), 16 weights
+// W[k][m] (o = 2).  The weights are warp-uniform shared-memory broadcasts.
+template <int NP>
+__device__ __forceinline__ void fma_block_o2(double (&acc)[4][2 * NP], const double *__restrict__ src,
+                                             size_t kq_stride, int VL, const double *__restrict__ Wp)
+{
+    // all input loads of the block first (4 NP in flight), weights k by k (broadcast loads, short latency)
+    double2 in[4][NP];
+#pragma unroll
+    for (int k = 0; k < 4; ++k)
+#pragma unroll
+        for (int p = 0; p < NP; ++p)
+            in[k][p] = *reinterpret_cast<const double2 *>(src + (k >> 1) * kq_stride + (k & 1) * VL + 64 * p);
+#pragma unroll
+    for (int k = 0; k < 4; ++k) {
+        const double2 w01 = *reinterpret_cast<const double2 *>(Wp + k * 4);
+        const double2 w23 = *reinterpret_cast<const double2 *>(Wp + k * 4 + 2);
+#pragma unroll
+        for (int p = 0; p < NP; ++p) {
+            acc[0][2 * p] = fma(w01.x, in[k][p].x, acc[0][2 * p]);
+            acc[0][2 * p + 1] = fma(w01.x, in[k][p].y, acc[0][2 * p + 1]);
+            acc[1][2 * p] = fma(w01.y, in[k][p].x, acc[1][2 * p]);
+            acc[1][2 * p + 1] = fma(w01.y, in[k][p].y, acc[1][2 * p + 1]);
+            acc[2][2 * p] = fma(w23.x, in[k][p].x, acc[2][2 * p]);
+            acc[2][2 * p + 1] = fma(w23.x, in[k][p].y, acc[2][2 * p + 1]);
+            acc[3][2 * p] = fma(w23.y, in[k][p].x, acc[3][2 * p]);
+            acc[3][2 * p + 1] = fma(w23.y, in[k][p].y, acc[3][2 * p + 1]);
+        }
+    }
+}
+
+// the same for two v values per lane, operands from global memory (fallback path)
+__device__ __forceinline__ void fma_block_o2_direct(double (&acc)[4][2], const double2 (&in)[4], const double *Wp)
 {
 #pragma unroll
     for (int k = 0; k < 4; ++k) {
@@ -84,22 +115,26 @@ __device__ __forceinline__ void fma_block_o2(double (&acc)[4][2], const double2 
 constexpr int STREAM_TX = 8;        // target cells per strip
 constexpr int STREAM_LMAX = 128;    // target rows per segment
 constexpr int STREAM_VMAX = 128;    // v values per chunk
-constexpr int STREAM_CWARPS = 16;   // consumer warps: cell x v half
-constexpr int STREAM_THREADS = 32 * (STREAM_CWARPS + 1);
+// consumer warps: VSPLIT per target cell of the strip (VSPLIT = 1: one warp, 4 v values per lane; 2: two warps, one
+// half of the v chunk each, 2 v values per lane); + 1 producer warp
 constexpr int STREAM_NRMAX = 8;     // ring slots (barrier arrays)
 constexpr int STREAM_NW = 5;        // weight stages (target rows)
-constexpr int STREAM_WROW = 48;     // weight blocks per target row stage (8 cells, <= 9 each, typically 35)
+constexpr int STREAM_WROW = 72;     // weight blocks per target row stage (8 cells x <= 9 blocks)
 constexpr int STREAM_NACC = 3;      // source rows per target row handled by the register accumulators
 constexpr size_t STREAM_RING_BYTES = 160 * 1024;
 constexpr size_t STREAM_WRING_BYTES = (size_t)STREAM_NW * STREAM_WROW * 128;
 constexpr size_t STREAM_HDR_BYTES = (size_t)STREAM_LMAX * STREAM_TX * 16;
 constexpr size_t STREAM_SMEM = STREAM_RING_BYTES + STREAM_WRING_BYTES + STREAM_HDR_BYTES + 512;
+constexpr long long STREAM_SPIN_LIMIT = 4000000000ll;  // cycles (~2 s): a stuck flag becomes an error, not a hang
 
-__global__ void __launch_bounds__(STREAM_THREADS, 1) xy_apply_stream_kernel(
+template <int VSPLIT>
+__global__ void __launch_bounds__(32 * (STREAM_TX * VSPLIT + 1), 1) xy_apply_stream_kernel(
     const double *__restrict__ fin, double *__restrict__ fout, const int4 *__restrict__ hdrg,
-    const double *__restrict__ W, GridDev g, int L)
+    const double *__restrict__ W, GridDev g, int L, const unsigned long long *zflag,
+    unsigned long long flag_target, int32_t *err)
 {
     constexpr int TX = STREAM_TX, NW = STREAM_NW, NACC = STREAM_NACC;
+    constexpr int STREAM_CWARPS = TX * VSPLIT, STREAM_THREADS = 32 * (STREAM_CWARPS + 1), NP = 2 / VSPLIT;
     extern __shared__ __align__(128) unsigned char smem_raw[];
     double *ring = reinterpret_cast<double *>(smem_raw);                                  // [NR][2 kq][2*RW][VL]
     double *wring = reinterpret_cast<double *>(smem_raw + STREAM_RING_BYTES);             // [NW][WROW][16]
@@ -126,12 +161,28 @@ __global__ void __launch_bounds__(STREAM_THREADS, 1) xy_apply_stream_kernel(
         for (int s = 0; s < STREAM_NRMAX; ++s) { mbar_init(&full[s], 1); mbar_init(&empty[s], STREAM_CWARPS); }
         for (int s = 0; s < NW; ++s) { mbar_init(&wfull[s], 1); mbar_init(&wempty[s], STREAM_CWARPS); }
         mbar_fence_init();
+        if (zflag) {
+            // the geometry kernel of this step runs concurrently on another stream: wait until every one of its
+            // blocks of this z node has published (acquire), bounded so that a lost flag cannot hang the GPU
+            const long long t0 = clock64();
+            unsigned long long seen;
+            for (;;) {
+                asm volatile("ld.acquire.gpu.global.u64 %0, [%1];" : "=l"(seen) : "l"(zflag + z) : "memory");
+                if (seen >= flag_target) break;
+                if (clock64() - t0 > STREAM_SPIN_LIMIT) {
+                    atomicMin(err, SLDG_ECUDA);
+                    break;
+                }
+                __nanosleep(256);
+            }
+            asm volatile("fence.proxy.async;" ::: "memory");  // the weights are then read through the async proxy
+        }
     }
     __syncthreads();
     for (int c = tid; c < rows * TX; c += STREAM_THREADS) {
         const int jr = c / TX, ci = c % TX;
         int4 h = make_int4(0, 0, 0, 0);
-        if (i0 + ci < nx) h = __ldg(hdrg + zc + (long long)(j0 + jr) * nx + i0 + ci);
+        if (i0 + ci < nx) h = __ldcg(hdrg + zc + (long long)(j0 + jr) * nx + i0 + ci);
         hdr[c] = h;
         if (h.z) {
             const int wx = (h.z & 0x124) ? 3 : ((h.z & 0x092) ? 2 : 1);
@@ -168,6 +219,7 @@ __global__ void __launch_bounds__(STREAM_THREADS, 1) xy_apply_stream_kernel(
 
     if (!staged) {
         // direct path: warp <-> cell, 64 v values per pass
+        if (tid == 0) atomicAdd(err + 1, 1);  // diagnostic counter 0 (sldg_debug_counter)
         for (int c = warp; c < rows * TX; c += STREAM_THREADS / 32) {
             const int jr = c / TX, ci = c % TX;
             const int4 h = hdr[c];
@@ -189,7 +241,7 @@ __global__ void __launch_bounds__(STREAM_THREADS, 1) xy_apply_stream_kernel(
                     for (int k = 0; k < 4; ++k)
                         in[k] = __ldg(reinterpret_cast<const double2 *>(
                             fz + (long long)(2 * s + (k >> 1)) * g.sY + (long long)(2 * r + (k & 1)) * g.sX + v));
-                    fma_block_o2(acc, in, W + ((size_t)cellid * 9 + nb++) * 16);
+                    fma_block_o2_direct(acc, in, W + ((size_t)cellid * 9 + nb++) * 16);
                 }
 #pragma unroll
                 for (int m = 0; m < 4; ++m)
@@ -201,6 +253,26 @@ __global__ void __launch_bounds__(STREAM_THREADS, 1) xy_apply_stream_kernel(
         return;
     }
 
+    // Headers -> per-target-row descriptors, in place.  A target row jr is touched by the source rows
+    // jr + d, d = 0..2 (relative to aymin); descriptor d = {bits 0-2: mask of the 3 source cells of that row,
+    // bits 3-11: index of its first weight block inside the row's weight stage, bits 12..: first source cell's
+    // position in the x window}; .w = {bits 0-7: offset of the cell's blocks in the stage, bits 8..: count}.
+    for (int c = tid; c < rows * TX; c += STREAM_THREADS) {
+        const int4 h = hdr[c];
+        int dsc[3] = {0, 0, 0};
+        const int bx = (c % TX) + h.x - axmin;
+#pragma unroll
+        for (int d = 0; d < 3; ++d) {
+            const int dy = d - (h.y - aymin);
+            if (h.z && dy >= 0 && dy <= 2) {
+                const int mrow = (h.z >> (3 * dy)) & 7;
+                if (mrow) dsc[d] = mrow | ((h.w + __popc(h.z & ((1 << (3 * dy)) - 1))) << 3) | (bx << 12);
+            }
+        }
+        hdr[c] = make_int4(dsc[0], dsc[1], dsc[2], h.w | (__popc(h.z) << 8));
+    }
+    __syncthreads();
+
     const int nsrc = rows + S - 1;  // source rows y' = 0 .. nsrc-1, Y = j0 + aymin + y'
 
     if (warp == STREAM_CWARPS) {
@@ -209,9 +281,9 @@ __global__ void __launch_bounds__(STREAM_THREADS, 1) xy_apply_stream_kernel(
         const int n1 = min(RW, nx - wx0);               // cells before the periodic seam
         const bool runs = (g.sX == (long long)VL) && RW <= nx;  // window lines contiguous in memory (z,y,x order)
         const uint32_t row_bytes = (uint32_t)(stage_doubles * 8);
+        int st = 0, ph = 1, ws = 0, wph = 1;  // ring slot / parity of the `empty` barriers to wait for
         for (int k = 0; k < nsrc; ++k) {
-            const int st = k % NR;
-            if (k >= NR) mbar_wait(&empty[st], ((k / NR) & 1) ^ 1);
+            if (k >= NR) mbar_wait(&empty[st], ph);
             if (lane == 0) mbar_arrive_expect_tx(&full[st], row_bytes);
             __syncwarp();
             const int sY = wrap_idx(j0 + aymin + k, ny);
@@ -235,16 +307,15 @@ __global__ void __launch_bounds__(STREAM_THREADS, 1) xy_apply_stream_kernel(
                              (uint32_t)(VL * 8), &full[st]);
                 }
             }
+            if (++st == NR) { st = 0; ph ^= 1; }
             // weights of target row k (first used with source row k)
             if (k < rows) {
-                const int ws = k % NW;
-                if (k >= NW) mbar_wait(&wempty[ws], ((k / NW) & 1) ^ 1);
-                const int ci = lane;                      // one packed run of weight blocks per cell
-                int cnt = 0, off = 0;
-                if (ci < TX) {
-                    const int4 h = hdr[k * TX + ci];
-                    cnt = __popc(h.z);
-                    off = h.w;
+                if (k >= NW) mbar_wait(&wempty[ws], wph);
+                int cnt = 0, off = 0;                     // one packed run of weight blocks per cell
+                if (lane < TX) {
+                    const int w = hdr[k * TX + lane].w;
+                    cnt = w >> 8;
+                    off = w & 0xff;
                 }
                 int tot = cnt;
 #pragma unroll
@@ -252,24 +323,35 @@ __global__ void __launch_bounds__(STREAM_THREADS, 1) xy_apply_stream_kernel(
                 if (lane == 0) mbar_arrive_expect_tx(&wfull[ws], (uint32_t)(tot * 128));
                 __syncwarp();
                 if (cnt > 0) {
-                    const long long cellid = zc + (long long)(j0 + k) * nx + i0 + ci;
+                    const long long cellid = zc + (long long)(j0 + k) * nx + i0 + lane;
                     bulk_g2s(wring + ((size_t)ws * STREAM_WROW + off) * 16, W + (size_t)cellid * 9 * 16,
                              (uint32_t)(cnt * 128), &wfull[ws]);
                 }
+                if (++ws == NW) { ws = 0; wph ^= 1; }
             }
         }
         return;
     }
 
-    // ---------------- consumer warps: cell = warp / 2, v half = warp % 2 -------------------------------------
-    const int ci = warp >> 1, vh = warp & 1;
-    const int v = vh * 64 + 2 * lane;
-    const bool live = (i0 + ci < nx) && (v < VL);
-    double acc[NACC][4][2];
+    // ---------------- consumer warps: one per target cell of the strip ---------------------------------------
+    // lane <-> the v pairs (2 lane, 2 lane + 1) and/or (64 + 2 lane, 64 + 2 lane + 1): every shared-memory load of a
+    // warp is a contiguous 512-byte run.  Lanes whose pair lies beyond VL compute on stale ring contents and
+    // never store.
+    const int ci = warp / VSPLIT, vbase = (warp % VSPLIT) * 64 + 2 * lane;
+    const size_t kq_stride = (size_t)2 * RW * VL;
+    double acc[NACC][4][2 * NP];
+    int4 dsc[NACC];
 #pragma unroll
-    for (int a = 0; a < NACC; ++a)
+    for (int a = 0; a < NACC; ++a) {
+        dsc[a] = make_int4(0, 0, 0, 0);
 #pragma unroll
-        for (int m = 0; m < 4; ++m) acc[a][m][0] = acc[a][m][1] = 0.0;
+        for (int m = 0; m < 4; ++m)
+#pragma unroll
+            for (int e = 0; e < 2 * NP; ++e) acc[a][m][e] = 0.0;
+    }
+    int st = 0, ph = 0, ws = 0, wph = 0;  // source ring slot / parity, weight stage / parity (of the `full` barriers)
+    int wsd = 0;                          // weight stage of the target row that is stored next
+    double *orow = oz + (long long)(2 * j0) * g.sY + (long long)(2 * (i0 + ci)) * g.sX + vbase;
 
     // one step: source row k; target rows k, k-1, k-2 (accumulator sets are indexed by row mod 3, static
     // because the step loop is unrolled by 3)
@@ -278,57 +360,63 @@ __global__ void __launch_bounds__(STREAM_THREADS, 1) xy_apply_stream_kernel(
         for (int u = 0; u < NACC; ++u) {
             const int k = kb + u;
             if (k >= rows + NACC - 1) break;
-            if (k < rows) mbar_wait(&wfull[k % NW], (k / NW) & 1);
+            if (k < rows) {
+                // target row k enters: its descriptor and weight stage
+                mbar_wait(&wfull[ws], wph);
+                dsc[u] = hdr[k * TX + ci];
+                const int wb = (ws * STREAM_WROW) << 3;  // block indices become absolute in the weight ring
+                dsc[u].x += wb;
+                dsc[u].y += wb;
+                dsc[u].z += wb;
+                if (++ws == NW) { ws = 0; wph ^= 1; }
+            }
             if (k < nsrc) {
-                const int st = k % NR;
-                mbar_wait(&full[st], (k / NR) & 1);
-                const double *srow = ring + (size_t)st * stage_doubles + v;
+                mbar_wait(&full[st], ph);
+                const double *srow = ring + (size_t)st * stage_doubles + vbase;
 #pragma unroll
                 for (int d = 0; d < NACC; ++d) {
-                    const int jr = k - d;
-                    if (jr < 0 || jr >= rows) continue;
-                    const int4 h = hdr[jr * TX + ci];
-                    const int dy = d - (h.y - aymin);
-                    if (!live || dy < 0 || dy > 2) continue;
-                    const int mrow = (h.z >> (3 * dy)) & 7;
-                    if (!mrow) continue;
-                    const double *Wp = wring + ((size_t)(jr % NW) * STREAM_WROW + h.w +
-                                                __popc(h.z & ((1 << (3 * dy)) - 1))) * 16;
-                    const int bx = ci + h.x - axmin;
+                    const int set = (u - d + NACC) % NACC;
+                    if (k - d < 0 || k - d >= rows) continue;
+                    const int desc = d == 0 ? dsc[set].x : (d == 1 ? dsc[set].y : dsc[set].z);
+                    if (!(desc & 7)) continue;
+                    const double *Wp = wring + ((desc >> 3) & 0x1ff) * 16;
+                    const double *src = srow + (size_t)(2 * (desc >> 12)) * VL;
 #pragma unroll
                     for (int dx = 0; dx < 3; ++dx) {
-                        if (!((mrow >> dx) & 1)) continue;
-                        const double *src = srow + (size_t)(2 * (bx + dx)) * VL;
-                        double2 in[4];
-                        in[0] = *reinterpret_cast<const double2 *>(src);
-                        in[1] = *reinterpret_cast<const double2 *>(src + VL);
-                        in[2] = *reinterpret_cast<const double2 *>(src + (size_t)2 * RW * VL);
-                        in[3] = *reinterpret_cast<const double2 *>(src + (size_t)2 * RW * VL + VL);
-                        fma_block_o2(acc[(u - d + NACC) % NACC], in, Wp);
-                        Wp += 16;
+                        if ((desc >> dx) & 1) {
+                            fma_block_o2<NP>(acc[set], src + (size_t)(2 * dx) * VL, kq_stride, VL, Wp);
+                            Wp += 16;
+                        }
                     }
                 }
                 __syncwarp();
                 if (lane == 0) mbar_arrive(&empty[st]);
+                if (++st == NR) { st = 0; ph ^= 1; }
             }
             // target row k - 2 has seen all its source rows
             const int jd = k - (NACC - 1);
             if (jd >= 0 && jd < rows) {
-                constexpr int unused = 0;
-                (void)unused;
-                double(&a)[4][2] = acc[(u + 1) % NACC];  // (u - 2 + 3) % 3
-                if (live && hdr[jd * TX + ci].z) {
-                    const int i = i0 + ci, j = j0 + jd;
+                const int set = (u + 1) % NACC;  // (u - 2 + 3) % 3
+                if (dsc[set].w >> 8) {
+                    double *o = orow;
 #pragma unroll
-                    for (int m = 0; m < 4; ++m)
-                        __stcs(reinterpret_cast<double2 *>(oz + (long long)(2 * j + (m >> 1)) * g.sY +
-                                                           (long long)(2 * i + (m & 1)) * g.sX + v),
-                               make_double2(a[m][0], a[m][1]));
+                    for (int m = 0; m < 4; ++m) {
+                        double *om = o + (m >> 1) * g.sY + (m & 1) * g.sX;
+#pragma unroll
+                        for (int p = 0; p < NP; ++p)
+                            if (vbase + 64 * p < VL)
+                                __stcs(reinterpret_cast<double2 *>(om + 64 * p),
+                                       make_double2(acc[set][m][2 * p], acc[set][m][2 * p + 1]));
+                    }
                 }
+                orow += 2 * g.sY;
 #pragma unroll
-                for (int m = 0; m < 4; ++m) a[m][0] = a[m][1] = 0.0;
+                for (int m = 0; m < 4; ++m)
+#pragma unroll
+                    for (int e = 0; e < 2 * NP; ++e) acc[set][m][e] = 0.0;
                 __syncwarp();
-                if (lane == 0) mbar_arrive(&wempty[jd % NW]);
+                if (lane == 0) mbar_arrive(&wempty[wsd]);
+                if (++wsd == NW) wsd = 0;
             }
         }
     }
@@ -413,17 +501,23 @@ __global__ void __launch_bounds__(256) xy_apply_direct_kernel(const double *__re
     }
 }
 
-cudaError_t launch_xy_apply(sldg_ctx *c, const double *fin, double *fout)
+bool xy_apply_can_overlap(const sldg_ctx *c) { return c->g.o[0] == 2 && !getenv("SLDG_APPLY_DIRECT"); }
+
+cudaError_t launch_xy_apply(sldg_ctx *c, const double *fin, double *fout, bool wait_flags)
 {
     const GridDev &g = c->g;
     const int O = g.o[0];
-    if (O == 2 && !getenv("SLDG_APPLY_DIRECT")) {
-        auto kern = xy_apply_stream_kernel;
+    if (xy_apply_can_overlap(c)) {
+        static const int vsplit = getenv("SLDG_APPLY_VSPLIT") ? atoi(getenv("SLDG_APPLY_VSPLIT")) : 1;
+        auto kern = vsplit == 1 ? xy_apply_stream_kernel<1> : xy_apply_stream_kernel<2>;
+        const int STREAM_THREADS = 32 * (STREAM_TX * (vsplit == 1 ? 1 : 2) + 1);
         cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)STREAM_SMEM);
         const int L = g.n[1] < STREAM_LMAX ? g.n[1] : STREAM_LMAX;
         const int strips = (g.n[0] + STREAM_TX - 1) / STREAM_TX, segs = (g.n[1] + L - 1) / L;
         dim3 grid((unsigned)(strips * segs), (unsigned)((g.Pv + STREAM_VMAX - 1) / STREAM_VMAX), (unsigned)g.N[2]);
-        kern<<<grid, STREAM_THREADS, STREAM_SMEM, c->stream>>>(fin, fout, c->hdr, c->W, g, L);
+        const unsigned long long target = c->xy_epoch * (unsigned long long)xy_geometry_blocks_per_z(c);
+        kern<<<grid, STREAM_THREADS, STREAM_SMEM, c->stream>>>(fin, fout, c->hdr, c->W, g, L,
+                                                               wait_flags ? c->zflag : nullptr, target, c->err);
         c->launches++;
         return cudaGetLastError();
     }

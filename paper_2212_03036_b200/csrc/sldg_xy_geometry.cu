@@ -209,19 +209,14 @@ __device__ __forceinline__ void piece_moments(const QuadEdges &q, double offx, d
 }
 
 template <int O>
-__global__ void __launch_bounds__(O == 3 ? 64 : 128) xy_geometry_kernel(const double *__restrict__ va,
-                                                                         const double *__restrict__ vb,
-                                                                         int4 *__restrict__ hdr,
-                                                                         double *__restrict__ W, int32_t *err,
-                                                                         GridDev g, Basis bs, double tau, int order,
-                                                                         int periodic)
+__device__ __forceinline__ void geometry_cell(const double *__restrict__ va, const double *__restrict__ vb,
+                                              int4 *__restrict__ hdr, double *__restrict__ W, int32_t *err,
+                                              const GridDev &g, const Basis &bs, double tau, int order,
+                                              int periodic, int t, int z)
 {
     constexpr int O2 = O * O, NM = 2 * O - 1;
     const int nx = g.n[0], ny = g.n[1];
     const int ncell = nx * ny;
-    const int t = blockIdx.x * blockDim.x + threadIdx.x;
-    if (t >= ncell) return;
-    const int z = blockIdx.y;
     const long long cellid = (long long)z * ncell + t;
     const int i = t % nx, j = t / nx;
     const long long vplane = (long long)(ny + 1) * (nx + 1);
@@ -410,6 +405,26 @@ __global__ void __launch_bounds__(O == 3 ? 64 : 128) xy_geometry_kernel(const do
     hdr[cellid] = make_int4(r0, s0, msk, cnt);
 }
 
+constexpr int GEOM_THREADS = 128;
+template <int O>
+__global__ void __launch_bounds__(O == 3 ? 64 : GEOM_THREADS) xy_geometry_kernel(const double *__restrict__ va,
+                                                                   const double *__restrict__ vb,
+                                                                   int4 *__restrict__ hdr, double *__restrict__ W,
+                                                                   int32_t *err, unsigned long long *zflag,
+                                                                   GridDev g, Basis bs, double tau, int order,
+                                                                   int periodic)
+{
+    const int t = blockIdx.x * blockDim.x + threadIdx.x;
+    const int z = blockIdx.y;
+    if (t < g.n[0] * g.n[1]) geometry_cell<O>(va, vb, hdr, W, err, g, bs, tau, order, periodic, t, z);
+    // publish: all writes of this block, then one release increment of the z node's counter
+    __syncthreads();
+    if (threadIdx.x == 0) {
+        __threadfence();
+        atomicAdd(zflag + z, 1ull);
+    }
+}
+
 // debug/test helper: expand the packed weight blocks of one z plane to the dense [cell][slot] form
 __global__ void geometry_expand_kernel(const int4 *__restrict__ hdr, const double *__restrict__ W, int ncell, int o4,
                                        int32_t *__restrict__ anchor, int32_t *__restrict__ mask,
@@ -436,16 +451,22 @@ __global__ void geometry_expand_kernel(const int4 *__restrict__ hdr, const doubl
 
 }  // namespace
 
-cudaError_t launch_xy_geometry(sldg_ctx *c, double tau, int trace_order)
+int xy_geometry_blocks_per_z(const sldg_ctx *c)
+{
+    const int ncell = c->g.n[0] * c->g.n[1];
+    const int threads = c->g.o[0] == 3 ? 64 : GEOM_THREADS;
+    return (ncell + threads - 1) / threads;
+}
+
+cudaError_t launch_xy_geometry(sldg_ctx *c, cudaStream_t stream, double tau, int trace_order)
 {
     const GridDev &g = c->g;
-    const int ncell = g.n[0] * g.n[1];
     const int O = g.o[0];
-    const int threads = O == 3 ? 64 : 128;
-    dim3 grid((unsigned)((ncell + threads - 1) / threads), (unsigned)g.N[2]);
-#define LAUNCH_G(OO)                                                                                         \
-    xy_geometry_kernel<OO><<<grid, threads, 0, c->stream>>>(c->va, c->vb, c->hdr, c->W, c->err, g, c->basis, \
-                                                            tau, trace_order, c->vel_periodic)
+    const int threads = O == 3 ? 64 : GEOM_THREADS;
+    dim3 grid((unsigned)xy_geometry_blocks_per_z(c), (unsigned)g.N[2]);
+#define LAUNCH_G(OO)                                                                                   \
+    xy_geometry_kernel<OO><<<grid, threads, 0, stream>>>(c->va, c->vb, c->hdr, c->W, c->err, c->zflag, \
+                                                         g, c->basis, tau, trace_order, c->vel_periodic)
     if (O == 1) LAUNCH_G(1); else if (O == 2) LAUNCH_G(2); else LAUNCH_G(3);
 #undef LAUNCH_G
     c->launches++;
