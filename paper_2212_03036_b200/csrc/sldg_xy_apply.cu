@@ -256,7 +256,7 @@ __global__ void __launch_bounds__(32 * (STREAM_TX * VSPLIT + 1), 1) xy_apply_str
     // Headers -> per-target-row descriptors, in place.  A target row jr is touched by the source rows
     // jr + d, d = 0..2 (relative to aymin); descriptor d = {bits 0-2: mask of the 3 source cells of that row,
     // bits 3-11: index of its first weight block inside the row's weight stage, bits 12..: first source cell's
-    // position in the x window}; .w = {bits 0-7: offset of the cell's blocks in the stage, bits 8..: count}.
+    // position in the x window}; .w = {bits 0-7: offset of the cell's blocks in the stage, bits 8-16: slot mask}.
     for (int c = tid; c < rows * TX; c += STREAM_THREADS) {
         const int4 h = hdr[c];
         int dsc[3] = {0, 0, 0};
@@ -269,7 +269,7 @@ __global__ void __launch_bounds__(32 * (STREAM_TX * VSPLIT + 1), 1) xy_apply_str
                 if (mrow) dsc[d] = mrow | ((h.w + __popc(h.z & ((1 << (3 * dy)) - 1))) << 3) | (bx << 12);
             }
         }
-        hdr[c] = make_int4(dsc[0], dsc[1], dsc[2], h.w | (__popc(h.z) << 8));
+        hdr[c] = make_int4(dsc[0], dsc[1], dsc[2], h.w | (h.z << 8));
     }
     __syncthreads();
 
@@ -314,7 +314,7 @@ __global__ void __launch_bounds__(32 * (STREAM_TX * VSPLIT + 1), 1) xy_apply_str
                 int cnt = 0, off = 0;                     // one packed run of weight blocks per cell
                 if (lane < TX) {
                     const int w = hdr[k * TX + lane].w;
-                    cnt = w >> 8;
+                    cnt = __popc(w >> 8);
                     off = w & 0xff;
                 }
                 int tot = cnt;

@@ -1,7 +1,7 @@
 // sldg_xy_geometry.cu -- geometry of the 2d SLDG step in the poloidal plane (Algorithm 3
 // PAPER.md:287-293): everything of eq. (14)-(18) that does not depend on v.
 //
-//   thread <-> one (z node, target cell).  Per cell, once:
+//   Per (z node, target cell), once:
 //     step 1  back-trace the four corners (eq. 14/15) -> upstream quadrilateral, its
 //             bounding box -> anchor (r0,s0) and the candidate source cells (Table 4 step 1);
 //     step 4  back-trace the o^2 Gauss-Legendre nodes, invert the Vandermonde matrix in centred
@@ -33,6 +33,11 @@ __device__ __forceinline__ int wrap_idx(int i, int n)
     int r = i % n;
     return r < 0 ? r + n : r;
 }
+
+// min / max as one compare + select.  fmin()/fmax() cost ~8 instructions each in fp64 on sm_100a (NaN
+// handling); nothing here can be NaN.
+__device__ __forceinline__ double dmin(double a, double b) { return a < b ? a : b; }
+__device__ __forceinline__ double dmax(double a, double b) { return a > b ? a : b; }
 
 // piecewise-bilinear velocity of cell (ci,cj) at local (xi,eta)
 __device__ __forceinline__ void bilinear_vel(const double *__restrict__ a, const double *__restrict__ b,
@@ -102,7 +107,7 @@ __device__ __forceinline__ double gauss_jordan(double (&V)[N][N], double (&X)[N]
                 }
             }
         }
-        minpiv = fmin(minpiv, best);
+        minpiv = dmin(minpiv, best);
         const double inv = 1.0 / V[c][c];
 #pragma unroll
         for (int k = 0; k < N; ++k) {
@@ -150,9 +155,9 @@ __device__ __forceinline__ void piece_moments(const QuadEdges &q, double offx, d
         // crossing with the line x = 1 (for the inner segment); decided from the actual end points
         const double x1 = q.x0[(e + 1) & 3] - offx;
         if (inner_right && dx != 0.0 && (x0 - 1.0) * (x1 - 1.0) <= 0.0) {
-            const double yc = fma(fmin(fmax((1.0 - x0) * q.idx[e], 0.0), 1.0), dy, y0);
-            ylo = fmin(ylo, yc);
-            yhi = fmax(yhi, yc);
+            const double yc = fma(dmin(dmax((1.0 - x0) * q.idx[e], 0.0), 1.0), dy, y0);
+            ylo = dmin(ylo, yc);
+            yhi = dmax(yhi, yc);
         }
         // outer segment: Liang-Barsky clip of the edge against the closed unit square
         double t0 = 0.0, t1 = 1.0;
@@ -161,17 +166,17 @@ __device__ __forceinline__ void piece_moments(const QuadEdges &q, double offx, d
             ok = ok && x0 >= 0.0 && x0 <= 1.0;
         } else {
             const double ta = -x0 * q.idx[e], tb = (1.0 - x0) * q.idx[e];
-            t0 = fmax(t0, fmin(ta, tb));
-            t1 = fmin(t1, fmax(ta, tb));
+            t0 = dmax(t0, dmin(ta, tb));
+            t1 = dmin(t1, dmax(ta, tb));
         }
         {
             const double ta = -y0 * q.idy[e], tb = (1.0 - y0) * q.idy[e];
-            t0 = fmax(t0, fmin(ta, tb));
-            t1 = fmin(t1, fmax(ta, tb));
+            t0 = dmax(t0, dmin(ta, tb));
+            t1 = dmin(t1, dmax(ta, tb));
         }
         if (ok && t1 > t0) {
-            const double xa = fmin(fmax(fma(t0, dx, x0), 0.0), 1.0), ya = fmin(fmax(fma(t0, dy, y0), 0.0), 1.0);
-            const double xb = fmin(fmax(fma(t1, dx, x0), 0.0), 1.0), yb = fmin(fmax(fma(t1, dy, y0), 0.0), 1.0);
+            const double xa = dmin(dmax(fma(t0, dx, x0), 0.0), 1.0), ya = dmin(dmax(fma(t0, dy, y0), 0.0), 1.0);
+            const double xb = dmin(dmax(fma(t1, dx, x0), 0.0), 1.0), yb = dmin(dmax(fma(t1, dy, y0), 0.0), 1.0);
             const double ex = xb - xa, ey = yb - ya;
 #pragma unroll
             for (int gq = 0; gq < NM; ++gq) {  // (2o-1)-point Gauss rule: exact for degree 4o-3
@@ -193,7 +198,7 @@ __device__ __forceinline__ void piece_moments(const QuadEdges &q, double offx, d
         }
     }
     if (inner_right) {
-        const double ya = fmax(ylo, 0.0), yb = fmin(yhi, 1.0);
+        const double ya = dmax(ylo, 0.0), yb = dmin(yhi, 1.0);
         if (yb > ya) {
             double pa = ya, pb = yb;  // y^{q+1}
 #pragma unroll
@@ -208,16 +213,37 @@ __device__ __forceinline__ void piece_moments(const QuadEdges &q, double offx, d
     }
 }
 
+// ---------------------------------------------------------------------------------------------------------
+// Two phases per block of GEOM_CELLS target cells of one z node, handing over through shared memory:
+//   phase 1, thread <-> target cell: steps 1 and 4 (corner feet, bounding box, node feet, inverse Vandermonde);
+//   phase 2, thread <-> work item = (target cell, candidate source cell of its bounding box): steps 2, 3, 5
+//            (clipped edges, moments, contraction) for ONE piece.  The items of the block are enumerated
+//            densely (prefix sum of the per-cell candidate counts), so a warp never idles on a cell with fewer
+//            candidates than its neighbours', and each phase keeps only its own state in registers.
+// The non-empty pieces of a cell are stored packed in slot order, W[cell][0 .. count); the header's mask says
+// which slots they are.
+// ---------------------------------------------------------------------------------------------------------
 template <int O>
-__device__ __forceinline__ void geometry_cell(const double *__restrict__ va, const double *__restrict__ vb,
-                                              int4 *__restrict__ hdr, double *__restrict__ W, int32_t *err,
-                                              const GridDev &g, const Basis &bs, double tau, int order,
-                                              int periodic, int t, int z)
+struct GeomShared {
+    static constexpr int O2 = O * O;
+    static constexpr int CELLS = O == 3 ? 64 : 128;
+    // structure of arrays, [field][cell]: phase 1 writes with consecutive lanes on consecutive words
+    double cx[4][CELLS], cy[4][CELLS];     // corner feet relative to the anchor cell, cell units
+    double idx[4][CELLS], idy[4][CELLS];   // reciprocals of the edge direction components (0 if the component is 0)
+    double Vi[O2 * O2][CELLS];             // inverse Vandermonde, Vi[ab * O2 + m]
+    double xc[CELLS], yc[CELLS];           // centre of the node feet
+    int r0[CELLS], s0[CELLS], nr[CELLS], ns[CELLS], mask[CELLS];
+    unsigned short item[CELLS * 11];       // work item -> cell | candidate index << 8, 0xffff = padding
+    int warp_tot[8];
+};
+
+template <int O>
+__device__ __forceinline__ int geometry_setup(const double *__restrict__ va, const double *__restrict__ vb, int32_t *err,
+                                              const GridDev &g, const Basis &bs, double tau, int order, int periodic,
+                                              int t, int z, GeomShared<O> &sh, int c)
 {
-    constexpr int O2 = O * O, NM = 2 * O - 1;
+    constexpr int O2 = O * O;
     const int nx = g.n[0], ny = g.n[1];
-    const int ncell = nx * ny;
-    const long long cellid = (long long)z * ncell + t;
     const int i = t % nx, j = t / nx;
     const long long vplane = (long long)(ny + 1) * (nx + 1);
     const double *a = va + z * vplane, *b = vb + z * vplane;
@@ -229,36 +255,36 @@ __device__ __forceinline__ void geometry_cell(const double *__restrict__ va, con
     trace_point(a, b, nx, ny, tx, ty, i, j, 1.0, 0.0, order, periodic, cx[1], cy[1]);
     trace_point(a, b, nx, ny, tx, ty, i, j, 1.0, 1.0, order, periodic, cx[2], cy[2]);
     trace_point(a, b, nx, ny, tx, ty, i, j, 0.0, 1.0, order, periodic, cx[3], cy[3]);
-    const double xmin = fmin(fmin(cx[0], cx[1]), fmin(cx[2], cx[3]));
-    const double ymin = fmin(fmin(cy[0], cy[1]), fmin(cy[2], cy[3]));
+    const double xmin = dmin(dmin(cx[0], cx[1]), dmin(cx[2], cx[3]));
+    const double ymin = dmin(dmin(cy[0], cy[1]), dmin(cy[2], cy[3]));
     const int r0 = (int)floor(xmin), s0 = (int)floor(ymin);
     int nr, ns;  // the bounding box covers source cells r0 .. r0+nr, s0 .. s0+ns
-    QuadEdges q;
     {
         // Corners relative to the anchor cell (keeps |coordinates| <= 4).  Everything below -- edge
         // directions, clip parameters, crossings -- is derived from these rounded coordinates only, so
         // that the clipped pieces of neighbouring source cells fit together exactly.
+        double qx[4], qy[4];
 #pragma unroll
         for (int e = 0; e < 4; ++e) {
-            q.x0[e] = cx[e] - r0;
-            q.y0[e] = cy[e] - s0;
+            qx[e] = cx[e] - r0;
+            qy[e] = cy[e] - s0;
+            sh.cx[e][c] = qx[e];
+            sh.cy[e][c] = qy[e];
         }
         bool convex = true;
 #pragma unroll
         for (int e = 0; e < 4; ++e) {
-            const double e1x = q.x0[(e + 1) & 3] - q.x0[e], e1y = q.y0[(e + 1) & 3] - q.y0[e];
-            const double e2x = q.x0[(e + 2) & 3] - q.x0[(e + 1) & 3], e2y = q.y0[(e + 2) & 3] - q.y0[(e + 1) & 3];
+            const double e1x = qx[(e + 1) & 3] - qx[e], e1y = qy[(e + 1) & 3] - qy[e];
+            const double e2x = qx[(e + 2) & 3] - qx[(e + 1) & 3], e2y = qy[(e + 2) & 3] - qy[(e + 1) & 3];
             if (!(e1x * e2y - e1y * e2x > 0.0)) convex = false;
-            q.dx[e] = e1x;
-            q.dy[e] = e1y;
-            q.idx[e] = e1x != 0.0 ? 1.0 / e1x : 0.0;
-            q.idy[e] = e1y != 0.0 ? 1.0 / e1y : 0.0;
+            sh.idx[e][c] = e1x != 0.0 ? 1.0 / e1x : 0.0;
+            sh.idy[e][c] = e1y != 0.0 ? 1.0 / e1y : 0.0;
         }
         if (!convex) atomicMin(err, SLDG_EGEOM);
         // half-open bounding box, taken from the same rounded coordinates (a foot exactly on a grid line
         // does not add a zero-area column, R12)
-        const double xmax = fmax(fmax(q.x0[0], q.x0[1]), fmax(q.x0[2], q.x0[3]));
-        const double ymax = fmax(fmax(q.y0[0], q.y0[1]), fmax(q.y0[2], q.y0[3]));
+        const double xmax = dmax(dmax(qx[0], qx[1]), dmax(qx[2], qx[3]));
+        const double ymax = dmax(dmax(qy[0], qy[1]), dmax(qy[2], qy[3]));
         nr = max((int)ceil(xmax) - 1, 0);
         ns = max((int)ceil(ymax) - 1, 0);
         if (nr > 2 || ns > 2) {
@@ -267,6 +293,11 @@ __device__ __forceinline__ void geometry_cell(const double *__restrict__ va, con
             ns = min(ns, 2);
         }
     }
+    sh.r0[c] = r0;
+    sh.s0[c] = s0;
+    sh.nr[c] = nr;
+    sh.ns[c] = ns;
+    sh.mask[c] = 0;
 
     // step 4: node feet and adjoint polynomials in centred coordinates (relative to the anchor cell)
     double Vi[O2][O2], xc = 0.0, yc = 0.0;
@@ -305,118 +336,188 @@ __device__ __forceinline__ void geometry_cell(const double *__restrict__ va, con
         const double minpiv = gauss_jordan<O2>(V, Vi);  // phi*_m = sum_ab Vi[ab][m] (x-xc)^a (y-yc)^b
         if (!(minpiv > 1e-10)) atomicMin(err, SLDG_EGEOM);
     }
+    sh.xc[c] = xc;
+    sh.yc[c] = yc;
+#pragma unroll
+    for (int ab = 0; ab < O2; ++ab)
+#pragma unroll
+        for (int m = 0; m < O2; ++m) sh.Vi[ab * O2 + m][c] = Vi[ab][m];
+    return (nr + 1) * (ns + 1);
+}
+
+// steps 2, 3, 5 for one piece: target cell c of the block, candidate source cell (dr, ds) of its bounding box
+// The pieces of one target cell sit on consecutive lanes of one warp, in slot order (k = candidate index of the
+// lane): the non-empty ones are stored packed, W[cell][rank], rank from a warp ballot.  `valid` is false on padding
+// lanes, which only take part in the ballot.
+template <int O>
+__device__ __forceinline__ void geometry_piece(const GeomShared<O> &sh, bool valid, int c, int k, int dr, int ds,
+                                               const Basis &bs, double *__restrict__ Wcell, int *mask_out)
+{
+    constexpr int O2 = O * O, NM = 2 * O - 1;
+    const int lane = threadIdx.x & 31;
+    if (!valid) c = 0;
+    QuadEdges q;
+#pragma unroll
+    for (int e = 0; e < 4; ++e) {
+        q.x0[e] = sh.cx[e][c];
+        q.y0[e] = sh.cy[e][c];
+        q.idx[e] = sh.idx[e][c];
+        q.idy[e] = sh.idy[e][c];
+    }
+#pragma unroll
+    for (int e = 0; e < 4; ++e) {
+        q.dx[e] = q.x0[(e + 1) & 3] - q.x0[e];
+        q.dy[e] = q.y0[(e + 1) & 3] - q.y0[e];
+    }
+    double M[NM][NM];
+    piece_moments<O>(q, (double)dr, (double)ds, dr < sh.nr[c], bs, M);
+    const bool nonempty = valid && M[0][0] > 0.0;
+    const unsigned ballot = __ballot_sync(0xffffffffu, nonempty);
+    if (!nonempty) return;  // empty intersection
+    const int rank = __popc((ballot >> (lane - k)) & ((1u << k) - 1u));
+    // phi*_m in the source cell's monomials: (x-xc)^a = sum_a' binom(a,a') (-xc)^(a-a') x^a'
+    const double lxc = sh.xc[c] - dr, lyc = sh.yc[c] - ds;
+    double cf[O2][O2];  // cf[a'+O b'][m]
+    {
+        double sxp[O][O], syp[O][O];  // sxp[a][a'] = binom(a,a') (-lxc)^(a-a')
+#pragma unroll
+        for (int aa = 0; aa < O; ++aa)
+#pragma unroll
+            for (int ap = 0; ap < O; ++ap) {
+                const double bin = (ap > aa) ? 0.0 : ((aa == 2 && ap == 1) ? 2.0 : 1.0);
+                double px = 1.0, py = 1.0;
+#pragma unroll
+                for (int e = 0; e < O; ++e)
+                    if (e < aa - ap) {
+                        px *= -lxc;
+                        py *= -lyc;
+                    }
+                sxp[aa][ap] = bin * px;
+                syp[aa][ap] = bin * py;
+            }
+#pragma unroll
+        for (int m = 0; m < O2; ++m)
+#pragma unroll
+            for (int bp_ = 0; bp_ < O; ++bp_)
+#pragma unroll
+                for (int ap = 0; ap < O; ++ap) {
+                    double acc = 0.0;
+#pragma unroll
+                    for (int bb = bp_; bb < O; ++bb)
+#pragma unroll
+                        for (int aa = ap; aa < O; ++aa)
+                            acc = fma(sh.Vi[(aa + O * bb) * O2 + m][c], sxp[aa][ap] * syp[bb][bp_], acc);
+                    cf[ap + O * bp_][m] = acc;
+                }
+    }
+    // G[k][a'+O b'] = int phi_k x^a' y^b' = sum_{p',q'} L[kp][p'] L[kq][q'] M[p'+a'][q'+b']  (separable)
+    double T[O][O][NM];  // T[kp][a'][q] = sum_p' L[kp][p'] M[p'+a'][q]
+#pragma unroll
+    for (int kp = 0; kp < O; ++kp)
+#pragma unroll
+        for (int ap = 0; ap < O; ++ap)
+#pragma unroll
+            for (int qq = 0; qq < NM; ++qq) {
+                double acc = 0.0;
+#pragma unroll
+                for (int pp = 0; pp < O; ++pp) acc = fma(bs.L[O][kp][pp], M[pp + ap][qq], acc);
+                T[kp][ap][qq] = acc;
+            }
     double iw[O2];
 #pragma unroll
     for (int m = 0; m < O2; ++m) iw[m] = 1.0 / (bs.w[O][m % O] * bs.w[O][m / O]);
-
-    // steps 2, 3, 5: one candidate source cell at a time
-    int msk = 0, cnt = 0;
-    double *Wcell = W + (size_t)cellid * 9 * (O2 * O2);
-#pragma unroll 1
-    for (int ds = 0; ds <= ns; ++ds)
-#pragma unroll 1
-        for (int dr = 0; dr <= nr; ++dr) {
-            double M[NM][NM];
-            piece_moments<O>(q, (double)dr, (double)ds, dr < nr, bs, M);
-            if (!(M[0][0] > 0.0)) continue;  // empty intersection
-            // phi*_m in the source cell's monomials: (x-xc)^a = sum_a' binom(a,a') (-xc)^(a-a') x^a'
-            const double lxc = xc - dr, lyc = yc - ds;
-            double cf[O2][O2];  // cf[a'+O b'][m]
-            {
-                double sxp[O][O], syp[O][O];  // sxp[a][a'] = binom(a,a') (-lxc)^(a-a')
+    const int slot = dr + 3 * ds;
+    double *Wout = Wcell + (size_t)rank * (O2 * O2);
 #pragma unroll
-                for (int aa = 0; aa < O; ++aa)
+    for (int kq = 0; kq < O; ++kq)
 #pragma unroll
-                    for (int ap = 0; ap < O; ++ap) {
-                        const double bin = (ap > aa) ? 0.0 : ((aa == 2 && ap == 1) ? 2.0 : 1.0);
-                        double px = 1.0, py = 1.0;
+        for (int kp = 0; kp < O; ++kp) {
+            double G[O2];
 #pragma unroll
-                        for (int e = 0; e < O; ++e)
-                            if (e < aa - ap) {
-                                px *= -lxc;
-                                py *= -lyc;
-                            }
-                        sxp[aa][ap] = bin * px;
-                        syp[aa][ap] = bin * py;
-                    }
+            for (int bp_ = 0; bp_ < O; ++bp_)
 #pragma unroll
-                for (int m = 0; m < O2; ++m)
+                for (int ap = 0; ap < O; ++ap) {
+                    double acc = 0.0;
 #pragma unroll
-                    for (int bp_ = 0; bp_ < O; ++bp_)
-#pragma unroll
-                        for (int ap = 0; ap < O; ++ap) {
-                            double acc = 0.0;
-#pragma unroll
-                            for (int bb = bp_; bb < O; ++bb)
-#pragma unroll
-                                for (int aa = ap; aa < O; ++aa)
-                                    acc = fma(Vi[aa + O * bb][m], sxp[aa][ap] * syp[bb][bp_], acc);
-                            cf[ap + O * bp_][m] = acc;
-                        }
-            }
-            // G[k][a'+O b'] = int phi_k x^a' y^b' = sum_{p',q'} L[kp][p'] L[kq][q'] M[p'+a'][q'+b']  (separable)
-            double T[O][O][NM];  // T[kp][a'][q] = sum_p' L[kp][p'] M[p'+a'][q]
-#pragma unroll
-            for (int kp = 0; kp < O; ++kp)
-#pragma unroll
-                for (int ap = 0; ap < O; ++ap)
-#pragma unroll
-                    for (int qq = 0; qq < NM; ++qq) {
-                        double acc = 0.0;
-#pragma unroll
-                        for (int pp = 0; pp < O; ++pp) acc = fma(bs.L[O][kp][pp], M[pp + ap][qq], acc);
-                        T[kp][ap][qq] = acc;
-                    }
-            double *Wout = Wcell + (size_t)cnt * (O2 * O2);
-#pragma unroll
-            for (int kq = 0; kq < O; ++kq)
-#pragma unroll
-                for (int kp = 0; kp < O; ++kp) {
-                    double G[O2];
-#pragma unroll
-                    for (int bp_ = 0; bp_ < O; ++bp_)
-#pragma unroll
-                        for (int ap = 0; ap < O; ++ap) {
-                            double acc = 0.0;
-#pragma unroll
-                            for (int qq = 0; qq < O; ++qq) acc = fma(bs.L[O][kq][qq], T[kp][ap][qq + bp_], acc);
-                            G[ap + O * bp_] = acc;
-                        }
-                    const int k = kp + O * kq;
-                    double out[O2];
-#pragma unroll
-                    for (int m = 0; m < O2; ++m) {
-                        double acc = 0.0;
-#pragma unroll
-                        for (int ab = 0; ab < O2; ++ab) acc = fma(cf[ab][m], G[ab], acc);
-                        out[m] = acc * iw[m];
-                    }
-                    if (O == 2) {
-                        reinterpret_cast<double2 *>(Wout + k * O2)[0] = make_double2(out[0], out[1]);
-                        reinterpret_cast<double2 *>(Wout + k * O2)[1] = make_double2(out[O2 - 2], out[O2 - 1]);
-                    } else {
-#pragma unroll
-                        for (int m = 0; m < O2; ++m) Wout[k * O2 + m] = out[m];
-                    }
+                    for (int qq = 0; qq < O; ++qq) acc = fma(bs.L[O][kq][qq], T[kp][ap][qq + bp_], acc);
+                    G[ap + O * bp_] = acc;
                 }
-            msk |= 1 << (dr + 3 * ds);
-            ++cnt;
+            const int k = kp + O * kq;
+            double out[O2];
+#pragma unroll
+            for (int m = 0; m < O2; ++m) {
+                double acc = 0.0;
+#pragma unroll
+                for (int ab = 0; ab < O2; ++ab) acc = fma(cf[ab][m], G[ab], acc);
+                out[m] = acc * iw[m];
+            }
+            if (O == 2) {
+                reinterpret_cast<double2 *>(Wout + k * O2)[0] = make_double2(out[0], out[1]);
+                reinterpret_cast<double2 *>(Wout + k * O2)[1] = make_double2(out[O2 - 2], out[O2 - 1]);
+            } else {
+#pragma unroll
+                for (int m = 0; m < O2; ++m) Wout[k * O2 + m] = out[m];
+            }
         }
-    hdr[cellid] = make_int4(r0, s0, msk, cnt);
+    atomicOr(mask_out, 1 << slot);
 }
 
-constexpr int GEOM_THREADS = 128;
 template <int O>
-__global__ void __launch_bounds__(O == 3 ? 64 : GEOM_THREADS) xy_geometry_kernel(const double *__restrict__ va,
-                                                                   const double *__restrict__ vb,
-                                                                   int4 *__restrict__ hdr, double *__restrict__ W,
-                                                                   int32_t *err, unsigned long long *zflag,
-                                                                   GridDev g, Basis bs, double tau, int order,
-                                                                   int periodic)
+__global__ void __launch_bounds__(GeomShared<O>::CELLS) xy_geometry_kernel(const double *__restrict__ va,
+                                                                           const double *__restrict__ vb,
+                                                                           int4 *__restrict__ hdr, double *__restrict__ W,
+                                                                           int32_t *err, unsigned long long *zflag,
+                                                                           GridDev g, Basis bs, double tau, int order,
+                                                                           int periodic)
 {
-    const int t = blockIdx.x * blockDim.x + threadIdx.x;
+    constexpr int CELLS = GeomShared<O>::CELLS, O4 = O * O * O * O;
+    extern __shared__ __align__(16) unsigned char geom_smem[];
+    GeomShared<O> &sh = *reinterpret_cast<GeomShared<O> *>(geom_smem);
+    const int c = threadIdx.x, lane = c & 31, warp = c >> 5;
+    const int ncell = g.n[0] * g.n[1];
+    const int t = blockIdx.x * CELLS + c;
     const int z = blockIdx.y;
-    if (t < g.n[0] * g.n[1]) geometry_cell<O>(va, vb, hdr, W, err, g, bs, tau, order, periodic, t, z);
+
+    // phase 1: per-cell set-up, number of candidate source cells
+    const int n = t < ncell ? geometry_setup<O>(va, vb, err, g, bs, tau, order, periodic, t, z, sh, c) : 0;
+    // Enumerate the work items: the cells of a warp in order, a cell's items on consecutive lanes of ONE warp
+    // (padded to the next multiple of 32 where they would straddle), each warp's list rounded up to 32.
+    int first = 0, pos = 0;
+#pragma unroll 1
+    for (int l = 0; l < 32; ++l) {
+        const int nl = __shfl_sync(0xffffffffu, n, l);
+        if ((pos & 31) + nl > 32) pos = (pos + 31) & ~31;
+        if (lane == l) first = pos;
+        pos += nl;
+    }
+    pos = (pos + 31) & ~31;
+    if (lane == 0) sh.warp_tot[warp] = pos;
+    __syncthreads();
+    int base = 0, total = 0;
+    for (int w = 0; w < CELLS / 32; ++w) {
+        if (w < warp) base += sh.warp_tot[w];
+        total += sh.warp_tot[w];
+    }
+    for (int it = c; it < total; it += CELLS) sh.item[it] = 0xffff;
+    __syncthreads();
+    for (int k = 0; k < n; ++k) sh.item[base + first + k] = (unsigned short)(c | (k << 8));
+    __syncthreads();
+
+    // phase 2: one piece per thread and pass (whole warps: total is a multiple of 32)
+    for (int it = c; it < total; it += CELLS) {
+        const int code = sh.item[it];
+        const bool valid = code != 0xffff;
+        const int cc = valid ? (code & 0xff) : 0, k = valid ? (code >> 8) : 0;
+        const int w = sh.nr[cc] + 1;
+        const int ds = k / w, dr = k - ds * w;
+        const long long cellid = (long long)z * ncell + blockIdx.x * CELLS + cc;
+        geometry_piece<O>(sh, valid, cc, k, dr, ds, bs, W + (size_t)cellid * 9 * O4, &sh.mask[cc]);
+    }
+    __syncthreads();
+    if (t < ncell) {
+        const int m = sh.mask[c];
+        hdr[(long long)z * ncell + t] = make_int4(sh.r0[c], sh.s0[c], m, __popc(m));
+    }
     // publish: all writes of this block, then one release increment of the z node's counter
     __syncthreads();
     if (threadIdx.x == 0) {
@@ -454,7 +555,7 @@ __global__ void geometry_expand_kernel(const int4 *__restrict__ hdr, const doubl
 int xy_geometry_blocks_per_z(const sldg_ctx *c)
 {
     const int ncell = c->g.n[0] * c->g.n[1];
-    const int threads = c->g.o[0] == 3 ? 64 : GEOM_THREADS;
+    const int threads = c->g.o[0] == 3 ? GeomShared<3>::CELLS : GeomShared<2>::CELLS;
     return (ncell + threads - 1) / threads;
 }
 
@@ -462,11 +563,14 @@ cudaError_t launch_xy_geometry(sldg_ctx *c, cudaStream_t stream, double tau, int
 {
     const GridDev &g = c->g;
     const int O = g.o[0];
-    const int threads = O == 3 ? 64 : GEOM_THREADS;
     dim3 grid((unsigned)xy_geometry_blocks_per_z(c), (unsigned)g.N[2]);
-#define LAUNCH_G(OO)                                                                                   \
-    xy_geometry_kernel<OO><<<grid, threads, 0, stream>>>(c->va, c->vb, c->hdr, c->W, c->err, c->zflag, \
-                                                         g, c->basis, tau, trace_order, c->vel_periodic)
+#define LAUNCH_G(OO)                                                                                              \
+    do {                                                                                                          \
+        auto kern = xy_geometry_kernel<OO>;                                                                       \
+        cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)sizeof(GeomShared<OO>));     \
+        kern<<<grid, GeomShared<OO>::CELLS, sizeof(GeomShared<OO>), stream>>>(                                    \
+            c->va, c->vb, c->hdr, c->W, c->err, c->zflag, g, c->basis, tau, trace_order, c->vel_periodic);        \
+    } while (0)
     if (O == 1) LAUNCH_G(1); else if (O == 2) LAUNCH_G(2); else LAUNCH_G(3);
 #undef LAUNCH_G
     c->launches++;
