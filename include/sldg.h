@@ -108,7 +108,10 @@ int sldg_charge_density(sldg_ctx *ctx, double *rho_dev);
 int sldg_mass(sldg_ctx *ctx, double *mass_dev);
 /* One Strang step with the fields currently set (Algorithm 1 steps 3,4,6,7,8; the
  * source terms vanish for the Cartesian full-f formulation):
- *   advect_z(dt/2), advect_v(dt/2), advect_xy(dt), advect_v(dt/2), advect_z(dt/2). */
+ *   advect_z(dt/2), advect_v(dt/2), advect_xy(dt), advect_v(dt/2), advect_z(dt/2).
+ * The result is bit-identical to those five calls.  Where the (z,v) plane of one (x,y) node fits in shared
+ * memory, each pair of adjacent sweeps runs as ONE kernel that reads and writes f once (3 passes over f per
+ * step instead of 5); environment variable SLDG_NO_FUSE at sldg_create time disables that. */
 int sldg_strang_step(sldg_ctx *ctx, double dt);
 int sldg_set_trace_order(sldg_ctx *ctx, int trace_order); /* used by sldg_strang_step; default 2 */
 
@@ -125,8 +128,9 @@ int sldg_check(sldg_ctx *ctx);
 /* Device times (CUDA events) of the last sldg_strang_step, in ms:
  * ms[0] z  ms[1] v  ms[3] the WHOLE xy substep (geometry + apply, first launch to last)  ms[4] v  ms[5] z
  * ms[7] total -- all on the context's stream; ms[2] = duration of the geometry kernel alone on the library's
- * internal stream (it is part of ms[3], not in addition to it); ms[6] = 1 if that kernel ran concurrently
- * with the apply (o = 2), 0 if the apply waited for it.
+ * internal stream (it is part of ms[3], not in addition to it); ms[6] = flags: +1 if that kernel ran concurrently
+ * with the apply, +2 if each pair of adjacent sweeps (z,v before the 2d step; v,z after it) ran fused in one pass
+ * over f -- then ms[0] and ms[4] hold the time of a whole pair and ms[1] = ms[5] = 0.
  * After a single sldg_advect_* call only that entry (and ms[7]) is set.  Synchronises. */
 int sldg_last_timing_ms(sldg_ctx *ctx, float ms[8]);
 /* Number of kernels the library launched on behalf of this context since creation. */

@@ -268,6 +268,7 @@ int sldg_create(const sldg_params *p, double *f_a_dev, double *f_b_dev, void *wo
     c->zflag = (unsigned long long *)(ws + m.zflag);
     c->xy_epoch = 0;
     c->overlap = getenv("SLDG_XY_OVERLAP") ? 1 : 0;  // experimental: co-running the two kernels is slower today
+    c->fuse = getenv("SLDG_NO_FUSE") ? 0 : 1;
     c->trace_order = 2;
     c->vel_periodic = 0;
     if (cudaDeviceGetAttribute(&c->sm_count, cudaDevAttrMultiProcessorCount, dev) != cudaSuccess) {
@@ -390,6 +391,28 @@ static int do_v(sldg_ctx *c, double tau)
     return SLDG_OK;
 }
 
+// The two adjacent sweeps of a Strang step (Algorithm 1 steps 3,4 or 7,8) in one pass over f when the (z,v)
+// plane of an (x,y) node fits in shared memory; *fused = 0 and the two separate kernels otherwise.
+static int do_pair(sldg_ctx *c, double tau, bool z_first, cudaEvent_t mid, int *fused)
+{
+    *fused = 0;
+    if (c->fuse) {
+        cudaError_t e = launch_fused_sweeps(c, c->f[c->cur], c->f[c->cur ^ 1], tau, tau, z_first);
+        if (e == cudaSuccess) {
+            swap_state(c);
+            cudaEventRecord(mid, c->stream);
+            *fused = 1;
+            return SLDG_OK;
+        }
+        if (e != cudaErrorNotSupported) return SLDG_ECUDA;
+        cudaGetLastError();
+    }
+    int rc = z_first ? do_z(c, tau) : do_v(c, tau);
+    if (rc) return rc;
+    cudaEventRecord(mid, c->stream);
+    return z_first ? do_v(c, tau) : do_z(c, tau);
+}
+
 // The geometry (once per z node) and the apply (every v) of one 2d step.  The geometry runs on the
 // internal stream: it starts when everything enqueued before this call has finished (fields set, previous
 // apply done with the weights) and publishes one counter per z node; the apply, on the caller's stream, starts
@@ -458,17 +481,15 @@ int sldg_strang_step(sldg_ctx *c, double dt)
 {
     if (!c) return SLDG_EINVAL;
     int rc;
+    int fused0 = 0, fused1 = 0;
     cudaEventRecord(c->ev[0], c->stream);
-    if ((rc = do_z(c, 0.5 * dt))) return rc;
-    cudaEventRecord(c->ev[1], c->stream);
-    if ((rc = do_v(c, 0.5 * dt))) return rc;
+    if ((rc = do_pair(c, 0.5 * dt, true, c->ev[1], &fused0))) return rc;
     cudaEventRecord(c->ev[2], c->stream);
     if ((rc = do_xy(c, dt, c->trace_order))) return rc;
     cudaEventRecord(c->ev[3], c->stream);
-    if ((rc = do_v(c, 0.5 * dt))) return rc;
-    cudaEventRecord(c->ev[4], c->stream);
-    if ((rc = do_z(c, 0.5 * dt))) return rc;
+    if ((rc = do_pair(c, 0.5 * dt, false, c->ev[4], &fused1))) return rc;
     cudaEventRecord(c->ev[5], c->stream);
+    c->last_fused = fused0 && fused1;
     c->ev_kind = 1;
     return SLDG_OK;
 }
@@ -537,7 +558,7 @@ int sldg_last_timing_ms(sldg_ctx *c, float ms[8])
     if (c->ev_kind == 1) {
         ms[0] = el(0, 1); ms[1] = el(1, 2); ms[3] = el(2, 3); ms[4] = el(3, 4); ms[5] = el(4, 5);
         ms[2] = geom();
-        ms[6] = (c->overlap && xy_apply_can_overlap(c)) ? 1.0f : 0.0f;
+        ms[6] = ((c->overlap && xy_apply_can_overlap(c)) ? 1.0f : 0.0f) + (c->last_fused ? 2.0f : 0.0f);
         ms[7] = el(0, 5);
     } else if (c->ev_kind == 2) {
         ms[0] = ms[7] = el(0, 1);

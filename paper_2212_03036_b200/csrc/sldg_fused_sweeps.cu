@@ -1,0 +1,366 @@
+// sldg_fused_sweeps.cu -- the two adjacent 1d SLDG sweeps of a Strang step in ONE pass over f (sm_100a).
+//
+// Algorithm 1 runs z(dt/2) v(dt/2) before the 2d step and v(dt/2) z(dt/2) after it, with
+// nothing in between the two sweeps of a pair.  Each sweep alone reads and writes all of f (16 B per DOF); the
+// pair fused moves the same 16 B per DOF once.  Both sweeps act inside one (x,y) node's (z,v) plane (the z sweep
+// mixes z cells at fixed v, the v sweep v cells at fixed z), and that plane -- Nz lines of Pv doubles, 128 KiB at
+// 128 x 128 -- fits in shared memory.  The arithmetic of each sweep is that of sldg_sweeps.cu, operation by
+// operation, so the fused pair is bit-identical to the two separate kernels.
+//
+// One persistent block (512 threads) per SM walks over the (Y,X) planes:
+//   stage   the plane's lines are read from global memory into REGISTERS (coalesced 16-byte loads, R doubles per
+//           thread) -- issued one plane ahead, so that they are in flight under the compute phases below;
+//   tile    registers -> shared-memory tile [Nz][Pv];
+//   ZV      phase A  z sweep in place, thread <-> (v, slice of z): the result for target cell i is written over
+//                    its left source cell (i+s) mod nz, which is dead by then -- column v ends up rotated by s(v);
+//           phase B  v sweep line by line, warp <-> line, gathering through the per-column rotation, results
+//                    straight to global memory;
+//   VZ      phase A  v sweep in place, warp <-> line (all sources of a warp's line are in registers before the
+//                    first write);
+//           phase B  z sweep, thread <-> (v, slice of z), results straight to global memory.
+#include "sldg_sweep_common.cuh"
+
+namespace {
+
+constexpr int FUSED_THREADS = 512;
+constexpr int FUSED_MAXCPL = 4;  // v cells per lane in the line-wise phases (nv <= 128)
+
+// dynamic shared memory: tile [Nz][Pv] doubles | per line: A, B of its v shift [Nz][2 O^2] doubles |
+// per column: A, B of its z shift [2 O^2][Pv] doubles | per line: s [Nz] ints | per column: rotation offset
+// [Pv] ints, z shift [Pv] ints
+__host__ __device__ inline size_t fused_smem_bytes(int Nz, int Pv, int O)
+{
+    return (size_t)Nz * Pv * 8 + (size_t)Nz * 2 * O * O * 8 + (size_t)Pv * 2 * O * O * 8 + (size_t)Nz * 4 +
+           (size_t)Pv * 8;
+}
+
+template <int O, int R, int CPL, bool ZFIRST>
+__global__ void __launch_bounds__(FUSED_THREADS, 1) fused_sweep_kernel(const double *__restrict__ fin,
+                                                                       double *__restrict__ fout,
+                                                                       const double *__restrict__ Ez, GridDev g,
+                                                                       ShiftPoly spz, ShiftPoly spv, Basis bs,
+                                                                       double tau_z, double tau_v)
+{
+    extern __shared__ __align__(16) unsigned char fused_smem[];
+    const int Nz = g.N[2], nz = g.n[2], Nv = g.N[3], nv = g.n[3], Pv = g.Pv;
+    double *tile = reinterpret_cast<double *>(fused_smem);
+    double *vAB = tile + (size_t)Nz * Pv;                  // [Nz][2][O][O]: A then B of the line's v shift
+    double *zAB = vAB + (size_t)Nz * 2 * O * O;            // [2 O O][Pv]: A then B of the column's z shift
+    int *vs = reinterpret_cast<int *>(zAB + (size_t)Pv * 2 * O * O);  // [Nz]: the line's integer v shift, wrapped
+    int *rotoff = vs + Nz;                                 // [Pv]: s_z(v) * O * Pv, the column's rotation in doubles
+    int *zs = rotoff + Pv;                                 // [Pv]: s_z(v), wrapped
+    const int NzPv = Nz * Pv;
+    const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
+    const int ncol = g.N[1] * g.N[0];
+    const long long plane_nodes = (long long)g.N[1] * g.N[0];
+
+    // z sweep: thread <-> (v, slice qd of the target z cells); (s, A, B) depend on the v node only
+    const int nq = min(FUSED_THREADS / Pv, nz);  // slices of z
+    const int v = tid % Pv, qd = tid / Pv;
+    const bool zact = qd < nq && v < Nv;
+    if (tid < Pv) {
+        // (s, A, B) of the z shift depend on the v node only: once per block, into shared memory
+        const int ov = g.o[3];
+        const int vv = tid < Nv ? tid : 0;
+        const int l = vv / ov, q = vv - l * ov;
+        const double vq = __dadd_rn(g.lo[3], __dmul_rn(__dadd_rn((double)l, bs.xi[ov][q]), g.h[3]));
+        int s0;
+        double alpha, A0[O][O], B0[O][O];
+        shift_of(vq, tau_z, g.h[2], s0, alpha);
+        eval_shift<O>(spz, alpha, A0, B0);
+        s0 = wrapi(s0, nz);
+        zs[tid] = s0;
+        rotoff[tid] = tid < Nv ? s0 * O * Pv : 0;
+#pragma unroll
+        for (int j = 0; j < O; ++j)
+#pragma unroll
+            for (int m = 0; m < O; ++m) {
+                zAB[(j * O + m) * Pv + tid] = A0[j][m];
+                zAB[(O * O + j * O + m) * Pv + tid] = B0[j][m];
+            }
+    }
+    const int zi0 = (int)((long long)qd * nz / nq), zi1 = (int)((long long)(qd + 1) * nz / nq);
+
+    // staging: thread <-> (line l0 + r * LPI, 16-byte word w0 of the line), r = 0 .. R/2-1
+    const int hw = Pv / 2, LPI = FUSED_THREADS / hw;
+    const int l0 = tid / hw, w0 = 2 * (tid - l0 * hw);
+    const bool sact = l0 < LPI;
+    const long long gstep = (long long)LPI * g.sZ;
+    const int tstep = LPI * Pv;
+    double stage[R];
+    double ez_next = 0.0;
+    auto load_plane = [&](int col) {
+        const int X = col % g.N[0], Y = col / g.N[0];
+        const double *src = fin + Y * g.sY + X * g.sX + l0 * g.sZ + w0;
+#pragma unroll
+        for (int r = 0; r < R / 2; ++r) {
+            if (sact && l0 + r * LPI < Nz) {
+                const double2 t = __ldcs(reinterpret_cast<const double2 *>(src));
+                stage[2 * r] = t.x;
+                stage[2 * r + 1] = t.y;
+            }
+            src += gstep;
+        }
+        if (tid < Nz) ez_next = __ldg(Ez + tid * plane_nodes + col);
+    };
+
+    int col = blockIdx.x;
+    if (col < ncol) load_plane(col);
+    for (; col < ncol; col += gridDim.x) {
+        // ---- registers -> tile; per line the (s, A, B) of its v shift -------------------------------------
+        {
+            double *t = tile + l0 * Pv + w0;
+#pragma unroll
+            for (int r = 0; r < R / 2; ++r) {
+                if (sact && l0 + r * LPI < Nz) *reinterpret_cast<double2 *>(t) = make_double2(stage[2 * r], stage[2 * r + 1]);
+                t += tstep;
+            }
+        }
+        if (tid < Nz) {
+            int s;
+            double alpha, A[O][O], B[O][O];
+            shift_of(ez_next, tau_v, g.h[3], s, alpha);
+            eval_shift<O>(spv, alpha, A, B);
+            vs[tid] = wrapi(s, nv);
+#pragma unroll
+            for (int j = 0; j < O; ++j)
+#pragma unroll
+                for (int m = 0; m < O; ++m) {
+                    vAB[(tid * 2) * O * O + j * O + m] = A[j][m];
+                    vAB[(tid * 2 + 1) * O * O + j * O + m] = B[j][m];
+                }
+        }
+        __syncthreads();
+        const int X = col % g.N[0], Y = col / g.N[0];
+        double *dst = fout + Y * g.sY + X * g.sX;
+        if (col + (int)gridDim.x < ncol) load_plane(col + gridDim.x);  // in flight under the phases below
+
+        if (ZFIRST) {
+            // ---- phase A: z sweep in place; the result of target cell i lands on slot (i + s) mod nz ------
+            int c = 0;
+            double up[O], last[O], Az[O][O], Bz[O][O];
+            if (zact) {
+                const int sz = zs[v];
+#pragma unroll
+                for (int j = 0; j < O; ++j)
+#pragma unroll
+                    for (int m = 0; m < O; ++m) {
+                        Az[j][m] = zAB[(j * O + m) * Pv + v];
+                        Bz[j][m] = zAB[(O * O + j * O + m) * Pv + v];
+                    }
+                c = zi0 + sz;
+                if (c >= nz) c -= nz;
+                int cl = zi1 + sz;
+                if (cl >= nz) cl -= nz;
+#pragma unroll
+                for (int m = 0; m < O; ++m) {
+                    up[m] = tile[(size_t)(c * O + m) * Pv + v];
+                    last[m] = tile[(size_t)(cl * O + m) * Pv + v];  // first slot of the next slice: it is overwritten
+                }
+            }
+            __syncthreads();
+            if (zact) {
+#pragma unroll 2
+                for (int i = zi0; i < zi1; ++i) {
+                    const int cn = (c + 1 == nz) ? 0 : c + 1;
+                    double un[O];
+#pragma unroll
+                    for (int m = 0; m < O; ++m) un[m] = (i + 1 == zi1) ? last[m] : tile[(size_t)(cn * O + m) * Pv + v];
+#pragma unroll
+                    for (int j = 0; j < O; ++j) {
+                        double acc = 0.0;
+#pragma unroll
+                        for (int m = 0; m < O; ++m) acc = fma(Az[j][m], up[m], acc);
+#pragma unroll
+                        for (int m = 0; m < O; ++m) acc = fma(Bz[j][m], un[m], acc);
+                        tile[(size_t)(c * O + j) * Pv + v] = acc;
+                    }
+#pragma unroll
+                    for (int m = 0; m < O; ++m) up[m] = un[m];
+                    c = cn;
+                }
+            }
+            __syncthreads();
+            // ---- phase B: v sweep of every line, gathering through the rotation, to global memory ---------
+#pragma unroll 1
+            for (int zr = warp; zr < Nz; zr += FUSED_THREADS / 32) {
+                const int s = vs[zr];
+                double A[O][O], B[O][O];
+#pragma unroll
+                for (int j = 0; j < O; ++j)
+#pragma unroll
+                    for (int m = 0; m < O; ++m) {
+                        A[j][m] = vAB[(zr * 2) * O * O + j * O + m];
+                        B[j][m] = vAB[(zr * 2 + 1) * O * O + j * O + m];
+                    }
+                double *w = dst + zr * g.sZ;
+                const int zoff = zr * Pv;
+                auto at = [&](int vcol) {  // value of line zr at column vcol: the column is rotated by whole cells
+                    int t = rotoff[vcol] + zoff;
+                    if (t >= NzPv) t -= NzPv;
+                    return tile[t + vcol];
+                };
+                for (int cell = lane; cell < nv; cell += 32) {
+                    int c0 = cell + s;
+                    if (c0 >= nv) c0 -= nv;
+                    int c1 = c0 + 1;
+                    if (c1 >= nv) c1 -= nv;
+                    double u0[O], u1[O], r[O];
+#pragma unroll
+                    for (int m = 0; m < O; ++m) {
+                        u0[m] = at(c0 * O + m);
+                        u1[m] = at(c1 * O + m);
+                    }
+#pragma unroll
+                    for (int j = 0; j < O; ++j) {
+                        double acc = 0.0;
+#pragma unroll
+                        for (int m = 0; m < O; ++m) acc = fma(A[j][m], u0[m], acc);
+#pragma unroll
+                        for (int m = 0; m < O; ++m) acc = fma(B[j][m], u1[m], acc);
+                        r[j] = acc;
+                    }
+                    if (O == 2) {
+                        __stcs(reinterpret_cast<double2 *>(w + 2 * cell), make_double2(r[0], r[O - 1]));
+                    } else {
+#pragma unroll
+                        for (int j = 0; j < O; ++j) __stcs(w + cell * O + j, r[j]);
+                    }
+                }
+            }
+        } else {
+            // ---- phase A: v sweep in place, warp <-> line ---------------------------------------------------
+#pragma unroll 1
+            for (int zr = warp; zr < Nz; zr += FUSED_THREADS / 32) {
+                const int s = vs[zr];
+                double A[O][O], B[O][O];
+#pragma unroll
+                for (int j = 0; j < O; ++j)
+#pragma unroll
+                    for (int m = 0; m < O; ++m) {
+                        A[j][m] = vAB[(zr * 2) * O * O + j * O + m];
+                        B[j][m] = vAB[(zr * 2 + 1) * O * O + j * O + m];
+                    }
+                double *u = tile + (size_t)zr * Pv;
+                double u0[CPL][O], u1[CPL][O];
+#pragma unroll
+                for (int k = 0; k < CPL; ++k) {
+                    const int cell = lane + 32 * k;
+                    if (cell < nv) {
+                        int c0 = cell + s;
+                        if (c0 >= nv) c0 -= nv;
+                        int c1 = c0 + 1;
+                        if (c1 >= nv) c1 -= nv;
+                        if (O == 2) {
+                            const double2 t0 = *reinterpret_cast<const double2 *>(u + 2 * c0);
+                            const double2 t1 = *reinterpret_cast<const double2 *>(u + 2 * c1);
+                            u0[k][0] = t0.x; u0[k][O - 1] = t0.y;
+                            u1[k][0] = t1.x; u1[k][O - 1] = t1.y;
+                        } else {
+#pragma unroll
+                            for (int m = 0; m < O; ++m) {
+                                u0[k][m] = u[c0 * O + m];
+                                u1[k][m] = u[c1 * O + m];
+                            }
+                        }
+                    }
+                }
+                __syncwarp();  // every source of this line is in registers: the line may be overwritten
+#pragma unroll
+                for (int k = 0; k < CPL; ++k) {
+                    const int cell = lane + 32 * k;
+                    if (cell < nv) {
+                        double r[O];
+#pragma unroll
+                        for (int j = 0; j < O; ++j) {
+                            double acc = 0.0;
+#pragma unroll
+                            for (int m = 0; m < O; ++m) acc = fma(A[j][m], u0[k][m], acc);
+#pragma unroll
+                            for (int m = 0; m < O; ++m) acc = fma(B[j][m], u1[k][m], acc);
+                            r[j] = acc;
+                        }
+                        if (O == 2) {
+                            *reinterpret_cast<double2 *>(u + 2 * cell) = make_double2(r[0], r[O - 1]);
+                        } else {
+#pragma unroll
+                            for (int j = 0; j < O; ++j) u[cell * O + j] = r[j];
+                        }
+                    }
+                }
+            }
+            __syncthreads();
+            // ---- phase B: z sweep, thread <-> (v, slice of z), to global memory -------------------------------
+            if (zact) {
+                double Az[O][O], Bz[O][O];
+#pragma unroll
+                for (int j = 0; j < O; ++j)
+#pragma unroll
+                    for (int m = 0; m < O; ++m) {
+                        Az[j][m] = zAB[(j * O + m) * Pv + v];
+                        Bz[j][m] = zAB[(O * O + j * O + m) * Pv + v];
+                    }
+                int c = zi0 + zs[v];
+                if (c >= nz) c -= nz;
+                double up[O];
+#pragma unroll
+                for (int m = 0; m < O; ++m) up[m] = tile[(size_t)(c * O + m) * Pv + v];
+                double *w = dst + v;
+#pragma unroll 2
+                for (int i = zi0; i < zi1; ++i) {
+                    c = (c + 1 == nz) ? 0 : c + 1;
+                    double un[O];
+#pragma unroll
+                    for (int m = 0; m < O; ++m) un[m] = tile[(size_t)(c * O + m) * Pv + v];
+#pragma unroll
+                    for (int j = 0; j < O; ++j) {
+                        double acc = 0.0;
+#pragma unroll
+                        for (int m = 0; m < O; ++m) acc = fma(Az[j][m], up[m], acc);
+#pragma unroll
+                        for (int m = 0; m < O; ++m) acc = fma(Bz[j][m], un[m], acc);
+                        __stcs(w + (long long)(i * O + j) * g.sZ, acc);
+                    }
+#pragma unroll
+                    for (int m = 0; m < O; ++m) up[m] = un[m];
+                }
+            }
+        }
+        __syncthreads();  // the tile is free for the next plane
+    }
+}
+
+}  // namespace
+
+// The pair (z then v, or v then z) in one pass; returns cudaErrorNotSupported when the (z,v) plane does not fit
+// (the caller then runs the two separate kernels).
+cudaError_t launch_fused_sweeps(sldg_ctx *c, const double *fin, double *fout, double tau_z, double tau_v, bool z_first)
+{
+    const GridDev &g = c->g;
+    const int O = g.o[2];
+    if (g.o[3] != O) return cudaErrorNotSupported;
+    if (g.Pv > FUSED_THREADS || g.n[3] > 32 * FUSED_MAXCPL) return cudaErrorNotSupported;
+    const size_t smem = fused_smem_bytes(g.N[2], g.Pv, O);
+    if (smem > 220 * 1024) return cudaErrorNotSupported;
+    const int lpi = FUSED_THREADS / (g.Pv / 2);              // lines staged per pass of the block
+    const int need = 2 * ((g.N[2] + lpi - 1) / lpi);         // staged doubles per thread
+    const bool cpl2 = g.n[3] <= 64;
+    const int ncol = g.N[0] * g.N[1];
+    const int grid = ncol < c->sm_count ? ncol : c->sm_count;
+#define LAUNCH_F(OO, RR)                                                                                          \
+    do {                                                                                                          \
+        auto kern = z_first ? (cpl2 ? fused_sweep_kernel<OO, RR, 2, true> : fused_sweep_kernel<OO, RR, 4, true>)  \
+                            : (cpl2 ? fused_sweep_kernel<OO, RR, 2, false> : fused_sweep_kernel<OO, RR, 4, false>); \
+        cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);                       \
+        kern<<<grid, FUSED_THREADS, smem, c->stream>>>(fin, fout, c->Ez, g, c->sp_z, c->sp_v, c->basis, tau_z,    \
+                                                       tau_v);                                                    \
+    } while (0)
+    if (O == 2 && need <= 16) LAUNCH_F(2, 16);
+    else if (O == 2 && need <= 32) LAUNCH_F(2, 32);
+    else if (O == 3 && need <= 16) LAUNCH_F(3, 16);
+    else if (O == 3 && need <= 44) LAUNCH_F(3, 44);
+    else return cudaErrorNotSupported;
+#undef LAUNCH_F
+    c->launches++;
+    return cudaGetLastError();
+}

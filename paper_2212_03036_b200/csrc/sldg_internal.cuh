@@ -60,6 +60,7 @@ struct sldg_ctx {
     unsigned long long xy_epoch;
     cudaStream_t gstream;   // internal high-priority stream: the geometry kernel runs here, under the apply
     cudaEvent_t gev[4];     // xy start (main), geometry start/end (gstream), previous apply done (main)
+    int fuse, last_fused;   // fuse: sldg_strang_step runs each pair of adjacent sweeps in one pass
     int overlap;            // 1: geometry and apply of one xy step run concurrently (o = 2 path)
     size_t n_partials;
     int trace_order, vel_periodic;
@@ -82,3 +83,4 @@ int xy_geometry_blocks_per_z(const sldg_ctx *c);
 bool xy_apply_can_overlap(const sldg_ctx *c);
 cudaError_t launch_geometry_expand(sldg_ctx *c, int z, int32_t *anchor, int32_t *mask, double *Wd);
 cudaError_t launch_xy_apply(sldg_ctx *c, const double *fin, double *fout, bool wait_flags);
+cudaError_t launch_fused_sweeps(sldg_ctx *c, const double *fin, double *fout, double tau_z, double tau_v, bool z_first);

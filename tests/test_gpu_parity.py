@@ -331,8 +331,51 @@ def test_config0_tiny_itg_20_strang_steps(torch):
     rho = s.charge_density().cpu().numpy()
     assert _rel(rho, oracle.charge_density(spec, ref)) <= TOL
     ms = s.last_timing_ms()
-    assert all(t > 0 for t in ms[:6]) and ms[7] >= max(ms[:6])
-    assert s.launch_count() >= 20 * 6
+    fused = int(ms[6]) & 2
+    timed = [ms[0], ms[2], ms[3], ms[4]] if fused else ms[:6]
+    assert all(t > 0 for t in timed) and ms[7] >= max(ms[:6])
+    assert s.launch_count() >= 20 * (4 if fused else 6)
+
+
+@pytest.mark.gpu
+@pytest.mark.parametrize("o,cells", [(2, (6, 5, 8, 16)), (2, (4, 4, 16, 64)), (3, (4, 3, 6, 16)), (2, (3, 3, 5, 7))])
+@pytest.mark.parametrize("cfl", [0.4, 7.3])
+def test_fused_sweep_pairs_are_bit_identical_to_separate_sweeps(torch, monkeypatch, o, cells, cfl):
+    """sldg_strang_step runs z,v and v,z as one kernel each where the (z,v) plane fits in shared memory: the
+    state must equal, bit for bit, the one produced by the five separate substep calls, for small and large
+    Courant numbers (wrap-around of the rotated columns) and ragged sizes."""
+    spec = inputs.itg_grid(*cells, o)
+    rng = np.random.default_rng(7)
+    f = rng.random(spec.shape)
+    dt = 2.0
+    a, b, Ez, _ = inputs.itg_fields(spec, dt, 0.6)
+    Ez = Ez * (cfl * spec.h[3] / (0.5 * dt) / max(np.abs(Ez).max(), 1e-300))
+    dtz = dt  # z Courant numbers come from the v nodes themselves (up to |v| dt/2 / h_z)
+    outs = []
+    for fuse in (True, False):
+        if fuse:
+            monkeypatch.delenv("SLDG_NO_FUSE", raising=False)
+        else:
+            monkeypatch.setenv("SLDG_NO_FUSE", "1")
+        s = _sldg(spec)
+        s.import_state(_dev(torch, f))
+        s.set_Ez(_dev(torch, Ez))
+        s.set_vxy(_dev(torch, a), _dev(torch, b), 1)
+        if fuse:
+            for _ in range(2):
+                s.strang_step(dtz)
+            assert int(s.last_timing_ms()[6]) & 2, "the fused path did not run"
+        else:
+            for _ in range(2):
+                s.advect_z(0.5 * dtz)
+                s.advect_v(0.5 * dtz)
+                s.advect_xy(dtz, 2)
+                s.advect_v(0.5 * dtz)
+                s.advect_z(0.5 * dtz)
+        s.check()
+        outs.append(s.export_state().cpu().numpy())
+        s.close()
+    assert np.array_equal(outs[0], outs[1])
 
 
 def test_layouts_agree_bitwise_on_a_strang_step(torch):
