@@ -8,9 +8,12 @@
 // operation, so the fused pair is bit-identical to the two separate kernels.
 //
 // One persistent block (512 threads) per SM walks over the (Y,X) planes:
-//   stage   the plane's lines are read from global memory into REGISTERS (coalesced 16-byte loads, R doubles per
-//           thread) -- issued one plane ahead, so that they are in flight under the compute phases below;
-//   tile    registers -> shared-memory tile [Nz][Pv];
+//   stage   the NEXT plane's lines are fetched under the compute phases of the current one: NL of its Nz lines by
+//           cp.async into the spare shared memory, the other NH = Nz - NL into REGISTERS (coalesced 16-byte
+//           loads, R doubles per thread).  Shared memory holds [L_a: NL lines | H: NH lines | L_b: NL lines];
+//           even planes live in [L_a | H] (lines 0..NL-1 asynchronous), odd planes in [H | L_b] (lines NH..Nz-1
+//           asynchronous), so a plane is always one contiguous tile [Nz][Pv] and the other L is free;
+//   tile    registers -> the H lines of the tile;
 //   ZV      phase A  z sweep in place, thread <-> (v, slice of z): the result for target cell i is written over
 //                    its left source cell (i+s) mod nz, which is dead by then -- column v ends up rotated by s(v);
 //           phase B  v sweep line by line, warp <-> line, gathering through the per-column rotation, results
@@ -22,29 +25,64 @@
 
 namespace {
 
-constexpr int FUSED_THREADS = 512;
-constexpr int FUSED_MAXCPL = 4;  // v cells per lane in the line-wise phases (nv <= 128)
-
-// dynamic shared memory: tile [Nz][Pv] doubles | per line: A, B of its v shift [Nz][2 O^2] doubles |
-// per column: A, B of its z shift [2 O^2][Pv] doubles | per line: s [Nz] ints | per column: rotation offset
-// [Pv] ints, z shift [Pv] ints
-__host__ __device__ inline size_t fused_smem_bytes(int Nz, int Pv, int O)
+// ---- mbarrier / bulk-copy primitives (PTX) --------------------------------------------------------
+__device__ __forceinline__ uint32_t smem_u32(const void *p) { return (uint32_t)__cvta_generic_to_shared(p); }
+__device__ __forceinline__ void mbar_init(uint64_t *bar, uint32_t count)
 {
-    return (size_t)Nz * Pv * 8 + (size_t)Nz * 2 * O * O * 8 + (size_t)Pv * 2 * O * O * 8 + (size_t)Nz * 4 +
-           (size_t)Pv * 8;
+    asm volatile("mbarrier.init.shared::cta.b64 [%0], %1;" ::"r"(smem_u32(bar)), "r"(count) : "memory");
+}
+__device__ __forceinline__ void mbar_fence_init() { asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory"); }
+__device__ __forceinline__ void mbar_arrive(uint64_t *bar)
+{
+    asm volatile("mbarrier.arrive.shared::cta.b64 _, [%0];" ::"r"(smem_u32(bar)) : "memory");
+}
+__device__ __forceinline__ void mbar_arrive_expect_tx(uint64_t *bar, uint32_t bytes)
+{
+    asm volatile("mbarrier.arrive.expect_tx.shared::cta.b64 _, [%0], %1;" ::"r"(smem_u32(bar)), "r"(bytes) : "memory");
+}
+__device__ __forceinline__ void bulk_g2s(void *dst, const void *src, uint32_t bytes, uint64_t *bar)
+{
+    asm volatile("cp.async.bulk.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1], %2, [%3];" ::"r"(
+                     smem_u32(dst)),
+                 "l"(src), "r"(bytes), "r"(smem_u32(bar))
+                 : "memory");
+}
+__device__ __forceinline__ void mbar_wait(uint64_t *bar, uint32_t parity)
+{
+    uint32_t ok;
+    do {
+        asm volatile(
+            "{\n.reg .pred p;\nmbarrier.try_wait.parity.shared::cta.b64 p, [%1], %2;\nselp.u32 %0, 1, 0, p;\n}"
+            : "=r"(ok)
+            : "r"(smem_u32(bar)), "r"(parity)
+            : "memory");
+    } while (!ok);
 }
 
-template <int O, int R, int CPL, bool ZFIRST>
-__global__ void __launch_bounds__(FUSED_THREADS, 1) fused_sweep_kernel(const double *__restrict__ fin,
+constexpr int FUSED_THREADS = 512;          // compute threads (16 warps)
+constexpr int FUSED_BLOCK = FUSED_THREADS + 32;  // + one producer warp
+constexpr int FUSED_MAXCPL = 4;  // v cells per lane in the line-wise phases (nv <= 128)
+
+// dynamic shared memory: planes [2 NL + NH][Pv] doubles | per line: A, B of its v shift [Nz][2 O^2] doubles |
+// per column: A, B of its z shift [2 O^2][Pv] doubles | per line: s [Nz] ints | per column: rotation offset
+// [Pv] ints, z shift [Pv] ints
+__host__ __device__ inline size_t fused_table_bytes(int Nz, int Pv, int O)
+{
+    return (size_t)Nz * 2 * O * O * 8 + (size_t)Pv * 2 * O * O * 8 + (size_t)Nz * 4 + (size_t)Pv * 8 + 64;
+}
+
+template <int O, int CPL, bool ZFIRST>
+__global__ void __launch_bounds__(FUSED_BLOCK, 1) fused_sweep_kernel(const double *__restrict__ fin,
                                                                        double *__restrict__ fout,
                                                                        const double *__restrict__ Ez, GridDev g,
                                                                        ShiftPoly spz, ShiftPoly spv, Basis bs,
-                                                                       double tau_z, double tau_v)
+                                                                       double tau_z, double tau_v, int NL)
 {
     extern __shared__ __align__(16) unsigned char fused_smem[];
     const int Nz = g.N[2], nz = g.n[2], Nv = g.N[3], nv = g.n[3], Pv = g.Pv;
-    double *tile = reinterpret_cast<double *>(fused_smem);
-    double *vAB = tile + (size_t)Nz * Pv;                  // [Nz][2][O][O]: A then B of the line's v shift
+    const int NH = Nz - NL;
+    double *buf = reinterpret_cast<double *>(fused_smem);  // [L_a | H | L_b]
+    double *vAB = buf + (size_t)(2 * NL + NH) * Pv;        // [Nz][2][O][O]: A then B of the line's v shift
     double *zAB = vAB + (size_t)Nz * 2 * O * O;            // [2 O O][Pv]: A then B of the column's z shift
     int *vs = reinterpret_cast<int *>(zAB + (size_t)Pv * 2 * O * O);  // [Nz]: the line's integer v shift, wrapped
     int *rotoff = vs + Nz;                                 // [Pv]: s_z(v) * O * Pv, the column's rotation in doubles
@@ -81,45 +119,59 @@ __global__ void __launch_bounds__(FUSED_THREADS, 1) fused_sweep_kernel(const dou
     }
     const int zi0 = (int)((long long)qd * nz / nq), zi1 = (int)((long long)(qd + 1) * nz / nq);
 
-    // staging: thread <-> (line l0 + r * LPI, 16-byte word w0 of the line), r = 0 .. R/2-1
-    const int hw = Pv / 2, LPI = FUSED_THREADS / hw;
-    const int l0 = tid / hw, w0 = 2 * (tid - l0 * hw);
-    const bool sact = l0 < LPI;
-    const long long gstep = (long long)LPI * g.sZ;
-    const int tstep = LPI * Pv;
-    double stage[R];
-    double ez_next = 0.0;
-    auto load_plane = [&](int col) {
+    // staging by bulk copies (TMA), issued by the producer warp, completing on mbarriers: line l of a plane ->
+    // tile + l * Pv.  bars: full_L[2], full_H, done (all compute warps are through with a plane)
+    uint64_t *bars = reinterpret_cast<uint64_t *>(zs + Pv + (Pv & 1));  // 8-byte aligned
+    if (tid == 0) {
+        for (int k = 0; k < 3; ++k) mbar_init(&bars[k], 1);
+        mbar_init(&bars[3], FUSED_THREADS / 32);
+        mbar_fence_init();
+    }
+    __syncthreads();
+    auto compute_sync = [&]() { asm volatile("bar.sync 1, %0;" ::"n"(FUSED_THREADS) : "memory"); };
+    const uint32_t line_bytes = (uint32_t)Pv * 8;
+    auto issue_lines = [&](int col, double *tl, int first, int count, uint64_t *bar) {  // producer warp only
+        if (count <= 0) return;
         const int X = col % g.N[0], Y = col / g.N[0];
-        const double *src = fin + Y * g.sY + X * g.sX + l0 * g.sZ + w0;
-#pragma unroll
-        for (int r = 0; r < R / 2; ++r) {
-            if (sact && l0 + r * LPI < Nz) {
-                const double2 t = __ldcs(reinterpret_cast<const double2 *>(src));
-                stage[2 * r] = t.x;
-                stage[2 * r + 1] = t.y;
-            }
-            src += gstep;
-        }
-        if (tid < Nz) ez_next = __ldg(Ez + tid * plane_nodes + col);
+        const double *src = fin + Y * g.sY + X * g.sX;
+        if (lane == 0) mbar_arrive_expect_tx(bar, (uint32_t)count * line_bytes);
+        __syncwarp();
+        for (int l = first + lane; l < first + count; l += 32) bulk_g2s(tl + l * Pv, src + l * g.sZ, line_bytes, bar);
     };
-
-    int col = blockIdx.x;
-    if (col < ncol) load_plane(col);
-    for (; col < ncol; col += gridDim.x) {
-        // ---- registers -> tile; per line the (s, A, B) of its v shift -------------------------------------
-        {
-            double *t = tile + l0 * Pv + w0;
-#pragma unroll
-            for (int r = 0; r < R / 2; ++r) {
-                if (sact && l0 + r * LPI < Nz) *reinterpret_cast<double2 *>(t) = make_double2(stage[2 * r], stage[2 * r + 1]);
-                t += tstep;
+    if (warp == FUSED_THREADS / 32) {
+        // ---------------- producer warp ------------------------------------------------------------------------
+        uint32_t phD = 0;
+        int col = blockIdx.x, par = 0;
+        if (col < ncol) issue_lines(col, buf, 0, NL, &bars[0]);  // L lines of the first (even) plane
+        for (bool first = true; col < ncol; col += gridDim.x, par ^= 1, first = false) {
+            if (!first) {
+                mbar_wait(&bars[3], phD);  // the previous plane is done: H and the other L are free
+                phD ^= 1;
             }
+            double *tile = buf + (par ? NL * Pv : 0);
+            const int ncolx = col + (int)gridDim.x;
+            // H lines of this plane: [NL,Nz) of an even plane, [0,NH) of an odd one
+            issue_lines(col, tile, par ? 0 : NL, NH, &bars[2]);
+            // L lines of the next plane into the other L: [0,NL) of an even plane, [NH,Nz) of an odd one
+            if (ncolx < ncol) issue_lines(ncolx, buf + (par ? 0 : NL * Pv), par ? 0 : NH, NL, &bars[par ^ 1]);
         }
+        return;
+    }
+
+    double ez_next = 0.0;
+    int col = blockIdx.x, par = 0;
+    uint32_t phL[2] = {0, 0}, phH = 0;
+    if (col < ncol && tid < Nz) ez_next = __ldg(Ez + tid * plane_nodes + col);
+    for (; col < ncol; col += gridDim.x, par ^= 1) {
+        double *tile = buf + (par ? NL * Pv : 0);
+        const int ncolx = col + (int)gridDim.x;
+        const double ez_cur = ez_next;
+        if (ncolx < ncol && tid < Nz) ez_next = __ldg(Ez + tid * plane_nodes + ncolx);
+        // ---- per line the (s, A, B) of its v shift (under the copies) ------------------------------------------
         if (tid < Nz) {
             int s;
             double alpha, A[O][O], B[O][O];
-            shift_of(ez_next, tau_v, g.h[3], s, alpha);
+            shift_of(ez_cur, tau_v, g.h[3], s, alpha);
             eval_shift<O>(spv, alpha, A, B);
             vs[tid] = wrapi(s, nv);
 #pragma unroll
@@ -130,10 +182,17 @@ __global__ void __launch_bounds__(FUSED_THREADS, 1) fused_sweep_kernel(const dou
                     vAB[(tid * 2 + 1) * O * O + j * O + m] = B[j][m];
                 }
         }
-        __syncthreads();
+        if (NL > 0) {
+            mbar_wait(&bars[par], phL[par]);
+            phL[par] ^= 1;
+        }
+        if (NH > 0) {
+            mbar_wait(&bars[2], phH);
+            phH ^= 1;
+        }
+        compute_sync();
         const int X = col % g.N[0], Y = col / g.N[0];
         double *dst = fout + Y * g.sY + X * g.sX;
-        if (col + (int)gridDim.x < ncol) load_plane(col + gridDim.x);  // in flight under the phases below
 
         if (ZFIRST) {
             // ---- phase A: z sweep in place; the result of target cell i lands on slot (i + s) mod nz ------
@@ -158,7 +217,7 @@ __global__ void __launch_bounds__(FUSED_THREADS, 1) fused_sweep_kernel(const dou
                     last[m] = tile[(size_t)(cl * O + m) * Pv + v];  // first slot of the next slice: it is overwritten
                 }
             }
-            __syncthreads();
+            compute_sync();
             if (zact) {
 #pragma unroll 2
                 for (int i = zi0; i < zi1; ++i) {
@@ -180,7 +239,7 @@ __global__ void __launch_bounds__(FUSED_THREADS, 1) fused_sweep_kernel(const dou
                     c = cn;
                 }
             }
-            __syncthreads();
+            compute_sync();
             // ---- phase B: v sweep of every line, gathering through the rotation, to global memory ---------
 #pragma unroll 1
             for (int zr = warp; zr < Nz; zr += FUSED_THREADS / 32) {
@@ -289,7 +348,7 @@ __global__ void __launch_bounds__(FUSED_THREADS, 1) fused_sweep_kernel(const dou
                     }
                 }
             }
-            __syncthreads();
+            compute_sync();
             // ---- phase B: z sweep, thread <-> (v, slice of z), to global memory -------------------------------
             if (zact) {
                 double Az[O][O], Bz[O][O];
@@ -326,7 +385,10 @@ __global__ void __launch_bounds__(FUSED_THREADS, 1) fused_sweep_kernel(const dou
                 }
             }
         }
-        __syncthreads();  // the tile is free for the next plane
+        asm volatile("fence.proxy.async.shared::cta;" ::: "memory");  // generic writes before the next bulk copies
+        __syncwarp();
+        if (lane == 0) mbar_arrive(&bars[3]);
+        compute_sync();  // the per-line tables are free for the next plane
     }
 }
 
@@ -340,26 +402,25 @@ cudaError_t launch_fused_sweeps(sldg_ctx *c, const double *fin, double *fout, do
     const int O = g.o[2];
     if (g.o[3] != O) return cudaErrorNotSupported;
     if (g.Pv > FUSED_THREADS || g.n[3] > 32 * FUSED_MAXCPL) return cudaErrorNotSupported;
-    const size_t smem = fused_smem_bytes(g.N[2], g.Pv, O);
-    if (smem > 220 * 1024) return cudaErrorNotSupported;
-    const int lpi = FUSED_THREADS / (g.Pv / 2);              // lines staged per pass of the block
-    const int need = 2 * ((g.N[2] + lpi - 1) / lpi);         // staged doubles per thread
+    const int Nz = g.N[2];
+    const size_t tables = fused_table_bytes(Nz, g.Pv, O), row = (size_t)g.Pv * 8;
+    const size_t budget = 227 * 1024 - 1024;
+    if (tables + row * Nz > budget) return cudaErrorNotSupported;
+    long long NLl = (long long)((budget - tables) / row) - Nz;  // spare lines = lines fetched one plane ahead
+    const int NL = (int)(NLl > Nz ? Nz : (NLl < 0 ? 0 : NLl));
+    const size_t smem = tables + row * (size_t)(2 * NL + (Nz - NL));
     const bool cpl2 = g.n[3] <= 64;
     const int ncol = g.N[0] * g.N[1];
     const int grid = ncol < c->sm_count ? ncol : c->sm_count;
-#define LAUNCH_F(OO, RR)                                                                                          \
+#define LAUNCH_F(OO)                                                                                              \
     do {                                                                                                          \
-        auto kern = z_first ? (cpl2 ? fused_sweep_kernel<OO, RR, 2, true> : fused_sweep_kernel<OO, RR, 4, true>)  \
-                            : (cpl2 ? fused_sweep_kernel<OO, RR, 2, false> : fused_sweep_kernel<OO, RR, 4, false>); \
+        auto kern = z_first ? (cpl2 ? fused_sweep_kernel<OO, 2, true> : fused_sweep_kernel<OO, 4, true>)  \
+                            : (cpl2 ? fused_sweep_kernel<OO, 2, false> : fused_sweep_kernel<OO, 4, false>); \
         cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);                       \
-        kern<<<grid, FUSED_THREADS, smem, c->stream>>>(fin, fout, c->Ez, g, c->sp_z, c->sp_v, c->basis, tau_z,    \
-                                                       tau_v);                                                    \
+        kern<<<grid, FUSED_BLOCK, smem, c->stream>>>(fin, fout, c->Ez, g, c->sp_z, c->sp_v, c->basis, tau_z,    \
+                                                       tau_v, NL);                                                \
     } while (0)
-    if (O == 2 && need <= 16) LAUNCH_F(2, 16);
-    else if (O == 2 && need <= 32) LAUNCH_F(2, 32);
-    else if (O == 3 && need <= 16) LAUNCH_F(3, 16);
-    else if (O == 3 && need <= 44) LAUNCH_F(3, 44);
-    else return cudaErrorNotSupported;
+    if (O == 1) LAUNCH_F(1); else if (O == 2) LAUNCH_F(2); else LAUNCH_F(3);
 #undef LAUNCH_F
     c->launches++;
     return cudaGetLastError();
