@@ -186,7 +186,7 @@ __global__ void __launch_bounds__(FUSED_BLOCK, 1) fused_sweep_kernel(const doubl
             mbar_wait(&bars[par], phL[par]);
             phL[par] ^= 1;
         }
-        if (NH > 0) {
+        if (ZFIRST && NH > 0) {  // the z sweep needs every line; the v sweep (VZ) starts on the L lines
             mbar_wait(&bars[2], phH);
             phH ^= 1;
         }
@@ -219,12 +219,10 @@ __global__ void __launch_bounds__(FUSED_BLOCK, 1) fused_sweep_kernel(const doubl
             }
             compute_sync();
             if (zact) {
-#pragma unroll 2
-                for (int i = zi0; i < zi1; ++i) {
-                    const int cn = (c + 1 == nz) ? 0 : c + 1;
-                    double un[O];
-#pragma unroll
-                    for (int m = 0; m < O; ++m) un[m] = (i + 1 == zi1) ? last[m] : tile[(size_t)(cn * O + m) * Pv + v];
+                // running offset of cell c's first row in column v; it wraps at the end of the plane
+                const int cstep = O * Pv;
+                int off = c * cstep + v;
+                auto step = [&](const double (&un)[O]) {
 #pragma unroll
                     for (int j = 0; j < O; ++j) {
                         double acc = 0.0;
@@ -232,12 +230,22 @@ __global__ void __launch_bounds__(FUSED_BLOCK, 1) fused_sweep_kernel(const doubl
                         for (int m = 0; m < O; ++m) acc = fma(Az[j][m], up[m], acc);
 #pragma unroll
                         for (int m = 0; m < O; ++m) acc = fma(Bz[j][m], un[m], acc);
-                        tile[(size_t)(c * O + j) * Pv + v] = acc;
+                        tile[off + j * Pv] = acc;
                     }
 #pragma unroll
                     for (int m = 0; m < O; ++m) up[m] = un[m];
-                    c = cn;
+                };
+#pragma unroll 2
+                for (int i = zi0; i + 1 < zi1; ++i) {
+                    int offn = off + cstep;
+                    if (offn >= NzPv) offn -= NzPv;
+                    double un[O];
+#pragma unroll
+                    for (int m = 0; m < O; ++m) un[m] = tile[offn + m * Pv];
+                    step(un);
+                    off = offn;
                 }
+                step(last);  // the last target of the slice: its right source cell was read before the sweep
             }
             compute_sync();
             // ---- phase B: v sweep of every line, gathering through the rotation, to global memory ---------
@@ -259,17 +267,35 @@ __global__ void __launch_bounds__(FUSED_BLOCK, 1) fused_sweep_kernel(const doubl
                     if (t >= NzPv) t -= NzPv;
                     return tile[t + vcol];
                 };
-                for (int cell = lane; cell < nv; cell += 32) {
+                auto load_cell = [&](int cc, double (&u)[O]) {
+                    if (O == 2) {
+                        const int2 ro = *reinterpret_cast<const int2 *>(rotoff + 2 * cc);
+                        int t0 = ro.x + zoff, t1 = ro.y + zoff;
+                        if (t0 >= NzPv) t0 -= NzPv;
+                        if (t1 >= NzPv) t1 -= NzPv;
+                        u[0] = tile[t0 + 2 * cc];
+                        u[O - 1] = tile[t1 + 2 * cc + 1];
+                    } else {
+#pragma unroll
+                        for (int m = 0; m < O; ++m) u[m] = at(cc * O + m);
+                    }
+                };
+                for (int cell0 = 0; cell0 < nv; cell0 += 32) {
+                    const int cell = cell0 + lane;
+                    const bool valid = cell < nv;
                     int c0 = cell + s;
                     if (c0 >= nv) c0 -= nv;
                     int c1 = c0 + 1;
                     if (c1 >= nv) c1 -= nv;
                     double u0[O], u1[O], r[O];
 #pragma unroll
-                    for (int m = 0; m < O; ++m) {
-                        u0[m] = at(c0 * O + m);
-                        u1[m] = at(c1 * O + m);
-                    }
+                    for (int m = 0; m < O; ++m) u0[m] = 0.0;
+                    if (valid) load_cell(c0, u0);
+                    // the right source cell of this lane's target is the left source cell of the next lane's
+#pragma unroll
+                    for (int m = 0; m < O; ++m) u1[m] = __shfl_down_sync(0xffffffffu, u0[m], 1);
+                    if (valid && (lane == 31 || cell + 1 >= nv)) load_cell(c1, u1);
+                    if (!valid) continue;
 #pragma unroll
                     for (int j = 0; j < O; ++j) {
                         double acc = 0.0;
@@ -288,9 +314,19 @@ __global__ void __launch_bounds__(FUSED_BLOCK, 1) fused_sweep_kernel(const doubl
                 }
             }
         } else {
-            // ---- phase A: v sweep in place, warp <-> line ---------------------------------------------------
+            // ---- phase A: v sweep in place, warp <-> line; first the L lines (fetched one plane ahead), then,
+            //      once they have arrived, the H lines ---------------------------------------------------------
 #pragma unroll 1
-            for (int zr = warp; zr < Nz; zr += FUSED_THREADS / 32) {
+            for (int pass = 0; pass < 2; ++pass) {
+            const int cnt = pass ? NH : NL;
+            const int base = pass ? (par ? 0 : NL) : (par ? NH : 0);
+            if (pass && NH > 0) {
+                mbar_wait(&bars[2], phH);
+                phH ^= 1;
+            }
+#pragma unroll 1
+            for (int k = warp; k < cnt; k += FUSED_THREADS / 32) {
+                const int zr = base + k;
                 const int s = vs[zr];
                 double A[O][O], B[O][O];
 #pragma unroll
@@ -348,6 +384,7 @@ __global__ void __launch_bounds__(FUSED_BLOCK, 1) fused_sweep_kernel(const doubl
                     }
                 }
             }
+            }
             compute_sync();
             // ---- phase B: z sweep, thread <-> (v, slice of z), to global memory -------------------------------
             if (zact) {
@@ -361,16 +398,19 @@ __global__ void __launch_bounds__(FUSED_BLOCK, 1) fused_sweep_kernel(const doubl
                     }
                 int c = zi0 + zs[v];
                 if (c >= nz) c -= nz;
+                const int cstep = O * Pv;
+                int off = c * cstep + v;
                 double up[O];
 #pragma unroll
-                for (int m = 0; m < O; ++m) up[m] = tile[(size_t)(c * O + m) * Pv + v];
-                double *w = dst + v;
+                for (int m = 0; m < O; ++m) up[m] = tile[off + m * Pv];
+                double *w = dst + v + (long long)(zi0 * O) * g.sZ;
 #pragma unroll 2
                 for (int i = zi0; i < zi1; ++i) {
-                    c = (c + 1 == nz) ? 0 : c + 1;
+                    off += cstep;
+                    if (off >= NzPv) off -= NzPv;
                     double un[O];
 #pragma unroll
-                    for (int m = 0; m < O; ++m) un[m] = tile[(size_t)(c * O + m) * Pv + v];
+                    for (int m = 0; m < O; ++m) un[m] = tile[off + m * Pv];
 #pragma unroll
                     for (int j = 0; j < O; ++j) {
                         double acc = 0.0;
@@ -378,7 +418,8 @@ __global__ void __launch_bounds__(FUSED_BLOCK, 1) fused_sweep_kernel(const doubl
                         for (int m = 0; m < O; ++m) acc = fma(Az[j][m], up[m], acc);
 #pragma unroll
                         for (int m = 0; m < O; ++m) acc = fma(Bz[j][m], un[m], acc);
-                        __stcs(w + (long long)(i * O + j) * g.sZ, acc);
+                        __stcs(w, acc);
+                        w += g.sZ;
                     }
 #pragma unroll
                     for (int m = 0; m < O; ++m) up[m] = un[m];
