@@ -219,13 +219,27 @@ def run_ours(args):
         total_ms = float(t[0])
     mass1 = float(s.mass().cpu()[0])
 
-    # per-substep breakdown: a few extra steps, device events inside the library (same stream)
+    # breakdown of the Strang step: a few extra steps, device events inside the library (same stream)
     per = []
     for _ in range(max(3, min(K, 10))):
         s.strang_step(dt)
         per.append(s.last_timing_ms())
-    per = np.array(per)
-    med = np.median(per, axis=0)
+    med = np.median(np.array(per), axis=0)
+    fused = bool(int(med[6]) & 2)
+    # the substeps one by one (the calls of the boundary): z(dt/2), v(dt/2), xy(dt), each 2*|f|*8 bytes
+    single = {"z": [], "v": [], "xy": [], "xy_geometry": []}
+    for _ in range(max(3, min(K, 5))):
+        s.advect_z(0.5 * dt)
+        single["z"].append(s.last_timing_ms()[7])
+        s.advect_v(0.5 * dt)
+        single["v"].append(s.last_timing_ms()[7])
+        s.advect_xy(dt, 2)
+        t = s.last_timing_ms()
+        single["xy"].append(t[7])
+        single["xy_geometry"].append(t[2])
+        s.advect_v(0.5 * dt)
+        s.advect_z(0.5 * dt)
+    sm = {k: float(np.median(v)) for k, v in single.items()}
     ev0.record()
     rho = s.charge_density()
     ev1.record()
@@ -241,30 +255,35 @@ def run_ours(args):
     value = world * gbs(10 * nbytes, step_ms)
     peak, peak_src = measured_peak()
     sub = {
-        "advect_z_gbs": gbs(2 * nbytes, 0.5 * (med[0] + med[5])),
-        "advect_v_gbs": gbs(2 * nbytes, 0.5 * (med[1] + med[4])),
-        "advect_xy_gbs": gbs(2 * nbytes, med[3]),
-        "xy_ms": float(med[3]), "xy_geometry_kernel_ms": float(med[2]),
-        "xy_geometry_overlapped_with_apply": bool(med[6] > 0.5),
+        "advect_z_gbs": gbs(2 * nbytes, sm["z"]), "advect_v_gbs": gbs(2 * nbytes, sm["v"]),
+        "advect_xy_gbs": gbs(2 * nbytes, sm["xy"]),
+        "ms_single_calls": sm,
+        "xy_geometry_overlapped_with_apply": bool(int(med[6]) & 1),
         "charge_density_gbs": gbs(nbytes, rho_ms),
         "xy_apply_direct_path_blocks_total": s.debug_counter(0),
-        "ms": {"z": float(med[0]), "v": float(med[1]), "xy": float(med[3]), "v2": float(med[4]), "z2": float(med[5])},
+        "strang_step_fused_sweep_pairs": fused,
+        "strang_step_ms": ({"zv_fused": float(med[0]), "xy": float(med[3]), "vz_fused": float(med[4])} if fused else
+                           {"z": float(med[0]), "v": float(med[1]), "xy": float(med[3]), "v2": float(med[4]),
+                            "z2": float(med[5])}),
     }
     for k in ("advect_z_gbs", "advect_v_gbs", "advect_xy_gbs"):
         sub[k.replace("_gbs", "_frac_of_8TBs")] = sub[k] / NOMINAL_PEAK_GBS
-    # dominant kernel = the one with the largest share of the step
-    shares = {"advect_z": med[0] + med[5], "advect_v": med[1] + med[4], "xy_apply": med[3]}
-    dom = max(shares, key=shares.get)
-    dom_ms = {"advect_z": 0.5 * (med[0] + med[5]), "advect_v": 0.5 * (med[1] + med[4]), "xy_apply": med[3]}[dom]
-    achieved = gbs(2 * nbytes, dom_ms)
-    roofline = {"kernel": dom, "bound": "hbm", "achieved": achieved, "peak": peak, "unit": "GB/s",
-                "frac": achieved / peak, "traffic": ncu_traffic(dom, args.workload), "peak_source": peak_src,
-                "algorithmic_bytes_per_launch": 2 * nbytes, "launch_ms": float(dom_ms),
-                "share_of_step": float(shares[dom] / med[7]),
-                "all": {k: {"achieved": gbs(2 * nbytes, t), "frac": gbs(2 * nbytes, t) / peak,
-                            "traffic": ncu_traffic(k, args.workload)}
-                        for k, t in (("advect_z", 0.5 * (med[0] + med[5])), ("advect_v", 0.5 * (med[1] + med[4])),
-                                     ("xy_apply", med[3]))}}
+    # Roofline per kernel of the Strang step: achieved = the kernel's own algorithmic bytes (16 B per DOF: every
+    # kernel reads f once and writes it once -- a fused pair too, that is its point) / its launch duration.
+    if fused:
+        kern = {"fused_zv": float(med[0]), "xy_apply": float(med[3] - med[2]), "fused_vz": float(med[4])}
+    else:
+        kern = {"advect_z": 0.5 * float(med[0] + med[5]), "advect_v": 0.5 * float(med[1] + med[4]),
+                "xy_apply": float(med[3] - med[2])}
+    dom = max(kern, key=kern.get)
+    allk = {k: {"achieved": gbs(2 * nbytes, t), "frac": gbs(2 * nbytes, t) / peak, "launch_ms": t,
+                "share_of_step": t / float(med[7]), "traffic": ncu_traffic(k, args.workload)} for k, t in kern.items()}
+    allk["xy_geometry"] = {"launch_ms": float(med[2]), "share_of_step": float(med[2] / med[7]), "bound": "alu",
+                           "traffic": ncu_traffic("xy_geometry", args.workload)}
+    roofline = {"kernel": dom, "bound": "hbm", "achieved": allk[dom]["achieved"], "peak": peak, "unit": "GB/s",
+                "frac": allk[dom]["frac"], "traffic": allk[dom]["traffic"], "peak_source": peak_src,
+                "algorithmic_bytes_per_launch": 2 * nbytes, "launch_ms": allk[dom]["launch_ms"],
+                "share_of_step": allk[dom]["share_of_step"], "all": allk}
 
     # ---------------- end-to-end leg: host buffers through the C-ABI --------------------------------
     Ez_h, a_h, b_h = (torch.from_numpy(x).pin_memory() for x in (Ez, a, b))

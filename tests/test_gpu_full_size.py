@@ -1,0 +1,143 @@
+"""Parity at BASELINE.json's full size, in the launch configuration bench.py times (configs[4]: 128x128x64x64
+cells, o=2, the ITG profile and the prescribed ITG-shaped fields, dt=4).
+
+The oracle cannot run the whole 1.07 G DOF array in seconds, so every substep is checked on SAMPLED outputs that
+the oracle computes one by one from the same inputs:
+  * advect_z : whole z lines at sampled (v, y, x)            -- oracle.shift_line on the input line
+  * advect_v : whole v lines at sampled (z, y, x)            -- oracle.shift_line on the input line
+  * advect_xy: whole (y, x) planes at sampled (z, v)         -- oracle.advect_xy on that one plane
+  * the fused sweep pairs of sldg_strang_step: the state after a Strang step must equal, bit for bit, the state after
+    the five separate substep calls (each of which is checked against the oracle above)
+and on properties that hold at any size: mass (<= 1e-13 relative) and the charge density at sampled nodes.
+The state is read back through the internal layout (v fastest, [Nz][Ny][Nx][Pv]) so that no third copy of f is needed.
+"""
+import numpy as np
+import pytest
+
+import oracle
+from paper_2212_03036_b200 import inputs
+from paper_2212_03036_b200.inputs import GridSpec
+
+pytestmark = pytest.mark.gpu
+
+TOL = 1e-11
+CELLS = (128, 128, 64, 64)
+DT = 4.0
+
+
+@pytest.fixture(scope="module")
+def torch():
+    import torch as t
+    if not t.cuda.is_available():
+        pytest.skip("needs a CUDA device")
+    if t.cuda.get_device_properties(0).total_memory < 60e9:
+        pytest.skip("needs 60 GB of device memory")
+    return t
+
+
+@pytest.fixture(scope="module")
+def case(torch):
+    from paper_2212_03036_b200.binding import Sldg
+    spec = inputs.itg_grid(*CELLS, 2)
+    f0 = inputs.itg_initial_f(spec)
+    a, b, Ez, _ = inputs.itg_fields(spec, DT, 0.8)
+    s = Sldg(spec)
+    s.import_state_host(f0)
+    s.set_Ez(torch.from_numpy(Ez).cuda())
+    s.set_vxy(torch.from_numpy(a).cuda(), torch.from_numpy(b).cuda(), 1)
+    yield spec, f0, a, b, Ez, s
+    s.close()
+
+
+def _view(s):
+    """The current state in the internal layout, as a [Nz][Ny][Nx][Pv] view (layout 1: z, y, x, v)."""
+    Nz, Nv, Ny, Nx = s.spec.shape
+    cur = s.f_a if s.current_ptr() == s.f_a.data_ptr() else s.f_b
+    Pv = s.state_bytes // 8 // (Nz * Ny * Nx)
+    return cur.view(Nz, Ny, Nx, Pv)
+
+
+def _rel(got, ref, scale):
+    return np.abs(got - ref).max() / scale
+
+
+def test_c4_substeps_on_sampled_outputs(torch, case):
+    spec, f0, a, b, Ez, s = case
+    Nz, Nv, Ny, Nx = spec.shape
+    rng = np.random.default_rng(11)
+    scale = np.abs(f0).max()
+    o = 2
+    xi, _ = oracle.gl(o)
+
+    # ---- advect_z(dt/2): z lines ------------------------------------------------------------------------
+    f_in = f0
+    s.advect_z(0.5 * DT)
+    s.check()
+    V = _view(s)
+    for _ in range(48):
+        v, y, x = int(rng.integers(Nv)), int(rng.integers(Ny)), int(rng.integers(Nx))
+        vq = spec.lo[3] + (v // o + xi[v % o]) * spec.h[3]
+        ref = oracle.shift_line(f_in[:, v, y, x].copy(), o, vq * (0.5 * DT) / spec.h[2])
+        got = V[:, y, x, v].cpu().numpy()
+        assert _rel(got, ref, scale) <= TOL, ("z", v, y, x)
+    # the next substep's input, on the host: only the sampled lines are needed -> read them from the device
+    # ---- advect_v(dt/2): v lines ------------------------------------------------------------------------
+    samples = [(int(rng.integers(Nz)), int(rng.integers(Ny)), int(rng.integers(Nx))) for _ in range(48)]
+    lines_in = [V[z, y, x, :Nv].cpu().numpy().copy() for (z, y, x) in samples]
+    s.advect_v(0.5 * DT)
+    s.check()
+    V = _view(s)
+    for (z, y, x), u in zip(samples, lines_in):
+        ref = oracle.shift_line(u, o, Ez[z, y, x] * (0.5 * DT) / spec.h[3])
+        got = V[z, y, x, :Nv].cpu().numpy()
+        assert _rel(got, ref, scale) <= TOL, ("v", z, y, x)
+    # ---- advect_xy(dt): (y, x) planes -------------------------------------------------------------------
+    planes = [(int(rng.integers(Nz)), int(rng.integers(Nv))) for _ in range(3)] + [(0, 0), (Nz - 1, Nv - 1)]
+    planes_in = [V[z, :, :, v].cpu().numpy().copy() for (z, v) in planes]
+    s.advect_xy(DT, 2)
+    s.check()
+    assert s.debug_counter(0) == 0, "some apply blocks left the staged path at bench size"
+    V = _view(s)
+    spec2 = GridSpec(n=(spec.n[0], spec.n[1], 1, 1), order=(o, o, 1, 1), lo=(spec.lo[0], spec.lo[1], 0.0, 0.0),
+                     hi=(spec.hi[0], spec.hi[1], 1.0, 1.0))
+    for (z, v), pin in zip(planes, planes_in):
+        fz = np.ascontiguousarray(pin.reshape(1, 1, Ny, Nx))
+        ref = oracle.advect_xy(spec2, fz, np.ascontiguousarray(a[z:z + 1]), np.ascontiguousarray(b[z:z + 1]), DT, 2, 1)
+        got = V[z, :, :, v].cpu().numpy()
+        assert _rel(got, ref[0, 0], scale) <= TOL, ("xy", z, v)
+
+
+def test_c4_strang_step_fused_equals_separate_calls_and_conserves_mass(torch, case, monkeypatch):
+    spec, f0, a, b, Ez, s = case
+    from paper_2212_03036_b200.binding import Sldg
+    Nz, Nv, Ny, Nx = spec.shape
+    s.import_state_host(f0)
+    m0 = float(s.mass().cpu()[0])
+    rho0 = s.charge_density().cpu().numpy()
+    # charge density at sampled nodes against the Gauss sum written out
+    _, w = oracle.gl(2)
+    rng = np.random.default_rng(5)
+    for _ in range(32):
+        z, y, x = int(rng.integers(Nz)), int(rng.integers(Ny)), int(rng.integers(Nx))
+        ref = spec.h[3] * float(np.sum(f0[z, :, y, x].reshape(-1, 2) * w[None, :]))
+        assert abs(rho0[z, y, x] - ref) <= TOL * abs(ref)
+    s.strang_step(DT)
+    s.check()
+    assert int(s.last_timing_ms()[6]) & 2, "the fused sweep pairs did not run at bench size"
+    m1 = float(s.mass().cpu()[0])
+    assert abs(m1 - m0) <= 1e-13 * abs(m0)
+    # the same step as five separate calls in a second context
+    monkeypatch.setenv("SLDG_NO_FUSE", "1")
+    t = Sldg(spec)
+    t.import_state_host(f0)
+    t.set_Ez(torch.from_numpy(Ez).cuda())
+    t.set_vxy(torch.from_numpy(a).cuda(), torch.from_numpy(b).cuda(), 1)
+    t.advect_z(0.5 * DT)
+    t.advect_v(0.5 * DT)
+    t.advect_xy(DT, 2)
+    t.advect_v(0.5 * DT)
+    t.advect_z(0.5 * DT)
+    t.check()
+    same = bool(torch.equal(_view(s)[..., :Nv], _view(t)[..., :Nv]))
+    t.close()
+    assert same
