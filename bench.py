@@ -225,7 +225,7 @@ def run_ours(args):
         s.strang_step(dt)
         per.append(s.last_timing_ms())
     med = np.median(np.array(per), axis=0)
-    fused = bool(int(med[6]) & 2)
+    fused_zv, fused_vz = bool(int(med[6]) & 2), bool(int(med[6]) & 4)
     # the substeps one by one (the calls of the boundary): z(dt/2), v(dt/2), xy(dt), each 2*|f|*8 bytes
     single = {"z": [], "v": [], "xy": [], "xy_geometry": []}
     for _ in range(max(3, min(K, 5))):
@@ -261,20 +261,18 @@ def run_ours(args):
         "xy_geometry_overlapped_with_apply": bool(int(med[6]) & 1),
         "charge_density_gbs": gbs(nbytes, rho_ms),
         "xy_apply_direct_path_blocks_total": s.debug_counter(0),
-        "strang_step_fused_sweep_pairs": fused,
-        "strang_step_ms": ({"zv_fused": float(med[0]), "xy": float(med[3]), "vz_fused": float(med[4])} if fused else
-                           {"z": float(med[0]), "v": float(med[1]), "xy": float(med[3]), "v2": float(med[4]),
-                            "z2": float(med[5])}),
+        "strang_step_fused_sweep_pairs": {"zv": fused_zv, "vz": fused_vz},
+        "strang_step_ms": dict(({"zv_fused": float(med[0])} if fused_zv else {"z": float(med[0]), "v": float(med[1])}),
+                               xy=float(med[3]),
+                               **({"vz_fused": float(med[4])} if fused_vz else {"v2": float(med[4]), "z2": float(med[5])})),
     }
     for k in ("advect_z_gbs", "advect_v_gbs", "advect_xy_gbs"):
         sub[k.replace("_gbs", "_frac_of_8TBs")] = sub[k] / NOMINAL_PEAK_GBS
     # Roofline per kernel of the Strang step: achieved = the kernel's own algorithmic bytes (16 B per DOF: every
     # kernel reads f once and writes it once -- a fused pair too, that is its point) / its launch duration.
-    if fused:
-        kern = {"fused_zv": float(med[0]), "xy_apply": float(med[3] - med[2]), "fused_vz": float(med[4])}
-    else:
-        kern = {"advect_z": 0.5 * float(med[0] + med[5]), "advect_v": 0.5 * float(med[1] + med[4]),
-                "xy_apply": float(med[3] - med[2])}
+    kern = {"xy_apply": float(med[3] - med[2])}
+    kern.update({"fused_zv": float(med[0])} if fused_zv else {"advect_z": float(med[0]), "advect_v": float(med[1])})
+    kern.update({"fused_vz": float(med[4])} if fused_vz else {"advect_v": float(med[4]), "advect_z": float(med[5])})
     dom = max(kern, key=kern.get)
     allk = {k: {"achieved": gbs(2 * nbytes, t), "frac": gbs(2 * nbytes, t) / peak, "launch_ms": t,
                 "share_of_step": t / float(med[7]), "traffic": ncu_traffic(k, args.workload)} for k, t in kern.items()}

@@ -129,8 +129,9 @@ int sldg_check(sldg_ctx *ctx);
  * ms[0] z  ms[1] v  ms[3] the WHOLE xy substep (geometry + apply, first launch to last)  ms[4] v  ms[5] z
  * ms[7] total -- all on the context's stream; ms[2] = duration of the geometry kernel alone on the library's
  * internal stream (it is part of ms[3], not in addition to it); ms[6] = flags: +1 if that kernel ran concurrently
- * with the apply, +2 if each pair of adjacent sweeps (z,v before the 2d step; v,z after it) ran fused in one pass
- * over f -- then ms[0] and ms[4] hold the time of a whole pair and ms[1] = ms[5] = 0.
+ * with the apply, +2 if the first pair of adjacent sweeps (z,v before the 2d step) ran fused in one pass over f
+ * -- then ms[0] holds the time of the pair and ms[1] = 0 --, +4 if the second pair (v,z after it) did -- then
+ * ms[4] holds the time of the pair and ms[5] = 0.
  * After a single sldg_advect_* call only that entry (and ms[7]) is set.  Synchronises. */
 int sldg_last_timing_ms(sldg_ctx *ctx, float ms[8]);
 /* Number of kernels the library launched on behalf of this context since creation. */

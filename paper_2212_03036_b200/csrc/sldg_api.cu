@@ -489,7 +489,7 @@ int sldg_strang_step(sldg_ctx *c, double dt)
     cudaEventRecord(c->ev[3], c->stream);
     if ((rc = do_pair(c, 0.5 * dt, false, c->ev[4], &fused1))) return rc;
     cudaEventRecord(c->ev[5], c->stream);
-    c->last_fused = fused0 && fused1;
+    c->last_fused = (fused0 ? 2 : 0) + (fused1 ? 4 : 0);
     c->ev_kind = 1;
     return SLDG_OK;
 }
@@ -558,7 +558,7 @@ int sldg_last_timing_ms(sldg_ctx *c, float ms[8])
     if (c->ev_kind == 1) {
         ms[0] = el(0, 1); ms[1] = el(1, 2); ms[3] = el(2, 3); ms[4] = el(3, 4); ms[5] = el(4, 5);
         ms[2] = geom();
-        ms[6] = ((c->overlap && xy_apply_can_overlap(c)) ? 1.0f : 0.0f) + (c->last_fused ? 2.0f : 0.0f);
+        ms[6] = ((c->overlap && xy_apply_can_overlap(c)) ? 1.0f : 0.0f) + (float)c->last_fused;
         ms[7] = el(0, 5);
     } else if (c->ev_kind == 2) {
         ms[0] = ms[7] = el(0, 1);

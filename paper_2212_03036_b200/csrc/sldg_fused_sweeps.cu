@@ -7,13 +7,12 @@
 // 128 x 128 -- fits in shared memory.  The arithmetic of each sweep is that of sldg_sweeps.cu, operation by
 // operation, so the fused pair is bit-identical to the two separate kernels.
 //
-// One persistent block (512 threads) per SM walks over the (Y,X) planes:
-//   stage   the NEXT plane's lines are fetched under the compute phases of the current one: NL of its Nz lines by
-//           cp.async into the spare shared memory, the other NH = Nz - NL into REGISTERS (coalesced 16-byte
-//           loads, R doubles per thread).  Shared memory holds [L_a: NL lines | H: NH lines | L_b: NL lines];
-//           even planes live in [L_a | H] (lines 0..NL-1 asynchronous), odd planes in [H | L_b] (lines NH..Nz-1
-//           asynchronous), so a plane is always one contiguous tile [Nz][Pv] and the other L is free;
-//   tile    registers -> the H lines of the tile;
+// One persistent block (16 compute warps + 1 producer warp) per SM walks over the (Y,X) planes:
+//   stage   a dedicated producer warp fetches the planes with bulk copies (one per line, completing on mbarriers).
+//           Shared memory holds [L_a: NL lines | H: NH lines | L_b: NL lines], NL + NH = Nz: even planes live in
+//           [L_a | H], odd planes in [H | L_b], so a plane is always one contiguous tile [Nz][Pv] and the other L
+//           is free: NL lines of the NEXT plane are fetched under the compute phases of the current one, the
+//           remaining NH lines as soon as the current plane is done (NL = 80 of 128 at 128 x 128, o = 2);
 //   ZV      phase A  z sweep in place, thread <-> (v, slice of z): the result for target cell i is written over
 //                    its left source cell (i+s) mod nz, which is dead by then -- column v ends up rotated by s(v);
 //           phase B  v sweep line by line, warp <-> line, gathering through the per-column rotation, results
@@ -449,6 +448,10 @@ cudaError_t launch_fused_sweeps(sldg_ctx *c, const double *fin, double *fout, do
     if (tables + row * Nz > budget) return cudaErrorNotSupported;
     long long NLl = (long long)((budget - tables) / row) - Nz;  // spare lines = lines fetched one plane ahead
     const int NL = (int)(NLl > Nz ? Nz : (NLl < 0 ? 0 : NLl));
+    // z first: the z sweep cannot start before the whole plane is there, so the lines that do not fit beside the
+    // current plane (NH = Nz - NL, fetched only when it is done) are fully exposed; measured at 144 x 144 (o = 3,
+    // NL = 0.28 Nz) the pair is then slower than the two separate kernels.  v first hides them under its L lines.
+    if (z_first && 2 * NL < Nz) return cudaErrorNotSupported;
     const size_t smem = tables + row * (size_t)(2 * NL + (Nz - NL));
     const bool cpl2 = g.n[3] <= 64;
     const int ncol = g.N[0] * g.N[1];

@@ -423,11 +423,14 @@ __global__ void __launch_bounds__(32 * (STREAM_TX * VSPLIT + 1), 1) xy_apply_str
 }
 
 // --------------------------------------------------------------------------------------------------
-// direct apply (any o): block = 8 warps, a tile of 8x4 target cells at one z node and one chunk of
-// 32*NVT v values; warp <-> target cell (4 cells per warp), lane <-> v.  Inputs through L1.
+// direct apply (any o): block = 8 warps, a tile of 8x4 target cells at one z node and one chunk of 32*NV v
+// values; warp <-> target cell (4 cells per warp), lane <-> the v values lane + 32 e, e < NV (coalesced 256-byte
+// loads).  Per source cell and source node k: NV inputs per lane, then o^2 weights W[k][m] (warp-uniform loads,
+// contiguous in m) each feeding NV FMAs -- o^2 NV accumulators per lane, o^2 + NV loads per o^2 NV FMAs.
+// Inputs and weights through L1/L2.  At o = 3 the step is bound by the fp64 pipe (2*9*c FMA per DOF).
 // --------------------------------------------------------------------------------------------------
-template <int O, int NVT>
-__global__ void __launch_bounds__(256) xy_apply_direct_kernel(const double *__restrict__ fin,
+template <int O, int NV>
+__global__ void __launch_bounds__(256, 2) xy_apply_direct_kernel(const double *__restrict__ fin,
                                                               double *__restrict__ fout,
                                                               const int4 *__restrict__ hdrg,
                                                               const double *__restrict__ W, GridDev g)
@@ -438,8 +441,11 @@ __global__ void __launch_bounds__(256) xy_apply_direct_kernel(const double *__re
     const int tile_i = (blockIdx.x % tiles_x) * TX, tile_j = (blockIdx.x / tiles_x) * TY;
     const int z = blockIdx.z;
     const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
-    const int v = (blockIdx.y * 32 + lane) * NVT;
+    const int v = blockIdx.y * 32 * NV + lane;
     if (v >= g.Pv) return;
+    int nve = 0;  // values of this lane inside the line
+#pragma unroll
+    for (int e = 0; e < NV; ++e) nve += (v + 32 * e < g.Pv) ? 1 : 0;
     const long long ncell = (long long)nx * ny;
     const double *fz = fin + z * g.sZ + v;
     double *oz = fout + z * g.sZ + v;
@@ -448,16 +454,16 @@ __global__ void __launch_bounds__(256) xy_apply_direct_kernel(const double *__re
         const int i = tile_i + (c % TX), j = tile_j + (c / TX);
         if (i >= nx || j >= ny) continue;
         const long long cellid = (long long)z * ncell + (long long)j * nx + i;
-        const int4 h = __ldg(hdrg + cellid);
+        const int4 h = __ldcg(hdrg + cellid);
         const int ax = wrap_idx(i + h.x, nx);
         const int ay = wrap_idx(j + h.y, ny);
         const int msk = h.z;
         int nb = 0;
-        double acc[O2][NVT];
+        double acc[O2][NV];
 #pragma unroll
         for (int m = 0; m < O2; ++m)
 #pragma unroll
-            for (int e = 0; e < NVT; ++e) acc[m][e] = 0.0;
+            for (int e = 0; e < NV; ++e) acc[m][e] = 0.0;
 #pragma unroll 1
         for (int slot = 0; slot < 9; ++slot) {
             if (!((msk >> slot) & 1)) continue;
@@ -470,20 +476,15 @@ __global__ void __launch_bounds__(256) xy_apply_direct_kernel(const double *__re
 #pragma unroll
                 for (int kp = 0; kp < O; ++kp) {
                     const double *src = fz + (long long)(s * O + kq) * g.sY + (long long)(r * O + kp) * g.sX;
-                    double in[NVT];
-                    if (NVT == 2) {
-                        double2 t = __ldg(reinterpret_cast<const double2 *>(src));
-                        in[0] = t.x;
-                        in[NVT - 1] = t.y;
-                    } else {
-                        in[0] = __ldg(src);
-                    }
+                    double in[NV];
+#pragma unroll
+                    for (int e = 0; e < NV; ++e) in[e] = e < nve ? __ldg(src + 32 * e) : 0.0;
                     const int k = kp + O * kq;
 #pragma unroll
                     for (int m = 0; m < O2; ++m) {
                         const double w = __ldg(Wp + k * O2 + m);
 #pragma unroll
-                        for (int e = 0; e < NVT; ++e) acc[m][e] = fma(w, in[e], acc[m][e]);
+                        for (int e = 0; e < NV; ++e) acc[m][e] = fma(w, in[e], acc[m][e]);
                     }
                 }
         }
@@ -493,10 +494,9 @@ __global__ void __launch_bounds__(256) xy_apply_direct_kernel(const double *__re
             for (int mp = 0; mp < O; ++mp) {
                 double *dst = oz + (long long)(j * O + mq) * g.sY + (long long)(i * O + mp) * g.sX;
                 const int m = mp + O * mq;
-                if (NVT == 2)
-                    *reinterpret_cast<double2 *>(dst) = make_double2(acc[m][0], acc[m][NVT - 1]);
-                else
-                    dst[0] = acc[m][0];
+#pragma unroll
+                for (int e = 0; e < NV; ++e)
+                    if (e < nve) __stcs(dst + 32 * e, acc[m][e]);
             }
     }
 }
@@ -521,13 +521,21 @@ cudaError_t launch_xy_apply(sldg_ctx *c, const double *fin, double *fout, bool w
         c->launches++;
         return cudaGetLastError();
     }
-    constexpr int NVT = 2;
     const int tiles = ((g.n[0] + 7) / 8) * ((g.n[1] + 3) / 4);
-    const int vchunks = (g.Pv + 32 * NVT - 1) / (32 * NVT);
+    // values per lane: as many as cover the line in one chunk, at most 5 (45 accumulators at o = 3)
+    int nv = (g.Pv + 31) / 32;
+    if (nv > 5) nv = 4;
+    const int vchunks = (g.Pv + 32 * nv - 1) / (32 * nv);
     dim3 grid((unsigned)tiles, (unsigned)vchunks, (unsigned)g.N[2]);
-#define LAUNCH_A(OO) \
-    xy_apply_direct_kernel<OO, NVT><<<grid, 256, 0, c->stream>>>(fin, fout, c->hdr, c->W, g)
-    if (O == 1) LAUNCH_A(1); else if (O == 2) LAUNCH_A(2); else LAUNCH_A(3);
+#define LAUNCH_A(OO, NN) \
+    xy_apply_direct_kernel<OO, NN><<<grid, 256, 0, c->stream>>>(fin, fout, c->hdr, c->W, g)
+#define LAUNCH_AN(OO)                                                                                         \
+    do {                                                                                                      \
+        if (nv == 1) LAUNCH_A(OO, 1); else if (nv == 2) LAUNCH_A(OO, 2); else if (nv == 3) LAUNCH_A(OO, 3);   \
+        else if (nv == 4) LAUNCH_A(OO, 4); else LAUNCH_A(OO, 5);                                              \
+    } while (0)
+    if (O == 1) LAUNCH_AN(1); else if (O == 2) LAUNCH_AN(2); else LAUNCH_AN(3);
+#undef LAUNCH_AN
 #undef LAUNCH_A
     c->launches++;
     return cudaGetLastError();
