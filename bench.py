@@ -113,6 +113,23 @@ class ClockSampler:
                 "reasons": sorted(reasons), "samples": len(sm)}
 
 
+def max_over_ranks(ms, world, device="cuda"):
+    """The time every replica-set number is quoted on: the slowest rank's (all ranks get the same value)."""
+    if world <= 1:
+        return float(ms)
+    import torch
+    import torch.distributed as dist
+    t = torch.tensor([ms], dtype=torch.float64, device=device)
+    dist.all_reduce(t, op=dist.ReduceOp.MAX)
+    return float(t[0])
+
+
+def replicas_value(nbytes_per_step_per_rank, ms_per_step, world):
+    """Whole-job throughput of `world` independent replicas (no sharding, no collectives on the data path):
+    bytes of all replicas over the slowest rank's time."""
+    return world * gbs(nbytes_per_step_per_rank, ms_per_step)
+
+
 def gbs(nbytes, ms):
     return nbytes / (ms * 1e-3) / 1e9 if ms > 0 else None
 
@@ -213,10 +230,7 @@ def run_ours(args):
     launches = s.launch_count() - launches0
     clocks = sampler.stop(t_wall0, t_wall1) if rank == 0 else None
     s.check()
-    if world > 1:
-        t = torch.tensor([total_ms], dtype=torch.float64, device="cuda")
-        dist.all_reduce(t, op=dist.ReduceOp.MAX)
-        total_ms = float(t[0])
+    total_ms = max_over_ranks(total_ms, world)
     mass1 = float(s.mass().cpu()[0])
 
     # breakdown of the Strang step: a few extra steps, device events inside the library (same stream)
@@ -252,7 +266,7 @@ def run_ours(args):
 
     nbytes = spec.dofs * 8.0
     step_ms = total_ms / K
-    value = world * gbs(10 * nbytes, step_ms)
+    value = replicas_value(10 * nbytes, step_ms, world)
     peak, peak_src = measured_peak()
     sub = {
         "advect_z_gbs": gbs(2 * nbytes, sm["z"]), "advect_v_gbs": gbs(2 * nbytes, sm["v"]),
@@ -295,11 +309,8 @@ def run_ours(args):
         s.strang_step_host(dt, Ez_h, a_h, b_h, 1, rho_h, mass_h)
     barrier()
     e2e_ms = (time.perf_counter() - t0) * 1e3 / K
-    if world > 1:
-        t = torch.tensor([e2e_ms], dtype=torch.float64, device="cuda")
-        dist.all_reduce(t, op=dist.ReduceOp.MAX)
-        e2e_ms = float(t[0])
-    e2e = {"value": world * gbs(10 * nbytes, e2e_ms), "unit": "GB/s", "ms_per_step": e2e_ms,
+    e2e_ms = max_over_ranks(e2e_ms, world)
+    e2e = {"value": replicas_value(10 * nbytes, e2e_ms, world), "unit": "GB/s", "ms_per_step": e2e_ms,
            "h2d_bytes_per_step": int(Ez_h.numel() * 8 + a_h.numel() * 8 + b_h.numel() * 8),
            "d2h_bytes_per_step": int(rho_h.numel() * 8 + 8),
            "what": "sldg_strang_step_host: pinned Ez,a,b -> device, Strang step, rho and mass -> host; f stays resident"}
