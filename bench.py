@@ -174,6 +174,54 @@ def run_reference(args):
     return 0
 
 
+def run_xy_only(args):
+    """BASELINE.json configs[1]: the 2d step alone on 256x256 cells, batched over 4096 planes that share one velocity
+    field; solid-body rotation, one period in 40 steps (trace order 2).  A step = one sldg_advect_xy."""
+    import math
+
+    import torch
+
+    from paper_2212_03036_b200.binding import Sldg
+
+    order = 3 if args.workload.endswith("o3") else 2
+    spec = inputs.bumps_grid(256, 4096, order)
+    s = Sldg(spec)
+    s.import_state_host(inputs.bumps_initial_f(spec, seed=1))
+    a, b = inputs.rotation_velocity(spec)
+    s.set_vxy(torch.from_numpy(a).cuda(), torch.from_numpy(b).cuda(), 0)
+    tau = 2.0 * math.pi / 40
+    mass0 = float(s.mass().cpu()[0])
+    for _ in range(args.warmup):
+        s.advect_xy(tau, 2)
+    s.check()
+    ev0, ev1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    torch.cuda.synchronize()
+    ev0.record()
+    for _ in range(args.steps):
+        s.advect_xy(tau, 2)
+    ev1.record()
+    torch.cuda.synchronize()
+    s.check()
+    ms = ev0.elapsed_time(ev1) / args.steps
+    geom_ms = s.last_timing_ms()[2]
+    mass1 = float(s.mass().cpu()[0])
+    nbytes = spec.dofs * 8.0
+    peak, peak_src = measured_peak()
+    v = gbs(2 * nbytes, ms)
+    print(json.dumps({
+        "metric": "effective_hbm_gbs_per_xy_substep", "value": v, "unit": "GB/s", "n_gpus": 1, "steps": args.steps,
+        "warmup": args.warmup, "ms_per_step": ms, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
+        "dtype": "f64", "data": "synthetic",
+        "config": {"workload": f"BASELINE.json configs[1]: 2d SLDG alone, 256x256 cells, o={order}, 4096 planes of seeded "
+                               "Gaussian bumps, solid-body rotation (one period = 40 steps)", "dofs": spec.dofs,
+                   "state_GB": nbytes / 1e9},
+        "frac_of_8TBs": v / NOMINAL_PEAK_GBS, "frac_of_measured": v / peak, "xy_geometry_kernel_ms": geom_ms,
+        "mass_drift_rel": abs(mass1 - mass0) / abs(mass0), "gpu_launches": int(s.launch_count()),
+    }), flush=True)
+    s.close()
+    return 0
+
+
 def run_ours(args):
     import torch
     import torch.distributed as dist
@@ -221,11 +269,20 @@ def run_ours(args):
     barrier()
     t_wall0 = time.time()
     ev0.record()
-    for _ in range(K):
+    log = open(args.per_step_log, "w") if (args.per_step_log and rank == 0) else None
+    for n in range(K):
         s.strang_step(dt)
+        if log:
+            t = s.last_timing_ms()
+            m = float(s.mass().cpu()[0])
+            log.write(json.dumps({"step": n, "ms": [float(x) for x in t[:6]], "total_ms": float(t[7]),
+                                  "strang_gbs": gbs(10 * spec.dofs * 8.0, t[7]),
+                                  "mass_drift_rel": abs(m - mass0) / abs(mass0)}) + "\n")
     ev1.record()
     barrier()
     t_wall1 = time.time()
+    if log:
+        log.close()
     total_ms = ev0.elapsed_time(ev1)
     launches = s.launch_count() - launches0
     clocks = sampler.stop(t_wall0, t_wall1) if rank == 0 else None
@@ -351,13 +408,18 @@ def main():
     ap.add_argument("--steps", type=int, default=10)
     ap.add_argument("--warmup", type=int, default=3)
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
-    ap.add_argument("--workload", default="c4", choices=sorted(WORKLOADS))
+    ap.add_argument("--workload", default="c4", choices=sorted(WORKLOADS) + ["c1o2", "c1o3"])
+    ap.add_argument("--per-step-log", default=None,
+                    help="write one JSON line per timed Strang step (substep ms, GB/s, mass drift) to this file; the "
+                         "step loop then synchronises every step (BASELINE.json configs[3] asks for these records)")
     ap.add_argument("--layout", type=int, default=0)
     ap.add_argument("--no-cpu-baseline", action="store_true")
     args = ap.parse_args()
     args.warmup = max(args.warmup, 3) if args.impl == "ours" else args.warmup
     if args.impl == "reference":
         return run_reference(args)
+    if args.workload in ("c1o2", "c1o3"):
+        return run_xy_only(args)
     return run_ours(args)
 
 

@@ -169,6 +169,10 @@ void fill_shift_poly(int o, ShiftPoly *sp)
     long double x[5], w[5], L[SLDG_MAXO][SLDG_MAXO];
     gl_nodes(o, x, w);
     lagrange_monomials(o, x, L);
+    for (int j = 0; j < o; ++j) {
+        sp->w[j] = (double)w[j];
+        sp->iw[j] = 1.0 / sp->w[j];
+    }
     const int deg = 2 * o;  // number of coefficients (degree 2o-1)
     auto one_minus_alpha_pow = [&](int n) {
         Poly r(n + 1);
@@ -269,6 +273,7 @@ int sldg_create(const sldg_params *p, double *f_a_dev, double *f_b_dev, void *wo
     c->xy_epoch = 0;
     c->overlap = getenv("SLDG_XY_OVERLAP") ? 1 : 0;  // experimental: co-running the two kernels is slower today
     c->fuse = getenv("SLDG_NO_FUSE") ? 0 : 1;
+    c->own_geometry = getenv("SLDG_XY_OWN_GEOMETRY") ? 1 : 0;
     c->trace_order = 2;
     c->vel_periodic = 0;
     if (cudaDeviceGetAttribute(&c->sm_count, cudaDevAttrMultiProcessorCount, dev) != cudaSuccess) {
@@ -421,16 +426,35 @@ static int do_pair(sldg_ctx *c, double tau, bool z_first, cudaEvent_t mid, int *
 // geometry kernel.
 static int do_xy(sldg_ctx *c, double tau, int trace_order)
 {
+    if (c->own_geometry && xy_apply_can_overlap(c)) {
+        // one kernel: every apply block computes the geometry of its own strip first
+        cudaEventRecord(c->gev[1], c->stream);
+        cudaEventRecord(c->gev[2], c->stream);
+        if (launch_xy_apply(c, c->f[c->cur], c->f[c->cur ^ 1], false, true, tau, trace_order) != cudaSuccess)
+            return SLDG_ECUDA;
+        swap_state(c);
+        return SLDG_OK;
+    }
     const bool overlap = c->overlap && xy_apply_can_overlap(c);
     c->xy_epoch++;
+    if (!overlap) {
+        // back to back on the caller's stream
+        cudaEventRecord(c->gev[1], c->stream);
+        if (launch_xy_geometry(c, c->stream, tau, trace_order) != cudaSuccess) return SLDG_ECUDA;
+        cudaEventRecord(c->gev[2], c->stream);
+        if (launch_xy_apply(c, c->f[c->cur], c->f[c->cur ^ 1], false, false, tau, trace_order) != cudaSuccess)
+            return SLDG_ECUDA;
+        swap_state(c);
+        return SLDG_OK;
+    }
     cudaEventRecord(c->gev[0], c->stream);
     cudaStreamWaitEvent(c->gstream, c->gev[0], 0);
     cudaEventRecord(c->gev[1], c->gstream);
     if (launch_xy_geometry(c, c->gstream, tau, trace_order) != cudaSuccess) return SLDG_ECUDA;
     cudaEventRecord(c->gev[2], c->gstream);
-    if (!overlap) cudaStreamWaitEvent(c->stream, c->gev[2], 0);
-    if (launch_xy_apply(c, c->f[c->cur], c->f[c->cur ^ 1], overlap) != cudaSuccess) return SLDG_ECUDA;
-    if (overlap) cudaStreamWaitEvent(c->stream, c->gev[2], 0);  // join (the geometry has long finished)
+    if (launch_xy_apply(c, c->f[c->cur], c->f[c->cur ^ 1], true, false, tau, trace_order) != cudaSuccess)
+        return SLDG_ECUDA;
+    cudaStreamWaitEvent(c->stream, c->gev[2], 0);  // join (the geometry has long finished)
     swap_state(c);
     return SLDG_OK;
 }

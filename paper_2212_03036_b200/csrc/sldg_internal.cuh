@@ -37,6 +37,7 @@ struct Basis {
 struct ShiftPoly {
     double a[SLDG_MAXO][SLDG_MAXO][2 * SLDG_MAXO];
     double b[SLDG_MAXO][SLDG_MAXO][2 * SLDG_MAXO];
+    double w[SLDG_MAXO], iw[SLDG_MAXO];  // Gauss-Legendre weights of this order and their reciprocals
     int o;
 };
 
@@ -61,6 +62,7 @@ struct sldg_ctx {
     cudaStream_t gstream;   // internal high-priority stream: the geometry kernel runs here, under the apply
     cudaEvent_t gev[4];     // xy start (main), geometry start/end (gstream), previous apply done (main)
     int fuse, last_fused;   // fuse: sldg_strang_step runs each pair of adjacent sweeps in one pass
+    int own_geometry;       // 1: the o = 2 apply kernel computes the geometry of its strips itself
     int overlap;            // 1: geometry and apply of one xy step run concurrently (o = 2 path)
     size_t n_partials;
     int trace_order, vel_periodic;
@@ -82,5 +84,6 @@ cudaError_t launch_xy_geometry(sldg_ctx *c, cudaStream_t stream, double tau, int
 int xy_geometry_blocks_per_z(const sldg_ctx *c);
 bool xy_apply_can_overlap(const sldg_ctx *c);
 cudaError_t launch_geometry_expand(sldg_ctx *c, int z, int32_t *anchor, int32_t *mask, double *Wd);
-cudaError_t launch_xy_apply(sldg_ctx *c, const double *fin, double *fout, bool wait_flags);
+cudaError_t launch_xy_apply(sldg_ctx *c, const double *fin, double *fout, bool wait_flags, bool own_geometry,
+                            double tau, int trace_order);
 cudaError_t launch_fused_sweeps(sldg_ctx *c, const double *fin, double *fout, double tau_z, double tau_v, bool z_first);

@@ -22,6 +22,7 @@
 #include <stdlib.h>
 
 #include "sldg_internal.cuh"
+#include "sldg_xy_geometry.cuh"
 
 __device__ __forceinline__ int wrap_idx(int i, int n)
 {
@@ -99,8 +100,8 @@ __device__ __forceinline__ void fma_block_o2_direct(double (&acc)[4][2], const d
 {
 #pragma unroll
     for (int k = 0; k < 4; ++k) {
-        const double2 w01 = *reinterpret_cast<const double2 *>(Wp + k * 4);
-        const double2 w23 = *reinterpret_cast<const double2 *>(Wp + k * 4 + 2);
+        const double2 w01 = __ldcg(reinterpret_cast<const double2 *>(Wp + k * 4));
+        const double2 w23 = __ldcg(reinterpret_cast<const double2 *>(Wp + k * 4 + 2));
         acc[0][0] = fma(w01.x, in[k].x, acc[0][0]);
         acc[0][1] = fma(w01.x, in[k].y, acc[0][1]);
         acc[1][0] = fma(w01.y, in[k].x, acc[1][0]);
@@ -127,11 +128,22 @@ constexpr size_t STREAM_HDR_BYTES = (size_t)STREAM_LMAX * STREAM_TX * 16;
 constexpr size_t STREAM_SMEM = STREAM_RING_BYTES + STREAM_WRING_BYTES + STREAM_HDR_BYTES + 512;
 constexpr long long STREAM_SPIN_LIMIT = 4000000000ll;  // cycles (~2 s): a stuck flag becomes an error, not a hang
 
-template <int VSPLIT>
+// Arguments of the geometry when the apply kernel computes it itself (GEOM): the fields and the step.
+struct GeomArgs {
+    const double *va, *vb;
+    double tau;
+    int order, periodic;
+};
+constexpr int STREAM_GEOM_CELLS = 256;  // target cells per geometry pass of a block (scratch: the idle input ring)
+
+// GEOM: every block first computes the geometry of its own strip (sldg_xy_geometry.cuh; headers and weights go to
+// global memory as in the stand-alone kernel and are read back through L2), then streams.  The geometry is
+// compute only, the streaming is bandwidth only: with the blocks of the grid out of step with one another the
+// one hides under the other, and the weights never wait in HBM for a second kernel.
+template <int VSPLIT, bool GEOM>
 __global__ void __launch_bounds__(32 * (STREAM_TX * VSPLIT + 1), 1) xy_apply_stream_kernel(
-    const double *__restrict__ fin, double *__restrict__ fout, const int4 *__restrict__ hdrg,
-    const double *__restrict__ W, GridDev g, int L, const unsigned long long *zflag,
-    unsigned long long flag_target, int32_t *err)
+    const double *__restrict__ fin, double *__restrict__ fout, int4 *hdrg, double *W, GridDev g, int L,
+    const unsigned long long *zflag, unsigned long long flag_target, int32_t *err, GeomArgs ga, Basis bs)
 {
     constexpr int TX = STREAM_TX, NW = STREAM_NW, NACC = STREAM_NACC;
     constexpr int STREAM_CWARPS = TX * VSPLIT, STREAM_THREADS = 32 * (STREAM_CWARPS + 1), NP = 2 / VSPLIT;
@@ -179,6 +191,21 @@ __global__ void __launch_bounds__(32 * (STREAM_TX * VSPLIT + 1), 1) xy_apply_str
         }
     }
     __syncthreads();
+    if (GEOM) {
+        static_assert(sizeof(sldg_geom::GeomShared<2, STREAM_GEOM_CELLS>) <= STREAM_RING_BYTES, "geometry scratch");
+        auto &gs = *reinterpret_cast<sldg_geom::GeomShared<2, STREAM_GEOM_CELLS> *>(smem_raw);
+        for (int c0 = 0; c0 < rows * TX; c0 += STREAM_GEOM_CELLS) {
+            auto cell_of = [&](int c) {
+                const int cc = c0 + c, jr = cc / TX, ci = cc - jr * TX;
+                return (cc < rows * TX && i0 + ci < nx) ? (j0 + jr) * nx + i0 + ci : -1;
+            };
+            sldg_geom::geometry_block<2, STREAM_GEOM_CELLS>(gs, tid, STREAM_THREADS, cell_of, z, ga.va, ga.vb, hdrg, W,
+                                                            err, g, bs, ga.tau, ga.order, ga.periodic);
+        }
+        __threadfence();  // this block's headers and weights are read back below, the weights through the async proxy
+        asm volatile("fence.proxy.async;" ::: "memory");
+        __syncthreads();
+    }
     for (int c = tid; c < rows * TX; c += STREAM_THREADS) {
         const int jr = c / TX, ci = c % TX;
         int4 h = make_int4(0, 0, 0, 0);
@@ -503,21 +530,26 @@ __global__ void __launch_bounds__(256, 2) xy_apply_direct_kernel(const double *_
 
 bool xy_apply_can_overlap(const sldg_ctx *c) { return c->g.o[0] == 2 && !getenv("SLDG_APPLY_DIRECT"); }
 
-cudaError_t launch_xy_apply(sldg_ctx *c, const double *fin, double *fout, bool wait_flags)
+cudaError_t launch_xy_apply(sldg_ctx *c, const double *fin, double *fout, bool wait_flags, bool own_geometry,
+                            double tau, int trace_order)
 {
     const GridDev &g = c->g;
     const int O = g.o[0];
     if (xy_apply_can_overlap(c)) {
         static const int vsplit = getenv("SLDG_APPLY_VSPLIT") ? atoi(getenv("SLDG_APPLY_VSPLIT")) : 1;
-        auto kern = vsplit == 1 ? xy_apply_stream_kernel<1> : xy_apply_stream_kernel<2>;
-        const int STREAM_THREADS = 32 * (STREAM_TX * (vsplit == 1 ? 1 : 2) + 1);
+        auto kern = own_geometry ? xy_apply_stream_kernel<1, true>
+                                 : (vsplit == 1 ? xy_apply_stream_kernel<1, false> : xy_apply_stream_kernel<2, false>);
+        if (own_geometry) wait_flags = false;
+        GeomArgs ga = {c->va, c->vb, tau, trace_order, c->vel_periodic};
+        const int STREAM_THREADS = 32 * (STREAM_TX * ((vsplit == 1 || own_geometry) ? 1 : 2) + 1);
         cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)STREAM_SMEM);
         const int L = g.n[1] < STREAM_LMAX ? g.n[1] : STREAM_LMAX;
         const int strips = (g.n[0] + STREAM_TX - 1) / STREAM_TX, segs = (g.n[1] + L - 1) / L;
         dim3 grid((unsigned)(strips * segs), (unsigned)((g.Pv + STREAM_VMAX - 1) / STREAM_VMAX), (unsigned)g.N[2]);
         const unsigned long long target = c->xy_epoch * (unsigned long long)xy_geometry_blocks_per_z(c);
         kern<<<grid, STREAM_THREADS, STREAM_SMEM, c->stream>>>(fin, fout, c->hdr, c->W, g, L,
-                                                               wait_flags ? c->zflag : nullptr, target, c->err);
+                                                               wait_flags ? c->zflag : nullptr, target, c->err, ga,
+                                                               c->basis);
         c->launches++;
         return cudaGetLastError();
     }

@@ -25,442 +25,11 @@
 // the target cell, unwrapped; mask over the 3x3 slots, bit dx + 3 dy) and `count` weight blocks of o^4
 // doubles, k-major (W[k*o2+m]), packed in increasing slot order at W[cell][0..count).
 #include "sldg_internal.cuh"
+#include "sldg_xy_geometry.cuh"
+
+using namespace sldg_geom;
 
 namespace {
-
-__device__ __forceinline__ int wrap_idx(int i, int n)
-{
-    int r = i % n;
-    return r < 0 ? r + n : r;
-}
-
-// min / max as one compare + select.  fmin()/fmax() cost ~8 instructions each in fp64 on sm_100a (NaN
-// handling); nothing here can be NaN.
-__device__ __forceinline__ double dmin(double a, double b) { return a < b ? a : b; }
-__device__ __forceinline__ double dmax(double a, double b) { return a > b ? a : b; }
-
-// piecewise-bilinear velocity of cell (ci,cj) at local (xi,eta)
-__device__ __forceinline__ void bilinear_vel(const double *__restrict__ a, const double *__restrict__ b,
-                                             int pitch, int ci, int cj, double xi, double eta,
-                                             double &ua, double &ub)
-{
-    const double *a0 = a + (long long)cj * pitch + ci;
-    const double *b0 = b + (long long)cj * pitch + ci;
-    const double w00 = (1.0 - xi) * (1.0 - eta), w10 = xi * (1.0 - eta), w01 = (1.0 - xi) * eta,
-                 w11 = xi * eta;
-    ua = w00 * __ldg(a0) + w10 * __ldg(a0 + 1) + w01 * __ldg(a0 + pitch) + w11 * __ldg(a0 + pitch + 1);
-    ub = w00 * __ldg(b0) + w10 * __ldg(b0 + 1) + w01 * __ldg(b0 + pitch) + w11 * __ldg(b0 + pitch + 1);
-}
-
-// foot of the characteristic through local (xi,eta) of cell (i,j), relative to that cell, cell units
-__device__ __forceinline__ void trace_point(const double *__restrict__ a, const double *__restrict__ b,
-                                            int nx, int ny, double tx, double ty, int i, int j,
-                                            double xi, double eta, int order, int periodic, double &fx,
-                                            double &fy)
-{
-    double ua, ub;
-    bilinear_vel(a, b, nx + 1, i, j, xi, eta, ua, ub);
-    if (order != 1) {
-        double mx = xi - 0.5 * tx * ua, my = eta - 0.5 * ty * ub;
-        int fi = (int)floor(mx), fj = (int)floor(my);
-        int ci, cj;
-        if (periodic) {
-            ci = wrap_idx(i + fi, nx);
-            cj = wrap_idx(j + fj, ny);
-        } else {
-            ci = min(max(i + fi, 0), nx - 1);
-            cj = min(max(j + fj, 0), ny - 1);
-            fi = ci - i;
-            fj = cj - j;
-        }
-        bilinear_vel(a, b, nx + 1, ci, cj, mx - fi, my - fj, ua, ub);
-    }
-    fx = xi - tx * ua;
-    fy = eta - ty * ub;
-}
-
-// Gauss-Jordan with partial pivoting on [V | X], fully unrolled so that everything stays in registers.
-// On exit X = V^{-1}.  Returns the smallest pivot magnitude.
-template <int N>
-__device__ __forceinline__ double gauss_jordan(double (&V)[N][N], double (&X)[N][N])
-{
-    double minpiv = 1e300;
-#pragma unroll
-    for (int c = 0; c < N; ++c) {
-        int p = c;
-        double best = fabs(V[c][c]);
-#pragma unroll
-        for (int r = c + 1; r < N; ++r) {
-            double v = fabs(V[r][c]);
-            if (v > best) {
-                best = v;
-                p = r;
-            }
-        }
-#pragma unroll
-        for (int r = c + 1; r < N; ++r) {
-            if (p == r) {
-#pragma unroll
-                for (int k = 0; k < N; ++k) {
-                    double t = V[c][k]; V[c][k] = V[r][k]; V[r][k] = t;
-                    t = X[c][k]; X[c][k] = X[r][k]; X[r][k] = t;
-                }
-            }
-        }
-        minpiv = dmin(minpiv, best);
-        const double inv = 1.0 / V[c][c];
-#pragma unroll
-        for (int k = 0; k < N; ++k) {
-            V[c][k] *= inv;
-            X[c][k] *= inv;
-        }
-#pragma unroll
-        for (int r = 0; r < N; ++r) {
-            if (r != c) {
-                const double fct = V[r][c];
-#pragma unroll
-                for (int k = 0; k < N; ++k) {
-                    V[r][k] = fma(-fct, V[c][k], V[r][k]);
-                    X[r][k] = fma(-fct, X[c][k], X[r][k]);
-                }
-            }
-        }
-    }
-    return minpiv;
-}
-
-// Per-cell description of the upstream quadrilateral's edges (corners counter-clockwise, target-cell
-// units): start point, direction and the reciprocals of the direction components (0 when the component is 0).
-struct QuadEdges {
-    double x0[4], y0[4], dx[4], dy[4], idx[4], idy[4];
-};
-
-// Monomial moments M[p][q] = int x^p y^q over (upstream quadrilateral) cap (source cell (r,s)), in that
-// cell's local coordinates, by Green's theorem.  inner_right: the grid line x_local = 1 lies inside the
-// quadrilateral's bounding box (r < r1).
-template <int O>
-__device__ __forceinline__ void piece_moments(const QuadEdges &q, double offx, double offy, bool inner_right,
-                                              const Basis &bs, double (&M)[2 * O - 1][2 * O - 1])
-{
-    constexpr int NM = 2 * O - 1;
-#pragma unroll
-    for (int p = 0; p < NM; ++p)
-#pragma unroll
-        for (int qq = 0; qq < NM; ++qq) M[p][qq] = 0.0;
-    double ylo = 1e300, yhi = -1e300;
-#pragma unroll
-    for (int e = 0; e < 4; ++e) {
-        const double x0 = q.x0[e] - offx, y0 = q.y0[e] - offy;
-        const double dx = q.dx[e], dy = q.dy[e];
-        // crossing with the line x = 1 (for the inner segment); decided from the actual end points
-        const double x1 = q.x0[(e + 1) & 3] - offx;
-        if (inner_right && dx != 0.0 && (x0 - 1.0) * (x1 - 1.0) <= 0.0) {
-            const double yc = fma(dmin(dmax((1.0 - x0) * q.idx[e], 0.0), 1.0), dy, y0);
-            ylo = dmin(ylo, yc);
-            yhi = dmax(yhi, yc);
-        }
-        // outer segment: Liang-Barsky clip of the edge against the closed unit square
-        double t0 = 0.0, t1 = 1.0;
-        bool ok = dy != 0.0;  // horizontal edges contribute nothing (dy = 0 in the line integral)
-        if (dx == 0.0) {
-            ok = ok && x0 >= 0.0 && x0 <= 1.0;
-        } else {
-            const double ta = -x0 * q.idx[e], tb = (1.0 - x0) * q.idx[e];
-            t0 = dmax(t0, dmin(ta, tb));
-            t1 = dmin(t1, dmax(ta, tb));
-        }
-        {
-            const double ta = -y0 * q.idy[e], tb = (1.0 - y0) * q.idy[e];
-            t0 = dmax(t0, dmin(ta, tb));
-            t1 = dmin(t1, dmax(ta, tb));
-        }
-        if (ok && t1 > t0) {
-            const double xa = dmin(dmax(fma(t0, dx, x0), 0.0), 1.0), ya = dmin(dmax(fma(t0, dy, y0), 0.0), 1.0);
-            const double xb = dmin(dmax(fma(t1, dx, x0), 0.0), 1.0), yb = dmin(dmax(fma(t1, dy, y0), 0.0), 1.0);
-            const double ex = xb - xa, ey = yb - ya;
-#pragma unroll
-            for (int gq = 0; gq < NM; ++gq) {  // (2o-1)-point Gauss rule: exact for degree 4o-3
-                const double t = bs.qx[gq];
-                const double x = fma(t, ex, xa), y = fma(t, ey, ya);
-                const double wgt = bs.qw[gq] * ey;
-                double xp = x;  // x^{p+1}
-#pragma unroll
-                for (int p = 0; p < NM; ++p) {
-                    double term = wgt * xp * (1.0 / (p + 1));
-#pragma unroll
-                    for (int qq = 0; qq < NM; ++qq) {
-                        M[p][qq] += term;
-                        term *= y;
-                    }
-                    xp *= x;
-                }
-            }
-        }
-    }
-    if (inner_right) {
-        const double ya = dmax(ylo, 0.0), yb = dmin(yhi, 1.0);
-        if (yb > ya) {
-            double pa = ya, pb = yb;  // y^{q+1}
-#pragma unroll
-            for (int qq = 0; qq < NM; ++qq) {
-                const double seg = (pb - pa) * (1.0 / (qq + 1));
-#pragma unroll
-                for (int p = 0; p < NM; ++p) M[p][qq] += seg * (1.0 / (p + 1));
-                pa *= ya;
-                pb *= yb;
-            }
-        }
-    }
-}
-
-// ---------------------------------------------------------------------------------------------------------
-// Two phases per block of GEOM_CELLS target cells of one z node, handing over through shared memory:
-//   phase 1, thread <-> target cell: steps 1 and 4 (corner feet, bounding box, node feet, inverse Vandermonde);
-//   phase 2, thread <-> work item = (target cell, candidate source cell of its bounding box): steps 2, 3, 5
-//            (clipped edges, moments, contraction) for ONE piece.  The items of the block are enumerated
-//            densely (prefix sum of the per-cell candidate counts), so a warp never idles on a cell with fewer
-//            candidates than its neighbours', and each phase keeps only its own state in registers.
-// The non-empty pieces of a cell are stored packed in slot order, W[cell][0 .. count); the header's mask says
-// which slots they are.
-// ---------------------------------------------------------------------------------------------------------
-template <int O>
-struct GeomShared {
-    static constexpr int O2 = O * O;
-    static constexpr int CELLS = O == 3 ? 64 : 128;
-    // structure of arrays, [field][cell]: phase 1 writes with consecutive lanes on consecutive words
-    double cx[4][CELLS], cy[4][CELLS];     // corner feet relative to the anchor cell, cell units
-    double idx[4][CELLS], idy[4][CELLS];   // reciprocals of the edge direction components (0 if the component is 0)
-    double Vi[O2 * O2][CELLS];             // inverse Vandermonde, Vi[ab * O2 + m]
-    double xc[CELLS], yc[CELLS];           // centre of the node feet
-    int r0[CELLS], s0[CELLS], nr[CELLS], ns[CELLS], mask[CELLS];
-    unsigned short item[CELLS * 11];       // work item -> cell | candidate index << 8, 0xffff = padding
-    int warp_tot[8];
-};
-
-template <int O>
-__device__ __forceinline__ int geometry_setup(const double *__restrict__ va, const double *__restrict__ vb, int32_t *err,
-                                              const GridDev &g, const Basis &bs, double tau, int order, int periodic,
-                                              int t, int z, GeomShared<O> &sh, int c)
-{
-    constexpr int O2 = O * O;
-    const int nx = g.n[0], ny = g.n[1];
-    const int i = t % nx, j = t / nx;
-    const long long vplane = (long long)(ny + 1) * (nx + 1);
-    const double *a = va + z * vplane, *b = vb + z * vplane;
-    const double tx = tau / g.h[0], ty = tau / g.h[1];
-
-    // step 1: corner feet -> upstream quadrilateral (counter-clockwise from lower-left)
-    double cx[4], cy[4];
-    trace_point(a, b, nx, ny, tx, ty, i, j, 0.0, 0.0, order, periodic, cx[0], cy[0]);
-    trace_point(a, b, nx, ny, tx, ty, i, j, 1.0, 0.0, order, periodic, cx[1], cy[1]);
-    trace_point(a, b, nx, ny, tx, ty, i, j, 1.0, 1.0, order, periodic, cx[2], cy[2]);
-    trace_point(a, b, nx, ny, tx, ty, i, j, 0.0, 1.0, order, periodic, cx[3], cy[3]);
-    const double xmin = dmin(dmin(cx[0], cx[1]), dmin(cx[2], cx[3]));
-    const double ymin = dmin(dmin(cy[0], cy[1]), dmin(cy[2], cy[3]));
-    const int r0 = (int)floor(xmin), s0 = (int)floor(ymin);
-    int nr, ns;  // the bounding box covers source cells r0 .. r0+nr, s0 .. s0+ns
-    {
-        // Corners relative to the anchor cell (keeps |coordinates| <= 4).  Everything below -- edge
-        // directions, clip parameters, crossings -- is derived from these rounded coordinates only, so
-        // that the clipped pieces of neighbouring source cells fit together exactly.
-        double qx[4], qy[4];
-#pragma unroll
-        for (int e = 0; e < 4; ++e) {
-            qx[e] = cx[e] - r0;
-            qy[e] = cy[e] - s0;
-            sh.cx[e][c] = qx[e];
-            sh.cy[e][c] = qy[e];
-        }
-        bool convex = true;
-#pragma unroll
-        for (int e = 0; e < 4; ++e) {
-            const double e1x = qx[(e + 1) & 3] - qx[e], e1y = qy[(e + 1) & 3] - qy[e];
-            const double e2x = qx[(e + 2) & 3] - qx[(e + 1) & 3], e2y = qy[(e + 2) & 3] - qy[(e + 1) & 3];
-            if (!(e1x * e2y - e1y * e2x > 0.0)) convex = false;
-            sh.idx[e][c] = e1x != 0.0 ? 1.0 / e1x : 0.0;
-            sh.idy[e][c] = e1y != 0.0 ? 1.0 / e1y : 0.0;
-        }
-        if (!convex) atomicMin(err, SLDG_EGEOM);
-        // half-open bounding box, taken from the same rounded coordinates (a foot exactly on a grid line
-        // does not add a zero-area column, R12)
-        const double xmax = dmax(dmax(qx[0], qx[1]), dmax(qx[2], qx[3]));
-        const double ymax = dmax(dmax(qy[0], qy[1]), dmax(qy[2], qy[3]));
-        nr = max((int)ceil(xmax) - 1, 0);
-        ns = max((int)ceil(ymax) - 1, 0);
-        if (nr > 2 || ns > 2) {
-            atomicMin(err, SLDG_ESTENCIL);
-            nr = min(nr, 2);
-            ns = min(ns, 2);
-        }
-    }
-    sh.r0[c] = r0;
-    sh.s0[c] = s0;
-    sh.nr[c] = nr;
-    sh.ns[c] = ns;
-    sh.mask[c] = 0;
-
-    // step 4: node feet and adjoint polynomials in centred coordinates (relative to the anchor cell)
-    double Vi[O2][O2], xc = 0.0, yc = 0.0;
-    {
-        double fx[O2], fy[O2];
-#pragma unroll
-        for (int qn = 0; qn < O; ++qn)
-#pragma unroll
-            for (int p = 0; p < O; ++p) {
-                double px, py;
-                trace_point(a, b, nx, ny, tx, ty, i, j, bs.xi[O][p], bs.xi[O][qn], order, periodic, px, py);
-                fx[p + O * qn] = px - r0;
-                fy[p + O * qn] = py - s0;
-                xc += px - r0;
-                yc += py - s0;
-            }
-        xc *= 1.0 / O2;
-        yc *= 1.0 / O2;
-        double V[O2][O2];
-#pragma unroll
-        for (int m = 0; m < O2; ++m) {
-            double py = 1.0;
-#pragma unroll
-            for (int bq = 0; bq < O; ++bq) {
-                double px = 1.0;
-#pragma unroll
-                for (int bp = 0; bp < O; ++bp) {
-                    V[m][bp + O * bq] = px * py;
-                    px *= fx[m] - xc;
-                }
-                py *= fy[m] - yc;
-            }
-#pragma unroll
-            for (int k = 0; k < O2; ++k) Vi[m][k] = (m == k) ? 1.0 : 0.0;
-        }
-        const double minpiv = gauss_jordan<O2>(V, Vi);  // phi*_m = sum_ab Vi[ab][m] (x-xc)^a (y-yc)^b
-        if (!(minpiv > 1e-10)) atomicMin(err, SLDG_EGEOM);
-    }
-    sh.xc[c] = xc;
-    sh.yc[c] = yc;
-#pragma unroll
-    for (int ab = 0; ab < O2; ++ab)
-#pragma unroll
-        for (int m = 0; m < O2; ++m) sh.Vi[ab * O2 + m][c] = Vi[ab][m];
-    return (nr + 1) * (ns + 1);
-}
-
-// steps 2, 3, 5 for one piece: target cell c of the block, candidate source cell (dr, ds) of its bounding box
-// The pieces of one target cell sit on consecutive lanes of one warp, in slot order (k = candidate index of the
-// lane): the non-empty ones are stored packed, W[cell][rank], rank from a warp ballot.  `valid` is false on padding
-// lanes, which only take part in the ballot.
-template <int O>
-__device__ __forceinline__ void geometry_piece(const GeomShared<O> &sh, bool valid, int c, int k, int dr, int ds,
-                                               const Basis &bs, double *__restrict__ Wcell, int *mask_out)
-{
-    constexpr int O2 = O * O, NM = 2 * O - 1;
-    const int lane = threadIdx.x & 31;
-    if (!valid) c = 0;
-    QuadEdges q;
-#pragma unroll
-    for (int e = 0; e < 4; ++e) {
-        q.x0[e] = sh.cx[e][c];
-        q.y0[e] = sh.cy[e][c];
-        q.idx[e] = sh.idx[e][c];
-        q.idy[e] = sh.idy[e][c];
-    }
-#pragma unroll
-    for (int e = 0; e < 4; ++e) {
-        q.dx[e] = q.x0[(e + 1) & 3] - q.x0[e];
-        q.dy[e] = q.y0[(e + 1) & 3] - q.y0[e];
-    }
-    double M[NM][NM];
-    piece_moments<O>(q, (double)dr, (double)ds, dr < sh.nr[c], bs, M);
-    const bool nonempty = valid && M[0][0] > 0.0;
-    const unsigned ballot = __ballot_sync(0xffffffffu, nonempty);
-    if (!nonempty) return;  // empty intersection
-    const int rank = __popc((ballot >> (lane - k)) & ((1u << k) - 1u));
-    // phi*_m in the source cell's monomials: (x-xc)^a = sum_a' binom(a,a') (-xc)^(a-a') x^a'
-    const double lxc = sh.xc[c] - dr, lyc = sh.yc[c] - ds;
-    double cf[O2][O2];  // cf[a'+O b'][m]
-    {
-        double sxp[O][O], syp[O][O];  // sxp[a][a'] = binom(a,a') (-lxc)^(a-a')
-#pragma unroll
-        for (int aa = 0; aa < O; ++aa)
-#pragma unroll
-            for (int ap = 0; ap < O; ++ap) {
-                const double bin = (ap > aa) ? 0.0 : ((aa == 2 && ap == 1) ? 2.0 : 1.0);
-                double px = 1.0, py = 1.0;
-#pragma unroll
-                for (int e = 0; e < O; ++e)
-                    if (e < aa - ap) {
-                        px *= -lxc;
-                        py *= -lyc;
-                    }
-                sxp[aa][ap] = bin * px;
-                syp[aa][ap] = bin * py;
-            }
-#pragma unroll
-        for (int m = 0; m < O2; ++m)
-#pragma unroll
-            for (int bp_ = 0; bp_ < O; ++bp_)
-#pragma unroll
-                for (int ap = 0; ap < O; ++ap) {
-                    double acc = 0.0;
-#pragma unroll
-                    for (int bb = bp_; bb < O; ++bb)
-#pragma unroll
-                        for (int aa = ap; aa < O; ++aa)
-                            acc = fma(sh.Vi[(aa + O * bb) * O2 + m][c], sxp[aa][ap] * syp[bb][bp_], acc);
-                    cf[ap + O * bp_][m] = acc;
-                }
-    }
-    // G[k][a'+O b'] = int phi_k x^a' y^b' = sum_{p',q'} L[kp][p'] L[kq][q'] M[p'+a'][q'+b']  (separable)
-    double T[O][O][NM];  // T[kp][a'][q] = sum_p' L[kp][p'] M[p'+a'][q]
-#pragma unroll
-    for (int kp = 0; kp < O; ++kp)
-#pragma unroll
-        for (int ap = 0; ap < O; ++ap)
-#pragma unroll
-            for (int qq = 0; qq < NM; ++qq) {
-                double acc = 0.0;
-#pragma unroll
-                for (int pp = 0; pp < O; ++pp) acc = fma(bs.L[O][kp][pp], M[pp + ap][qq], acc);
-                T[kp][ap][qq] = acc;
-            }
-    double iw[O2];
-#pragma unroll
-    for (int m = 0; m < O2; ++m) iw[m] = 1.0 / (bs.w[O][m % O] * bs.w[O][m / O]);
-    const int slot = dr + 3 * ds;
-    double *Wout = Wcell + (size_t)rank * (O2 * O2);
-#pragma unroll
-    for (int kq = 0; kq < O; ++kq)
-#pragma unroll
-        for (int kp = 0; kp < O; ++kp) {
-            double G[O2];
-#pragma unroll
-            for (int bp_ = 0; bp_ < O; ++bp_)
-#pragma unroll
-                for (int ap = 0; ap < O; ++ap) {
-                    double acc = 0.0;
-#pragma unroll
-                    for (int qq = 0; qq < O; ++qq) acc = fma(bs.L[O][kq][qq], T[kp][ap][qq + bp_], acc);
-                    G[ap + O * bp_] = acc;
-                }
-            const int k = kp + O * kq;
-            double out[O2];
-#pragma unroll
-            for (int m = 0; m < O2; ++m) {
-                double acc = 0.0;
-#pragma unroll
-                for (int ab = 0; ab < O2; ++ab) acc = fma(cf[ab][m], G[ab], acc);
-                out[m] = acc * iw[m];
-            }
-            if (O == 2) {
-                reinterpret_cast<double2 *>(Wout + k * O2)[0] = make_double2(out[0], out[1]);
-                reinterpret_cast<double2 *>(Wout + k * O2)[1] = make_double2(out[O2 - 2], out[O2 - 1]);
-            } else {
-#pragma unroll
-                for (int m = 0; m < O2; ++m) Wout[k * O2 + m] = out[m];
-            }
-        }
-    atomicOr(mask_out, 1 << slot);
-}
 
 template <int O>
 __global__ void __launch_bounds__(GeomShared<O>::CELLS) xy_geometry_kernel(const double *__restrict__ va,
@@ -470,56 +39,14 @@ __global__ void __launch_bounds__(GeomShared<O>::CELLS) xy_geometry_kernel(const
                                                                            GridDev g, Basis bs, double tau, int order,
                                                                            int periodic)
 {
-    constexpr int CELLS = GeomShared<O>::CELLS, O4 = O * O * O * O;
+    constexpr int CELLS = GeomShared<O>::CELLS;
     extern __shared__ __align__(16) unsigned char geom_smem[];
     GeomShared<O> &sh = *reinterpret_cast<GeomShared<O> *>(geom_smem);
-    const int c = threadIdx.x, lane = c & 31, warp = c >> 5;
     const int ncell = g.n[0] * g.n[1];
-    const int t = blockIdx.x * CELLS + c;
-    const int z = blockIdx.y;
-
-    // phase 1: per-cell set-up, number of candidate source cells
-    const int n = t < ncell ? geometry_setup<O>(va, vb, err, g, bs, tau, order, periodic, t, z, sh, c) : 0;
-    // Enumerate the work items: the cells of a warp in order, a cell's items on consecutive lanes of ONE warp
-    // (padded to the next multiple of 32 where they would straddle), each warp's list rounded up to 32.
-    int first = 0, pos = 0;
-#pragma unroll 1
-    for (int l = 0; l < 32; ++l) {
-        const int nl = __shfl_sync(0xffffffffu, n, l);
-        if ((pos & 31) + nl > 32) pos = (pos + 31) & ~31;
-        if (lane == l) first = pos;
-        pos += nl;
-    }
-    pos = (pos + 31) & ~31;
-    if (lane == 0) sh.warp_tot[warp] = pos;
-    __syncthreads();
-    int base = 0, total = 0;
-    for (int w = 0; w < CELLS / 32; ++w) {
-        if (w < warp) base += sh.warp_tot[w];
-        total += sh.warp_tot[w];
-    }
-    for (int it = c; it < total; it += CELLS) sh.item[it] = 0xffff;
-    __syncthreads();
-    for (int k = 0; k < n; ++k) sh.item[base + first + k] = (unsigned short)(c | (k << 8));
-    __syncthreads();
-
-    // phase 2: one piece per thread and pass (whole warps: total is a multiple of 32)
-    for (int it = c; it < total; it += CELLS) {
-        const int code = sh.item[it];
-        const bool valid = code != 0xffff;
-        const int cc = valid ? (code & 0xff) : 0, k = valid ? (code >> 8) : 0;
-        const int w = sh.nr[cc] + 1;
-        const int ds = k / w, dr = k - ds * w;
-        const long long cellid = (long long)z * ncell + blockIdx.x * CELLS + cc;
-        geometry_piece<O>(sh, valid, cc, k, dr, ds, bs, W + (size_t)cellid * 9 * O4, &sh.mask[cc]);
-    }
-    __syncthreads();
-    if (t < ncell) {
-        const int m = sh.mask[c];
-        hdr[(long long)z * ncell + t] = make_int4(sh.r0[c], sh.s0[c], m, __popc(m));
-    }
+    const int t0 = blockIdx.x * CELLS, z = blockIdx.y;
+    geometry_block<O, CELLS>(sh, threadIdx.x, CELLS, [&](int c) { return t0 + c < ncell ? t0 + c : -1; }, z, va, vb,
+                             hdr, W, err, g, bs, tau, order, periodic);
     // publish: all writes of this block, then one release increment of the z node's counter
-    __syncthreads();
     if (threadIdx.x == 0) {
         __threadfence();
         atomicAdd(zflag + z, 1ull);

@@ -378,6 +378,27 @@ def test_fused_sweep_pairs_are_bit_identical_to_separate_sweeps(torch, monkeypat
     assert np.array_equal(outs[0], outs[1])
 
 
+def test_mass_drift_over_200_strang_steps(torch):
+    """BASELINE.json configs[3] runs 200 Strang steps and records the mass drift every step: it must stay below
+    1e-13 relative over the whole run.  (Before the conservation correction of the 1d overlap matrices -- see
+    eval_shift -- every sweep lost 1.5e-16 with a fixed sign and 200 steps ended at 1.5e-13.)"""
+    spec = inputs.itg_grid(64, 64, 4, 16, 2)  # configs[3]'s resolution in (x, y), fewer z and v cells
+    dt = 4.0
+    a, b, Ez, _ = inputs.itg_fields(spec, dt, 0.8)
+    s = _sldg(spec)
+    s.import_state(_dev(torch, inputs.itg_initial_f(spec)))
+    s.set_Ez(_dev(torch, Ez))
+    s.set_vxy(_dev(torch, a), _dev(torch, b), 1)
+    m0 = float(s.mass().cpu()[0])
+    worst = 0.0
+    for n in range(200):
+        s.strang_step(dt)
+        if n % 10 == 9:
+            worst = max(worst, abs(float(s.mass().cpu()[0]) - m0) / abs(m0))
+    s.check()
+    assert worst <= 1e-13, worst
+
+
 def test_layouts_agree_bitwise_on_a_strang_step(torch):
     spec = inputs.itg_grid(8, 8, 4, 8, 2)
     f = inputs.itg_initial_f(spec)
