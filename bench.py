@@ -329,7 +329,6 @@ def run_ours(args):
         "advect_z_gbs": gbs(2 * nbytes, sm["z"]), "advect_v_gbs": gbs(2 * nbytes, sm["v"]),
         "advect_xy_gbs": gbs(2 * nbytes, sm["xy"]),
         "ms_single_calls": sm,
-        "xy_geometry_overlapped_with_apply": bool(int(med[6]) & 1),
         "charge_density_gbs": gbs(nbytes, rho_ms),
         "xy_apply_direct_path_blocks_total": s.debug_counter(0),
         "strang_step_fused_sweep_pairs": {"zv": fused_zv, "vz": fused_vz},

@@ -22,8 +22,7 @@
  *   state           the library keeps f in an INTERNAL layout (v fastest) inside f_a/f_b and
  *                   ping-pongs between them; sldg_import_state / sldg_export_state convert.
  *   stream          every call enqueues on the cudaStream_t given at sldg_create and returns without
- *                   synchronising, unless stated otherwise.  (Inside sldg_advect_xy the geometry kernel runs on
- *                   an internal stream that forks from and joins that stream; invisible to the caller.)
+ *                   synchronising, unless stated otherwise.
  *   errors          return value 0 = success, negative = SLDG_E* below.  Errors detected on the device
  *                   (geometry) are sticky and reported by sldg_check.  There is no CPU fallback: without
  *                   a CUDA device every compute call returns SLDG_ECUDA.
@@ -127,9 +126,8 @@ int sldg_strang_step_host(sldg_ctx *ctx, double dt, const double *Ez_host, const
 int sldg_check(sldg_ctx *ctx);
 /* Device times (CUDA events) of the last sldg_strang_step, in ms:
  * ms[0] z  ms[1] v  ms[3] the WHOLE xy substep (geometry + apply, first launch to last)  ms[4] v  ms[5] z
- * ms[7] total -- all on the context's stream; ms[2] = duration of the geometry kernel alone on the library's
- * internal stream (it is part of ms[3], not in addition to it); ms[6] = flags: +1 if that kernel ran concurrently
- * with the apply, +2 if the first pair of adjacent sweeps (z,v before the 2d step) ran fused in one pass over f
+ * ms[7] total; ms[2] = duration of the geometry kernel alone (it is part of ms[3], not in addition to it);
+ * ms[6] = flags: +2 if the first pair of adjacent sweeps (z,v before the 2d step) ran fused in one pass over f
  * -- then ms[0] holds the time of the pair and ms[1] = 0 --, +4 if the second pair (v,z after it) did -- then
  * ms[4] holds the time of the pair and ms[5] = 0.
  * After a single sldg_advect_* call only that entry (and ms[7]) is set.  Synchronises. */
@@ -143,8 +141,9 @@ long long sldg_launch_count(sldg_ctx *ctx);
  * entries of empty slots are unspecified).  Device buffers; asynchronous. */
 int sldg_debug_geometry(sldg_ctx *ctx, int z, int32_t *anchor_dev, int32_t *mask_dev, double *W_dev);
 /* Diagnostic counter `which` since creation, into *value_host; synchronises the stream.
- *   0: blocks of the 2d apply kernel that could not use the staged (shared-memory ring) path and fell back to
- *      direct global loads (windows too wide for the ring, more than 3 source rows per target row). */
+ *   0: blocks (strip x segment x z node) of the 2d apply whose source window does not fit the streaming kernel's
+ *      shared-memory ring (anchors varying by many cells inside the block, more than 3 source rows per target
+ *      row) and were handed to the direct kernel instead. */
 int sldg_debug_counter(sldg_ctx *ctx, int which, long long *value_host);
 const char *sldg_strerror(int code);
 

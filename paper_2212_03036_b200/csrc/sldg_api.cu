@@ -51,7 +51,7 @@ void fill_grid(const sldg_params *p, GridDev *g)
 }
 
 struct WorkspaceMap {
-    size_t Ez, va, vb, hdr, W, partials, rho, scalar, err, zflag, total;
+    size_t Ez, va, vb, hdr, W, partials, rho, scalar, err, stage_ok, total;
     size_t n_partials;
 };
 
@@ -75,7 +75,7 @@ WorkspaceMap map_workspace(const sldg_params *p)
     m.rho = take((size_t)g.lines * 8);
     m.scalar = take(256);
     m.err = take(256);
-    m.zflag = take(Nz * 8);
+    m.stage_ok = take(xy_apply_stage_flags(p) * 4);
     m.total = off;
     return m;
 }
@@ -269,11 +269,8 @@ int sldg_create(const sldg_params *p, double *f_a_dev, double *f_b_dev, void *wo
     c->rho_ws = (double *)(ws + m.rho);
     c->scalar_ws = (double *)(ws + m.scalar);
     c->err = (int32_t *)(ws + m.err);
-    c->zflag = (unsigned long long *)(ws + m.zflag);
-    c->xy_epoch = 0;
-    c->overlap = getenv("SLDG_XY_OVERLAP") ? 1 : 0;  // experimental: co-running the two kernels is slower today
+    c->stage_ok = (int32_t *)(ws + m.stage_ok);
     c->fuse = getenv("SLDG_NO_FUSE") ? 0 : 1;
-    c->own_geometry = getenv("SLDG_XY_OWN_GEOMETRY") ? 1 : 0;
     c->trace_order = 2;
     c->vel_periodic = 0;
     if (cudaDeviceGetAttribute(&c->sm_count, cudaDevAttrMultiProcessorCount, dev) != cudaSuccess) {
@@ -285,21 +282,14 @@ int sldg_create(const sldg_params *p, double *f_a_dev, double *f_b_dev, void *wo
             sldg_destroy(c);
             return SLDG_ECUDA;
         }
-    {
-        // the geometry kernel runs on an internal stream of the highest priority, concurrently with the apply
-        int lo_pri = 0, hi_pri = 0;
-        cudaDeviceGetStreamPriorityRange(&lo_pri, &hi_pri);
-        bool ok = cudaStreamCreateWithPriority(&c->gstream, cudaStreamNonBlocking, hi_pri) == cudaSuccess;
-        for (int k = 0; k < 4 && ok; ++k) ok = cudaEventCreate(&c->gev[k]) == cudaSuccess;
-        if (!ok) {
+    for (int k = 0; k < 2; ++k)
+        if (cudaEventCreate(&c->gev[k]) != cudaSuccess) {
             sldg_destroy(c);
             return SLDG_ECUDA;
         }
-    }
     // fields default to zero, error word cleared
     cudaError_t e = cudaMemsetAsync(ws + m.Ez, 0, m.hdr - m.Ez, c->stream);
     if (e == cudaSuccess) e = cudaMemsetAsync(c->err, 0, 256, c->stream);
-    if (e == cudaSuccess) e = cudaMemsetAsync(c->zflag, 0, (size_t)c->g.N[2] * 8, c->stream);
     if (e != cudaSuccess) {
         sldg_destroy(c);
         return SLDG_ECUDA;
@@ -311,12 +301,10 @@ int sldg_create(const sldg_params *p, double *f_a_dev, double *f_b_dev, void *wo
 int sldg_destroy(sldg_ctx *c)
 {
     if (!c) return SLDG_EINVAL;
-    if (c->gstream) cudaStreamSynchronize(c->gstream);
     for (int k = 0; k < 8; ++k)
         if (c->ev[k]) cudaEventDestroy(c->ev[k]);
-    for (int k = 0; k < 4; ++k)
+    for (int k = 0; k < 2; ++k)
         if (c->gev[k]) cudaEventDestroy(c->gev[k]);
-    if (c->gstream) cudaStreamDestroy(c->gstream);
     delete c;
     return SLDG_OK;
 }
@@ -418,43 +406,15 @@ static int do_pair(sldg_ctx *c, double tau, bool z_first, cudaEvent_t mid, int *
     return z_first ? do_v(c, tau) : do_z(c, tau);
 }
 
-// The geometry (once per z node) and the apply (every v) of one 2d step.  The geometry runs on the
-// internal stream: it starts when everything enqueued before this call has finished (fields set, previous
-// apply done with the weights) and publishes one counter per z node; the apply, on the caller's stream, starts
-// at the same time and each of its blocks waits for its z node's counter -- the ALU-bound geometry is hidden
-// under the bandwidth-bound apply.  Without overlap (o != 2, SLDG_NO_OVERLAP) the apply waits for the whole
-// geometry kernel.
+// The geometry (once per z node) and the apply (every v) of one 2d step, back to back on the
+// caller's stream.  (Running the ALU-bound geometry concurrently with the bandwidth-bound apply -- on a second
+// stream with per-z counters, or as a prologue of every apply block -- was built and measured slower: DESIGN.md 6.3.)
 static int do_xy(sldg_ctx *c, double tau, int trace_order)
 {
-    if (c->own_geometry && xy_apply_can_overlap(c)) {
-        // one kernel: every apply block computes the geometry of its own strip first
-        cudaEventRecord(c->gev[1], c->stream);
-        cudaEventRecord(c->gev[2], c->stream);
-        if (launch_xy_apply(c, c->f[c->cur], c->f[c->cur ^ 1], false, true, tau, trace_order) != cudaSuccess)
-            return SLDG_ECUDA;
-        swap_state(c);
-        return SLDG_OK;
-    }
-    const bool overlap = c->overlap && xy_apply_can_overlap(c);
-    c->xy_epoch++;
-    if (!overlap) {
-        // back to back on the caller's stream
-        cudaEventRecord(c->gev[1], c->stream);
-        if (launch_xy_geometry(c, c->stream, tau, trace_order) != cudaSuccess) return SLDG_ECUDA;
-        cudaEventRecord(c->gev[2], c->stream);
-        if (launch_xy_apply(c, c->f[c->cur], c->f[c->cur ^ 1], false, false, tau, trace_order) != cudaSuccess)
-            return SLDG_ECUDA;
-        swap_state(c);
-        return SLDG_OK;
-    }
     cudaEventRecord(c->gev[0], c->stream);
-    cudaStreamWaitEvent(c->gstream, c->gev[0], 0);
-    cudaEventRecord(c->gev[1], c->gstream);
-    if (launch_xy_geometry(c, c->gstream, tau, trace_order) != cudaSuccess) return SLDG_ECUDA;
-    cudaEventRecord(c->gev[2], c->gstream);
-    if (launch_xy_apply(c, c->f[c->cur], c->f[c->cur ^ 1], true, false, tau, trace_order) != cudaSuccess)
-        return SLDG_ECUDA;
-    cudaStreamWaitEvent(c->stream, c->gev[2], 0);  // join (the geometry has long finished)
+    if (launch_xy_geometry(c, tau, trace_order) != cudaSuccess) return SLDG_ECUDA;
+    cudaEventRecord(c->gev[1], c->stream);
+    if (launch_xy_apply(c, c->f[c->cur], c->f[c->cur ^ 1]) != cudaSuccess) return SLDG_ECUDA;
     swap_state(c);
     return SLDG_OK;
 }
@@ -575,14 +535,14 @@ int sldg_last_timing_ms(sldg_ctx *c, float ms[8])
     };
     auto geom = [&]() {
         float t = 0.0f;
-        cudaEventSynchronize(c->gev[2]);
-        cudaEventElapsedTime(&t, c->gev[1], c->gev[2]);
+        cudaEventSynchronize(c->gev[1]);
+        cudaEventElapsedTime(&t, c->gev[0], c->gev[1]);
         return t;
     };
     if (c->ev_kind == 1) {
         ms[0] = el(0, 1); ms[1] = el(1, 2); ms[3] = el(2, 3); ms[4] = el(3, 4); ms[5] = el(4, 5);
         ms[2] = geom();
-        ms[6] = ((c->overlap && xy_apply_can_overlap(c)) ? 1.0f : 0.0f) + (float)c->last_fused;
+        ms[6] = (float)c->last_fused;
         ms[7] = el(0, 5);
     } else if (c->ev_kind == 2) {
         ms[0] = ms[7] = el(0, 1);
@@ -591,7 +551,6 @@ int sldg_last_timing_ms(sldg_ctx *c, float ms[8])
     } else if (c->ev_kind == 4) {
         ms[2] = geom();
         ms[3] = ms[7] = el(0, 1);
-        ms[6] = (c->overlap && xy_apply_can_overlap(c)) ? 1.0f : 0.0f;
     }
     return SLDG_OK;
 }

@@ -57,13 +57,9 @@ struct sldg_ctx {
     double *rho_ws;         // [Nz][Ny][Nx] scratch charge density (mass, host entry point)
     double *scalar_ws;      // one double
     int32_t *err;           // sticky device error word
-    unsigned long long *zflag;  // [Nz] geometry blocks finished per z node (monotone over the xy steps)
-    unsigned long long xy_epoch;
-    cudaStream_t gstream;   // internal high-priority stream: the geometry kernel runs here, under the apply
-    cudaEvent_t gev[4];     // xy start (main), geometry start/end (gstream), previous apply done (main)
+    int32_t *stage_ok;      // [Nz][strips*segments] 1: that block of the streaming 2d apply can stage its rows
+    cudaEvent_t gev[2];     // start / end of the geometry kernel of the last 2d step
     int fuse, last_fused;   // fuse: sldg_strang_step runs each pair of adjacent sweeps in one pass
-    int own_geometry;       // 1: the o = 2 apply kernel computes the geometry of its strips itself
-    int overlap;            // 1: geometry and apply of one xy step run concurrently (o = 2 path)
     size_t n_partials;
     int trace_order, vel_periodic;
     cudaEvent_t ev[8];
@@ -80,10 +76,8 @@ cudaError_t launch_advect_v(sldg_ctx *c, const double *fin, double *fout, double
 cudaError_t launch_charge_density(sldg_ctx *c, const double *fin, double *rho);
 cudaError_t launch_mass(sldg_ctx *c, const double *fin, double *mass_out);
 cudaError_t launch_mass_from_rho(sldg_ctx *c, const double *rho, double *mass_out);
-cudaError_t launch_xy_geometry(sldg_ctx *c, cudaStream_t stream, double tau, int trace_order);
-int xy_geometry_blocks_per_z(const sldg_ctx *c);
-bool xy_apply_can_overlap(const sldg_ctx *c);
+cudaError_t launch_xy_geometry(sldg_ctx *c, double tau, int trace_order);
+size_t xy_apply_stage_flags(const sldg_params *p);  // number of stage_ok entries
 cudaError_t launch_geometry_expand(sldg_ctx *c, int z, int32_t *anchor, int32_t *mask, double *Wd);
-cudaError_t launch_xy_apply(sldg_ctx *c, const double *fin, double *fout, bool wait_flags, bool own_geometry,
-                            double tau, int trace_order);
+cudaError_t launch_xy_apply(sldg_ctx *c, const double *fin, double *fout);
 cudaError_t launch_fused_sweeps(sldg_ctx *c, const double *fin, double *fout, double tau_z, double tau_v, bool z_first);

@@ -95,24 +95,6 @@ __device__ __forceinline__ void fma_block_o2(double (&acc)[4][2 * NP], const dou
     }
 }
 
-// the same for two v values per lane, operands from global memory (fallback path)
-__device__ __forceinline__ void fma_block_o2_direct(double (&acc)[4][2], const double2 (&in)[4], const double *Wp)
-{
-#pragma unroll
-    for (int k = 0; k < 4; ++k) {
-        const double2 w01 = __ldcg(reinterpret_cast<const double2 *>(Wp + k * 4));
-        const double2 w23 = __ldcg(reinterpret_cast<const double2 *>(Wp + k * 4 + 2));
-        acc[0][0] = fma(w01.x, in[k].x, acc[0][0]);
-        acc[0][1] = fma(w01.x, in[k].y, acc[0][1]);
-        acc[1][0] = fma(w01.y, in[k].x, acc[1][0]);
-        acc[1][1] = fma(w01.y, in[k].y, acc[1][1]);
-        acc[2][0] = fma(w23.x, in[k].x, acc[2][0]);
-        acc[2][1] = fma(w23.x, in[k].y, acc[2][1]);
-        acc[3][0] = fma(w23.y, in[k].x, acc[3][0]);
-        acc[3][1] = fma(w23.y, in[k].y, acc[3][1]);
-    }
-}
-
 constexpr int STREAM_TX = 8;        // target cells per strip
 constexpr int STREAM_LMAX = 128;    // target rows per segment
 constexpr int STREAM_VMAX = 128;    // v values per chunk
@@ -126,25 +108,57 @@ constexpr size_t STREAM_RING_BYTES = 160 * 1024;
 constexpr size_t STREAM_WRING_BYTES = (size_t)STREAM_NW * STREAM_WROW * 128;
 constexpr size_t STREAM_HDR_BYTES = (size_t)STREAM_LMAX * STREAM_TX * 16;
 constexpr size_t STREAM_SMEM = STREAM_RING_BYTES + STREAM_WRING_BYTES + STREAM_HDR_BYTES + 512;
-constexpr long long STREAM_SPIN_LIMIT = 4000000000ll;  // cycles (~2 s): a stuck flag becomes an error, not a hang
 
-// Arguments of the geometry when the apply kernel computes it itself (GEOM): the fields and the step.
-struct GeomArgs {
-    const double *va, *vb;
-    double tau;
-    int order, periodic;
-};
-constexpr int STREAM_GEOM_CELLS = 256;  // target cells per geometry pass of a block (scratch: the idle input ring)
-
-// GEOM: every block first computes the geometry of its own strip (sldg_xy_geometry.cuh; headers and weights go to
-// global memory as in the stand-alone kernel and are read back through L2), then streams.  The geometry is
-// compute only, the streaming is bandwidth only: with the blocks of the grid out of step with one another the
-// one hides under the other, and the weights never wait in HBM for a second kernel.
-template <int VSPLIT, bool GEOM>
-__global__ void __launch_bounds__(32 * (STREAM_TX * VSPLIT + 1), 1) xy_apply_stream_kernel(
-    const double *__restrict__ fin, double *__restrict__ fout, int4 *hdrg, double *W, GridDev g, int L,
-    const unsigned long long *zflag, unsigned long long flag_target, int32_t *err, GeomArgs ga, Basis bs)
+// Whether the block (strip, segment, z node) of the streaming kernel can stage its rows: the x window of the
+// strip over the whole segment must leave at least two ring slots, and a target row may use at most NACC source rows.
+// One criterion, evaluated by the scan kernel below and relied upon by the streaming kernel.
+__device__ __forceinline__ bool stream_block_stageable(int axmin, int axmax, int aymin, int aymax, int VL)
 {
+    const int RW = STREAM_TX + axmax - axmin;
+    const size_t stage_bytes = (size_t)2 * 2 * RW * VL * 8;
+    return STREAM_RING_BYTES / stage_bytes >= 2 && aymax - aymin + 1 <= STREAM_NACC;
+}
+
+// grid (strips * segments, Nz): bounds of the anchors of one streaming block -> stage_ok[z][block]
+__global__ void __launch_bounds__(128) xy_stageable_kernel(const int4 *__restrict__ hdrg, GridDev g, int L, int VL,
+                                                           int32_t *__restrict__ stage_ok, int32_t *err)
+{
+    constexpr int TX = STREAM_TX;
+    __shared__ int bnd[4];
+    const int nx = g.n[0], ny = g.n[1];
+    const int strips = (nx + TX - 1) / TX;
+    const int strip = blockIdx.x % strips, seg = blockIdx.x / strips;
+    const int i0 = strip * TX, j0 = seg * L;
+    const int rows = min(L, ny - j0);
+    const long long zc = (long long)blockIdx.y * nx * ny;
+    if (threadIdx.x == 0) { bnd[0] = 1 << 30; bnd[1] = -(1 << 30); bnd[2] = 1 << 30; bnd[3] = -(1 << 30); }
+    __syncthreads();
+    int lo_x = 1 << 30, hi_x = -(1 << 30), lo_y = 1 << 30, hi_y = -(1 << 30);
+    for (int c = threadIdx.x; c < rows * TX; c += blockDim.x) {
+        const int jr = c / TX, ci = c - jr * TX;
+        if (i0 + ci >= nx) continue;
+        const int4 h = __ldcg(hdrg + zc + (long long)(j0 + jr) * nx + i0 + ci);
+        if (!h.z) continue;
+        const int wx = (h.z & 0x124) ? 3 : ((h.z & 0x092) ? 2 : 1);
+        const int wy = (h.z & 0x1c0) ? 3 : ((h.z & 0x038) ? 2 : 1);
+        lo_x = min(lo_x, h.x); hi_x = max(hi_x, h.x + wx - 1);
+        lo_y = min(lo_y, h.y); hi_y = max(hi_y, h.y + wy - 1);
+    }
+    atomicMin(&bnd[0], lo_x); atomicMax(&bnd[1], hi_x); atomicMin(&bnd[2], lo_y); atomicMax(&bnd[3], hi_y);
+    __syncthreads();
+    if (threadIdx.x == 0) {
+        const bool ok = bnd[1] < bnd[0] || stream_block_stageable(bnd[0], bnd[1], bnd[2], bnd[3], VL);
+        stage_ok[blockIdx.y * gridDim.x + blockIdx.x] = ok ? 1 : 0;
+        if (!ok) atomicAdd(err + 1, 1);  // diagnostic counter 0 (sldg_debug_counter)
+    }
+}
+
+template <int VSPLIT>
+__global__ void __launch_bounds__(32 * (STREAM_TX * VSPLIT + 1), 1) xy_apply_stream_kernel(
+    const double *__restrict__ fin, double *__restrict__ fout, const int4 *__restrict__ hdrg,
+    const double *__restrict__ W, GridDev g, int L, const int32_t *__restrict__ stage_ok)
+{
+    if (!stage_ok[blockIdx.z * gridDim.x + blockIdx.x]) return;  // the direct kernel handles this block
     constexpr int TX = STREAM_TX, NW = STREAM_NW, NACC = STREAM_NACC;
     constexpr int STREAM_CWARPS = TX * VSPLIT, STREAM_THREADS = 32 * (STREAM_CWARPS + 1), NP = 2 / VSPLIT;
     extern __shared__ __align__(128) unsigned char smem_raw[];
@@ -173,39 +187,8 @@ __global__ void __launch_bounds__(32 * (STREAM_TX * VSPLIT + 1), 1) xy_apply_str
         for (int s = 0; s < STREAM_NRMAX; ++s) { mbar_init(&full[s], 1); mbar_init(&empty[s], STREAM_CWARPS); }
         for (int s = 0; s < NW; ++s) { mbar_init(&wfull[s], 1); mbar_init(&wempty[s], STREAM_CWARPS); }
         mbar_fence_init();
-        if (zflag) {
-            // the geometry kernel of this step runs concurrently on another stream: wait until every one of its
-            // blocks of this z node has published (acquire), bounded so that a lost flag cannot hang the GPU
-            const long long t0 = clock64();
-            unsigned long long seen;
-            for (;;) {
-                asm volatile("ld.acquire.gpu.global.u64 %0, [%1];" : "=l"(seen) : "l"(zflag + z) : "memory");
-                if (seen >= flag_target) break;
-                if (clock64() - t0 > STREAM_SPIN_LIMIT) {
-                    atomicMin(err, SLDG_ECUDA);
-                    break;
-                }
-                __nanosleep(256);
-            }
-            asm volatile("fence.proxy.async;" ::: "memory");  // the weights are then read through the async proxy
-        }
     }
     __syncthreads();
-    if (GEOM) {
-        static_assert(sizeof(sldg_geom::GeomShared<2, STREAM_GEOM_CELLS>) <= STREAM_RING_BYTES, "geometry scratch");
-        auto &gs = *reinterpret_cast<sldg_geom::GeomShared<2, STREAM_GEOM_CELLS> *>(smem_raw);
-        for (int c0 = 0; c0 < rows * TX; c0 += STREAM_GEOM_CELLS) {
-            auto cell_of = [&](int c) {
-                const int cc = c0 + c, jr = cc / TX, ci = cc - jr * TX;
-                return (cc < rows * TX && i0 + ci < nx) ? (j0 + jr) * nx + i0 + ci : -1;
-            };
-            sldg_geom::geometry_block<2, STREAM_GEOM_CELLS>(gs, tid, STREAM_THREADS, cell_of, z, ga.va, ga.vb, hdrg, W,
-                                                            err, g, bs, ga.tau, ga.order, ga.periodic);
-        }
-        __threadfence();  // this block's headers and weights are read back below, the weights through the async proxy
-        asm volatile("fence.proxy.async;" ::: "memory");
-        __syncthreads();
-    }
     for (int c = tid; c < rows * TX; c += STREAM_THREADS) {
         const int jr = c / TX, ci = c % TX;
         int4 h = make_int4(0, 0, 0, 0);
@@ -240,45 +223,8 @@ __global__ void __launch_bounds__(32 * (STREAM_TX * VSPLIT + 1), 1) xy_apply_str
     const size_t stage_doubles = (size_t)2 * 2 * RW * VL;
     int NR = (int)(STREAM_RING_BYTES / (stage_doubles * 8));
     NR = NR > STREAM_NRMAX ? STREAM_NRMAX : NR;
-    const bool staged = NR >= 2 && S <= NACC && bnd[4] <= STREAM_WROW;
     const double *fz = fin + z * g.sZ + v0;
     double *oz = fout + z * g.sZ + v0;
-
-    if (!staged) {
-        // direct path: warp <-> cell, 64 v values per pass
-        if (tid == 0) atomicAdd(err + 1, 1);  // diagnostic counter 0 (sldg_debug_counter)
-        for (int c = warp; c < rows * TX; c += STREAM_THREADS / 32) {
-            const int jr = c / TX, ci = c % TX;
-            const int4 h = hdr[c];
-            if (i0 + ci >= nx || !h.z) continue;
-            const int i = i0 + ci, j = j0 + jr;
-            const long long cellid = zc + (long long)j * nx + i;
-            const int gx = wrap_idx(i + h.x, nx), gy = wrap_idx(j + h.y, ny);
-            for (int v = 2 * lane; v < VL; v += 64) {
-                double acc[4][2] = {};
-                int nb = 0;
-#pragma unroll 1
-                for (int slot = 0; slot < 9; ++slot) {
-                    if (!((h.z >> slot) & 1)) continue;
-                    int r = gx + slot % 3, s = gy + slot / 3;
-                    if (r >= nx) r -= nx;
-                    if (s >= ny) s -= ny;
-                    double2 in[4];
-#pragma unroll
-                    for (int k = 0; k < 4; ++k)
-                        in[k] = __ldg(reinterpret_cast<const double2 *>(
-                            fz + (long long)(2 * s + (k >> 1)) * g.sY + (long long)(2 * r + (k & 1)) * g.sX + v));
-                    fma_block_o2_direct(acc, in, W + ((size_t)cellid * 9 + nb++) * 16);
-                }
-#pragma unroll
-                for (int m = 0; m < 4; ++m)
-                    *reinterpret_cast<double2 *>(oz + (long long)(2 * j + (m >> 1)) * g.sY +
-                                                 (long long)(2 * i + (m & 1)) * g.sX + v) =
-                        make_double2(acc[m][0], acc[m][1]);
-            }
-        }
-        return;
-    }
 
     // Headers -> per-target-row descriptors, in place.  A target row jr is touched by the source rows
     // jr + d, d = 0..2 (relative to aymin); descriptor d = {bits 0-2: mask of the 3 source cells of that row,
@@ -456,17 +402,24 @@ __global__ void __launch_bounds__(32 * (STREAM_TX * VSPLIT + 1), 1) xy_apply_str
 // contiguous in m) each feeding NV FMAs -- o^2 NV accumulators per lane, o^2 + NV loads per o^2 NV FMAs.
 // Inputs and weights through L1/L2.  At o = 3 the step is bound by the fp64 pipe (2*9*c FMA per DOF).
 // --------------------------------------------------------------------------------------------------
+// stage_ok != nullptr: only the tiles whose streaming block (strip = the tile's 8 columns, segment of L rows, z
+// node) is NOT stageable are done here (the streaming kernel does the others).
 template <int O, int NV>
 __global__ void __launch_bounds__(256, 2) xy_apply_direct_kernel(const double *__restrict__ fin,
                                                               double *__restrict__ fout,
                                                               const int4 *__restrict__ hdrg,
-                                                              const double *__restrict__ W, GridDev g)
+                                                              const double *__restrict__ W, GridDev g,
+                                                              const int32_t *__restrict__ stage_ok, int L)
 {
     constexpr int O2 = O * O, TX = 8, TY = 4;
     const int nx = g.n[0], ny = g.n[1];
     const int tiles_x = (nx + TX - 1) / TX;
     const int tile_i = (blockIdx.x % tiles_x) * TX, tile_j = (blockIdx.x / tiles_x) * TY;
     const int z = blockIdx.z;
+    if (stage_ok) {
+        const int segs = (ny + L - 1) / L;
+        if (stage_ok[(z * segs + tile_j / L) * tiles_x + tile_i / TX]) return;
+    }
     const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
     const int v = blockIdx.y * 32 * NV + lane;
     if (v >= g.Pv) return;
@@ -528,44 +481,55 @@ __global__ void __launch_bounds__(256, 2) xy_apply_direct_kernel(const double *_
     }
 }
 
-bool xy_apply_can_overlap(const sldg_ctx *c) { return c->g.o[0] == 2 && !getenv("SLDG_APPLY_DIRECT"); }
+static bool xy_apply_streams(const GridDev &g) { return g.o[0] == 2 && !getenv("SLDG_APPLY_DIRECT"); }
+static int stream_segment_rows(int ny) { return ny < STREAM_LMAX ? ny : STREAM_LMAX; }
 
-cudaError_t launch_xy_apply(sldg_ctx *c, const double *fin, double *fout, bool wait_flags, bool own_geometry,
-                            double tau, int trace_order)
+size_t xy_apply_stage_flags(const sldg_params *p)
+{
+    const int L = stream_segment_rows(p->n[1]);
+    const size_t strips = (p->n[0] + STREAM_TX - 1) / STREAM_TX, segs = (p->n[1] + L - 1) / L;
+    return strips * segs * (size_t)p->n[2] * p->order[2];
+}
+
+cudaError_t launch_xy_apply(sldg_ctx *c, const double *fin, double *fout)
 {
     const GridDev &g = c->g;
     const int O = g.o[0];
-    if (xy_apply_can_overlap(c)) {
-        static const int vsplit = getenv("SLDG_APPLY_VSPLIT") ? atoi(getenv("SLDG_APPLY_VSPLIT")) : 1;
-        auto kern = own_geometry ? xy_apply_stream_kernel<1, true>
-                                 : (vsplit == 1 ? xy_apply_stream_kernel<1, false> : xy_apply_stream_kernel<2, false>);
-        if (own_geometry) wait_flags = false;
-        GeomArgs ga = {c->va, c->vb, tau, trace_order, c->vel_periodic};
-        const int STREAM_THREADS = 32 * (STREAM_TX * ((vsplit == 1 || own_geometry) ? 1 : 2) + 1);
-        cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)STREAM_SMEM);
-        const int L = g.n[1] < STREAM_LMAX ? g.n[1] : STREAM_LMAX;
-        const int strips = (g.n[0] + STREAM_TX - 1) / STREAM_TX, segs = (g.n[1] + L - 1) / L;
-        dim3 grid((unsigned)(strips * segs), (unsigned)((g.Pv + STREAM_VMAX - 1) / STREAM_VMAX), (unsigned)g.N[2]);
-        const unsigned long long target = c->xy_epoch * (unsigned long long)xy_geometry_blocks_per_z(c);
-        kern<<<grid, STREAM_THREADS, STREAM_SMEM, c->stream>>>(fin, fout, c->hdr, c->W, g, L,
-                                                               wait_flags ? c->zflag : nullptr, target, c->err, ga,
-                                                               c->basis);
-        c->launches++;
-        return cudaGetLastError();
-    }
     const int tiles = ((g.n[0] + 7) / 8) * ((g.n[1] + 3) / 4);
-    // values per lane: as many as cover the line in one chunk, at most 5 (45 accumulators at o = 3)
+    // direct kernel, values per lane: as many as cover the line in one chunk, at most 5 (45 accumulators at o = 3)
     int nv = (g.Pv + 31) / 32;
     if (nv > 5) nv = 4;
     const int vchunks = (g.Pv + 32 * nv - 1) / (32 * nv);
-    dim3 grid((unsigned)tiles, (unsigned)vchunks, (unsigned)g.N[2]);
+    dim3 dgrid((unsigned)tiles, (unsigned)vchunks, (unsigned)g.N[2]);
+    const int32_t *flags = nullptr;
+    int L = 0;
 #define LAUNCH_A(OO, NN) \
-    xy_apply_direct_kernel<OO, NN><<<grid, 256, 0, c->stream>>>(fin, fout, c->hdr, c->W, g)
+    xy_apply_direct_kernel<OO, NN><<<dgrid, 256, 0, c->stream>>>(fin, fout, c->hdr, c->W, g, flags, L)
 #define LAUNCH_AN(OO)                                                                                         \
     do {                                                                                                      \
         if (nv == 1) LAUNCH_A(OO, 1); else if (nv == 2) LAUNCH_A(OO, 2); else if (nv == 3) LAUNCH_A(OO, 3);   \
         else if (nv == 4) LAUNCH_A(OO, 4); else LAUNCH_A(OO, 5);                                              \
     } while (0)
+    if (xy_apply_streams(g)) {
+        // o = 2: which blocks can stream is decided on the device (scan of the headers); the streaming kernel does
+        // those, the direct kernel the others (none in an ITG step; most of them in a solid-body rotation, where the
+        // anchors change by many cells along a strip).  No host synchronisation.
+        static const int vsplit = getenv("SLDG_APPLY_VSPLIT") ? atoi(getenv("SLDG_APPLY_VSPLIT")) : 1;
+        auto kern = vsplit == 1 ? xy_apply_stream_kernel<1> : xy_apply_stream_kernel<2>;
+        const int STREAM_THREADS = 32 * (STREAM_TX * (vsplit == 1 ? 1 : 2) + 1);
+        cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)STREAM_SMEM);
+        L = stream_segment_rows(g.n[1]);
+        const int strips = (g.n[0] + STREAM_TX - 1) / STREAM_TX, segs = (g.n[1] + L - 1) / L;
+        const int VL = g.Pv < STREAM_VMAX ? g.Pv : STREAM_VMAX;
+        xy_stageable_kernel<<<dim3((unsigned)(strips * segs), (unsigned)g.N[2]), 128, 0, c->stream>>>(
+            c->hdr, g, L, VL, c->stage_ok, c->err);
+        dim3 grid((unsigned)(strips * segs), (unsigned)((g.Pv + STREAM_VMAX - 1) / STREAM_VMAX), (unsigned)g.N[2]);
+        kern<<<grid, STREAM_THREADS, STREAM_SMEM, c->stream>>>(fin, fout, c->hdr, c->W, g, L, c->stage_ok);
+        flags = c->stage_ok;
+        LAUNCH_AN(2);
+        c->launches += 3;
+        return cudaGetLastError();
+    }
     if (O == 1) LAUNCH_AN(1); else if (O == 2) LAUNCH_AN(2); else LAUNCH_AN(3);
 #undef LAUNCH_AN
 #undef LAUNCH_A

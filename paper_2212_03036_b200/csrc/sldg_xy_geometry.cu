@@ -35,7 +35,7 @@ template <int O>
 __global__ void __launch_bounds__(GeomShared<O>::CELLS) xy_geometry_kernel(const double *__restrict__ va,
                                                                            const double *__restrict__ vb,
                                                                            int4 *__restrict__ hdr, double *__restrict__ W,
-                                                                           int32_t *err, unsigned long long *zflag,
+                                                                           int32_t *err,
                                                                            GridDev g, Basis bs, double tau, int order,
                                                                            int periodic)
 {
@@ -46,11 +46,6 @@ __global__ void __launch_bounds__(GeomShared<O>::CELLS) xy_geometry_kernel(const
     const int t0 = blockIdx.x * CELLS, z = blockIdx.y;
     geometry_block<O, CELLS>(sh, threadIdx.x, CELLS, [&](int c) { return t0 + c < ncell ? t0 + c : -1; }, z, va, vb,
                              hdr, W, err, g, bs, tau, order, periodic);
-    // publish: all writes of this block, then one release increment of the z node's counter
-    if (threadIdx.x == 0) {
-        __threadfence();
-        atomicAdd(zflag + z, 1ull);
-    }
 }
 
 // debug/test helper: expand the packed weight blocks of one z plane to the dense [cell][slot] form
@@ -79,15 +74,16 @@ __global__ void geometry_expand_kernel(const int4 *__restrict__ hdr, const doubl
 
 }  // namespace
 
-int xy_geometry_blocks_per_z(const sldg_ctx *c)
+static int xy_geometry_blocks_per_z(const sldg_ctx *c)
 {
     const int ncell = c->g.n[0] * c->g.n[1];
     const int threads = c->g.o[0] == 3 ? GeomShared<3>::CELLS : GeomShared<2>::CELLS;
     return (ncell + threads - 1) / threads;
 }
 
-cudaError_t launch_xy_geometry(sldg_ctx *c, cudaStream_t stream, double tau, int trace_order)
+cudaError_t launch_xy_geometry(sldg_ctx *c, double tau, int trace_order)
 {
+    cudaStream_t stream = c->stream;
     const GridDev &g = c->g;
     const int O = g.o[0];
     dim3 grid((unsigned)xy_geometry_blocks_per_z(c), (unsigned)g.N[2]);
@@ -96,7 +92,7 @@ cudaError_t launch_xy_geometry(sldg_ctx *c, cudaStream_t stream, double tau, int
         auto kern = xy_geometry_kernel<OO>;                                                                       \
         cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)sizeof(GeomShared<OO>));     \
         kern<<<grid, GeomShared<OO>::CELLS, sizeof(GeomShared<OO>), stream>>>(                                    \
-            c->va, c->vb, c->hdr, c->W, c->err, c->zflag, g, c->basis, tau, trace_order, c->vel_periodic);        \
+            c->va, c->vb, c->hdr, c->W, c->err, g, c->basis, tau, trace_order, c->vel_periodic);        \
     } while (0)
     if (O == 1) LAUNCH_G(1); else if (O == 2) LAUNCH_G(2); else LAUNCH_G(3);
 #undef LAUNCH_G

@@ -290,6 +290,32 @@ def test_advect_xy_parity_rotation_and_swirl(torch, o):
     assert abs(m1 - m0) <= 1e-13 * abs(m0)
 
 
+def test_advect_xy_mixed_streaming_and_direct_blocks(torch):
+    """o = 2: the blocks (strip x segment) whose anchors vary too much for the streaming kernel's ring go to the
+    direct kernel, the others stream -- decided on the device.  A flow whose y displacement swings by +-2.5 cells
+    inside the first segment of 128 rows and is nearly uniform in the second must use both kernels in one step."""
+    spec = GridSpec(n=(16, 160, 1, 24), order=(2, 2, 1, 1), lo=(0.0, 0.0, 0.0, 0.0), hi=(1.0, 10.0, 1.0, 1.0))
+    rng = np.random.default_rng(21)
+    f = rng.random(spec.shape)
+    tau = 1.0
+    yv = np.linspace(0.0, 1.0, spec.n[1] + 1)  # y / Ly at the vertices
+    xv = np.linspace(0.0, 1.0, spec.n[0] + 1)
+    env = (0.5 + 0.5 * np.cos(2 * np.pi * (yv - 0.4))) ** 4
+    by = (2.5 * np.sin(2 * np.pi * (yv - 0.4)) * env + 0.3) * spec.h[1] / tau
+    ax = 0.4 * np.sin(2 * np.pi * xv) * spec.h[0] / tau
+    a = np.ascontiguousarray(np.broadcast_to(ax[None, None, :], (1, spec.n[1] + 1, spec.n[0] + 1)))
+    b = np.ascontiguousarray(np.broadcast_to(by[None, :, None], (1, spec.n[1] + 1, spec.n[0] + 1)))
+    for u in (a, b):  # bitwise periodic
+        u[:, -1, :] = u[:, 0, :]
+        u[:, :, -1] = u[:, :, 0]
+    got, ref, s = _xy_case(torch, spec, f, a, b, tau, 2, 1)
+    direct_blocks = s.debug_counter(0)
+    assert 0 < direct_blocks < 2 * 2, direct_blocks  # 2 strips x 2 segments x 1 z node
+    assert _rel(got, ref) <= TOL
+    m0 = oracle.mass(spec, f)
+    assert abs(float(s.mass().cpu()[0]) - m0) <= 1e-13 * m0
+
+
 def test_zero_and_constant_velocity(torch):
     spec = GridSpec(n=(6, 5, 1, 4), order=(2, 2, 1, 2), lo=(0, 0, 0, 0), hi=(3.0, 2.5, 1, 1))
     rng = np.random.default_rng(9)
