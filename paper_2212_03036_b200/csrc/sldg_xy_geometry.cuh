@@ -405,9 +405,11 @@ __device__ __forceinline__ void geometry_piece(const SH &sh, bool valid, int c, 
     for (int m = 0; m < O2; ++m) iw[m] = 1.0 / (bs.w[O][m % O] * bs.w[O][m / O]);
     const int slot = dr + 3 * ds;
     double *Wout = Wcell + (size_t)rank * (O2 * O2);
-#pragma unroll
+    // o = 3: the two loops over the source node stay rolled -- unrolled, the kernel's code no longer fits the
+    // instruction cache (`no_instruction` was its largest stall) and T, cf spill anyway
+#pragma unroll(O == 3 ? 1 : O)
     for (int kq = 0; kq < O; ++kq)
-#pragma unroll
+#pragma unroll(O == 3 ? 1 : O)
         for (int kp = 0; kp < O; ++kp) {
             double G[O2];
 #pragma unroll
