@@ -62,14 +62,13 @@ WorkspaceMap map_workspace(const sldg_params *p)
     WorkspaceMap m;
     const size_t ncell = (size_t)g.n[0] * g.n[1], Nz = (size_t)g.N[2];
     const size_t vplane = (size_t)(g.n[0] + 1) * (g.n[1] + 1);
-    const size_t o4 = (size_t)g.o[0] * g.o[0] * g.o[0] * g.o[0];
     size_t off = 0;
     auto take = [&](size_t bytes) { size_t at = off; off = align_up(off + bytes, 256); return at; };
     m.Ez = take((size_t)g.lines * 8);
     m.va = take(Nz * vplane * 8);
     m.vb = take(Nz * vplane * 8);
     m.hdr = take(Nz * ncell * 16);
-    m.W = take(Nz * ncell * 9 * o4 * 8);
+    m.W = take(Nz * ncell * 9 * (size_t)sldg_w_block_doubles(g.o[0]) * 8);
     m.n_partials = 8192;
     m.partials = take(m.n_partials * 8);
     m.rho = take((size_t)g.lines * 8);

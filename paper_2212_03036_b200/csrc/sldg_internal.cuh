@@ -11,6 +11,10 @@
 #define SLDG_MAXQ 5       // quadrature points per edge for the Green's-theorem line integrals (2o-1)
 #define SLDG_PV_ALIGN 16  // internal v-line pitch is a multiple of 16 doubles (128 B)
 
+// Doubles between two weight blocks of the 2d geometry in memory: o^4, at o = 3 padded to an even number (bulk
+// copies move multiples of 16 bytes).
+__host__ __device__ constexpr int sldg_w_block_doubles(int O) { return O == 3 ? 82 : O * O * O * O; }
+
 // Grid description passed by value to kernels (lives in the constant bank).
 struct GridDev {
     int n[4];   // cells x,y,z,v

@@ -64,66 +64,79 @@ __device__ __forceinline__ void mbar_wait(uint64_t *bar, uint32_t parity)
     } while (!ok);
 }
 
-// One source cell's contribution for NP v pairs per lane (pair p at v = 64 p + 2 lane): 4 inputs (k), 16 weights
-// W[k][m] (o = 2).  The weights are warp-uniform shared-memory broadcasts.
-template <int NP>
-__device__ __forceinline__ void fma_block_o2(double (&acc)[4][2 * NP], const double *__restrict__ src,
-                                             size_t kq_stride, int VL, const double *__restrict__ Wp)
+// One source cell's contribution for NP v pairs per lane (pair p at v = 64 p + 2 lane): o^2 inputs (k), o^4
+// weights W[k][m].  The weights are warp-uniform shared-memory broadcasts.
+template <int O, int NP>
+__device__ __forceinline__ void fma_block(double (&acc)[O * O][2 * NP], const double *__restrict__ src,
+                                          size_t kq_stride, int VL, const double *__restrict__ Wp)
 {
-    // all input loads of the block first (4 NP in flight), weights k by k (broadcast loads, short latency)
-    double2 in[4][NP];
+    constexpr int O2 = O * O;
+    // all input loads of the block first (o^2 NP in flight), weights k by k (broadcast loads, short latency)
+    double2 in[O2][NP];
 #pragma unroll
-    for (int k = 0; k < 4; ++k)
+    for (int k = 0; k < O2; ++k)
 #pragma unroll
         for (int p = 0; p < NP; ++p)
-            in[k][p] = *reinterpret_cast<const double2 *>(src + (k >> 1) * kq_stride + (k & 1) * VL + 64 * p);
+            in[k][p] = *reinterpret_cast<const double2 *>(src + (k / O) * kq_stride + (k % O) * VL + 64 * p);
 #pragma unroll
-    for (int k = 0; k < 4; ++k) {
-        const double2 w01 = *reinterpret_cast<const double2 *>(Wp + k * 4);
-        const double2 w23 = *reinterpret_cast<const double2 *>(Wp + k * 4 + 2);
+    for (int k = 0; k < O2; ++k) {
+        double w[O2];
+        if (O == 2) {
+            const double2 w01 = *reinterpret_cast<const double2 *>(Wp + k * 4);
+            const double2 w23 = *reinterpret_cast<const double2 *>(Wp + k * 4 + 2);
+            w[0] = w01.x; w[1] = w01.y; w[2] = w23.x; w[O2 - 1] = w23.y;
+        } else {
 #pragma unroll
-        for (int p = 0; p < NP; ++p) {
-            acc[0][2 * p] = fma(w01.x, in[k][p].x, acc[0][2 * p]);
-            acc[0][2 * p + 1] = fma(w01.x, in[k][p].y, acc[0][2 * p + 1]);
-            acc[1][2 * p] = fma(w01.y, in[k][p].x, acc[1][2 * p]);
-            acc[1][2 * p + 1] = fma(w01.y, in[k][p].y, acc[1][2 * p + 1]);
-            acc[2][2 * p] = fma(w23.x, in[k][p].x, acc[2][2 * p]);
-            acc[2][2 * p + 1] = fma(w23.x, in[k][p].y, acc[2][2 * p + 1]);
-            acc[3][2 * p] = fma(w23.y, in[k][p].x, acc[3][2 * p]);
-            acc[3][2 * p + 1] = fma(w23.y, in[k][p].y, acc[3][2 * p + 1]);
+            for (int m = 0; m < O2; ++m) w[m] = Wp[k * O2 + m];
         }
+#pragma unroll
+        for (int m = 0; m < O2; ++m)
+#pragma unroll
+            for (int p = 0; p < NP; ++p) {
+                acc[m][2 * p] = fma(w[m], in[k][p].x, acc[m][2 * p]);
+                acc[m][2 * p + 1] = fma(w[m], in[k][p].y, acc[m][2 * p + 1]);
+            }
     }
 }
 
-constexpr int STREAM_TX = 8;        // target cells per strip
+// Per order: target cells per strip, weight stages (target rows), weight blocks per stage (TX cells x <= 9 blocks),
+// doubles per weight block in memory (o = 3: 81 padded to 82, bulk copies move multiples of 16 bytes), ring bytes.
+template <int O> struct StreamCfg;
+template <> struct StreamCfg<2> {
+    static constexpr int TX = 8, NW = 5, WROW = 72, WB = 16;
+    static constexpr size_t RING = 160 * 1024;
+};
+template <> struct StreamCfg<3> {
+    static constexpr int TX = 4, NW = 4, WROW = 36, WB = 82;
+    static constexpr size_t RING = 126 * 1024;
+};
 constexpr int STREAM_LMAX = 128;    // target rows per segment
 constexpr int STREAM_VMAX = 128;    // v values per chunk
 // consumer warps: VSPLIT per target cell of the strip (VSPLIT = 1: one warp, 4 v values per lane; 2: two warps, one
 // half of the v chunk each, 2 v values per lane); + 1 producer warp
 constexpr int STREAM_NRMAX = 8;     // ring slots (barrier arrays)
-constexpr int STREAM_NW = 5;        // weight stages (target rows)
-constexpr int STREAM_WROW = 72;     // weight blocks per target row stage (8 cells x <= 9 blocks)
 constexpr int STREAM_NACC = 3;      // source rows per target row handled by the register accumulators
-constexpr size_t STREAM_RING_BYTES = 160 * 1024;
-constexpr size_t STREAM_WRING_BYTES = (size_t)STREAM_NW * STREAM_WROW * 128;
-constexpr size_t STREAM_HDR_BYTES = (size_t)STREAM_LMAX * STREAM_TX * 16;
-constexpr size_t STREAM_SMEM = STREAM_RING_BYTES + STREAM_WRING_BYTES + STREAM_HDR_BYTES + 512;
+template <int O> __host__ __device__ constexpr size_t stream_wring_bytes() { return (size_t)StreamCfg<O>::NW * StreamCfg<O>::WROW * StreamCfg<O>::WB * 8; }
+template <int O> __host__ __device__ constexpr size_t stream_hdr_bytes() { return (size_t)STREAM_LMAX * StreamCfg<O>::TX * 16; }
+template <int O> __host__ __device__ constexpr size_t stream_smem_bytes() { return StreamCfg<O>::RING + stream_wring_bytes<O>() + stream_hdr_bytes<O>() + 512; }
+static int stream_tx(int O) { return O == 3 ? StreamCfg<3>::TX : StreamCfg<2>::TX; }
 
 // Whether the block (strip, segment, z node) of the streaming kernel can stage its rows: the x window of the
 // strip over the whole segment must leave at least two ring slots, and a target row may use at most NACC source rows.
 // One criterion, evaluated by the scan kernel below and relied upon by the streaming kernel.
-__device__ __forceinline__ bool stream_block_stageable(int axmin, int axmax, int aymin, int aymax, int VL)
+__device__ __forceinline__ bool stream_block_stageable(int axmin, int axmax, int aymin, int aymax, int VL, int O,
+                                                       int TX, size_t ring_bytes)
 {
-    const int RW = STREAM_TX + axmax - axmin;
-    const size_t stage_bytes = (size_t)2 * 2 * RW * VL * 8;
-    return STREAM_RING_BYTES / stage_bytes >= 2 && aymax - aymin + 1 <= STREAM_NACC;
+    const int RW = TX + axmax - axmin;
+    const size_t stage_bytes = (size_t)O * O * RW * VL * 8;
+    return ring_bytes / stage_bytes >= 2 && aymax - aymin + 1 <= STREAM_NACC;
 }
 
 // grid (strips * segments, Nz): bounds of the anchors of one streaming block -> stage_ok[z][block]
 __global__ void __launch_bounds__(128) xy_stageable_kernel(const int4 *__restrict__ hdrg, GridDev g, int L, int VL,
+                                                           int TX, size_t ring_bytes,
                                                            int32_t *__restrict__ stage_ok, int32_t *err)
 {
-    constexpr int TX = STREAM_TX;
     __shared__ int bnd[4];
     const int nx = g.n[0], ny = g.n[1];
     const int strips = (nx + TX - 1) / TX;
@@ -147,23 +160,26 @@ __global__ void __launch_bounds__(128) xy_stageable_kernel(const int4 *__restric
     atomicMin(&bnd[0], lo_x); atomicMax(&bnd[1], hi_x); atomicMin(&bnd[2], lo_y); atomicMax(&bnd[3], hi_y);
     __syncthreads();
     if (threadIdx.x == 0) {
-        const bool ok = bnd[1] < bnd[0] || stream_block_stageable(bnd[0], bnd[1], bnd[2], bnd[3], VL);
+        const bool ok = bnd[1] < bnd[0] || stream_block_stageable(bnd[0], bnd[1], bnd[2], bnd[3], VL, g.o[0], TX, ring_bytes);
         stage_ok[blockIdx.y * gridDim.x + blockIdx.x] = ok ? 1 : 0;
         if (!ok) atomicAdd(err + 1, 1);  // diagnostic counter 0 (sldg_debug_counter)
     }
 }
 
-template <int VSPLIT>
-__global__ void __launch_bounds__(32 * (STREAM_TX * VSPLIT + 1), 1) xy_apply_stream_kernel(
+template <int O, int VSPLIT>
+__global__ void __launch_bounds__(32 * (StreamCfg<O>::TX * VSPLIT + 1), 1) xy_apply_stream_kernel(
     const double *__restrict__ fin, double *__restrict__ fout, const int4 *__restrict__ hdrg,
     const double *__restrict__ W, GridDev g, int L, const int32_t *__restrict__ stage_ok)
 {
     if (!stage_ok[blockIdx.z * gridDim.x + blockIdx.x]) return;  // the direct kernel handles this block
-    constexpr int TX = STREAM_TX, NW = STREAM_NW, NACC = STREAM_NACC;
+    using Cfg = StreamCfg<O>;
+    constexpr int TX = Cfg::TX, NW = Cfg::NW, NACC = STREAM_NACC, O2 = O * O, WB = Cfg::WB, STREAM_WROW = Cfg::WROW;
     constexpr int STREAM_CWARPS = TX * VSPLIT, STREAM_THREADS = 32 * (STREAM_CWARPS + 1), NP = 2 / VSPLIT;
+    constexpr size_t STREAM_RING_BYTES = Cfg::RING, STREAM_WRING_BYTES = stream_wring_bytes<O>(),
+                     STREAM_HDR_BYTES = stream_hdr_bytes<O>();
     extern __shared__ __align__(128) unsigned char smem_raw[];
-    double *ring = reinterpret_cast<double *>(smem_raw);                                  // [NR][2 kq][2*RW][VL]
-    double *wring = reinterpret_cast<double *>(smem_raw + STREAM_RING_BYTES);             // [NW][WROW][16]
+    double *ring = reinterpret_cast<double *>(smem_raw);                                  // [NR][O kq][O*RW][VL]
+    double *wring = reinterpret_cast<double *>(smem_raw + STREAM_RING_BYTES);             // [NW][WROW][WB]
     int4 *hdr = reinterpret_cast<int4 *>(smem_raw + STREAM_RING_BYTES + STREAM_WRING_BYTES);  // [L][TX]
     int *bnd = reinterpret_cast<int *>(smem_raw + STREAM_RING_BYTES + STREAM_WRING_BYTES + STREAM_HDR_BYTES);
     uint64_t *full = reinterpret_cast<uint64_t *>(bnd + 16);
@@ -220,7 +236,7 @@ __global__ void __launch_bounds__(32 * (STREAM_TX * VSPLIT + 1), 1) xy_apply_str
     const int axmin = bnd[0], aymin = bnd[2];
     const int RW = TX + bnd[1] - axmin;      // window width in cells
     const int S = bnd[3] - aymin + 1;        // source rows per target row
-    const size_t stage_doubles = (size_t)2 * 2 * RW * VL;
+    const size_t stage_doubles = (size_t)O * O * RW * VL;
     int NR = (int)(STREAM_RING_BYTES / (stage_doubles * 8));
     NR = NR > STREAM_NRMAX ? STREAM_NRMAX : NR;
     const double *fz = fin + z * g.sZ + v0;
@@ -263,20 +279,20 @@ __global__ void __launch_bounds__(32 * (STREAM_TX * VSPLIT + 1), 1) xy_apply_str
             double *dst = ring + (size_t)st * stage_doubles;
             if (runs) {
                 // per kq: one copy up to the seam, one after it
-                if (lane < 4) {
-                    const int kq = lane & 1, part = lane >> 1;
+                if (lane < 2 * O) {
+                    const int kq = lane % O, part = lane / O;
                     const int c0 = part ? 0 : wx0, nc = part ? RW - n1 : n1, off = part ? n1 : 0;
                     if (nc > 0)
-                        bulk_g2s(dst + ((size_t)kq * 2 * RW + 2 * off) * VL,
-                                 fz + (long long)(2 * sY + kq) * g.sY + (long long)(2 * c0) * g.sX,
-                                 (uint32_t)(2 * nc * VL * 8), &full[st]);
+                        bulk_g2s(dst + ((size_t)kq * O * RW + O * off) * VL,
+                                 fz + (long long)(O * sY + kq) * g.sY + (long long)(O * c0) * g.sX,
+                                 (uint32_t)(O * nc * VL * 8), &full[st]);
                 }
             } else {
-                for (int l = lane; l < 4 * RW; l += 32) {
-                    const int kq = l / (2 * RW), xd = l - kq * 2 * RW;
-                    const int r = (wx0 + (xd >> 1)) % nx;  // the window may be wider than the periodic box
-                    bulk_g2s(dst + ((size_t)kq * 2 * RW + xd) * VL,
-                             fz + (long long)(2 * sY + kq) * g.sY + (long long)(2 * r + (xd & 1)) * g.sX,
+                for (int l = lane; l < O * O * RW; l += 32) {
+                    const int kq = l / (O * RW), xd = l - kq * O * RW;
+                    const int r = (wx0 + xd / O) % nx;  // the window may be wider than the periodic box
+                    bulk_g2s(dst + ((size_t)kq * O * RW + xd) * VL,
+                             fz + (long long)(O * sY + kq) * g.sY + (long long)(O * r + xd % O) * g.sX,
                              (uint32_t)(VL * 8), &full[st]);
                 }
             }
@@ -293,12 +309,12 @@ __global__ void __launch_bounds__(32 * (STREAM_TX * VSPLIT + 1), 1) xy_apply_str
                 int tot = cnt;
 #pragma unroll
                 for (int o = 1; o < TX; o <<= 1) tot += __shfl_xor_sync(0xffffffffu, tot, o);
-                if (lane == 0) mbar_arrive_expect_tx(&wfull[ws], (uint32_t)(tot * 128));
+                if (lane == 0) mbar_arrive_expect_tx(&wfull[ws], (uint32_t)(tot * WB * 8));
                 __syncwarp();
                 if (cnt > 0) {
                     const long long cellid = zc + (long long)(j0 + k) * nx + i0 + lane;
-                    bulk_g2s(wring + ((size_t)ws * STREAM_WROW + off) * 16, W + (size_t)cellid * 9 * 16,
-                             (uint32_t)(cnt * 128), &wfull[ws]);
+                    bulk_g2s(wring + ((size_t)ws * STREAM_WROW + off) * WB, W + (size_t)cellid * 9 * WB,
+                             (uint32_t)(cnt * WB * 8), &wfull[ws]);
                 }
                 if (++ws == NW) { ws = 0; wph ^= 1; }
             }
@@ -311,20 +327,21 @@ __global__ void __launch_bounds__(32 * (STREAM_TX * VSPLIT + 1), 1) xy_apply_str
     // warp is a contiguous 512-byte run.  Lanes whose pair lies beyond VL compute on stale ring contents and
     // never store.
     const int ci = warp / VSPLIT, vbase = (warp % VSPLIT) * 64 + 2 * lane;
-    const size_t kq_stride = (size_t)2 * RW * VL;
-    double acc[NACC][4][2 * NP];
+    const size_t kq_stride = (size_t)O * RW * VL;
+    const bool wlive = VSPLIT == 1 || (warp % VSPLIT) * 64 < VL;  // this warp's half of the chunk holds data
+    double acc[NACC][O2][2 * NP];
     int4 dsc[NACC];
 #pragma unroll
     for (int a = 0; a < NACC; ++a) {
         dsc[a] = make_int4(0, 0, 0, 0);
 #pragma unroll
-        for (int m = 0; m < 4; ++m)
+        for (int m = 0; m < O2; ++m)
 #pragma unroll
             for (int e = 0; e < 2 * NP; ++e) acc[a][m][e] = 0.0;
     }
     int st = 0, ph = 0, ws = 0, wph = 0;  // source ring slot / parity, weight stage / parity (of the `full` barriers)
     int wsd = 0;                          // weight stage of the target row that is stored next
-    double *orow = oz + (long long)(2 * j0) * g.sY + (long long)(2 * (i0 + ci)) * g.sX + vbase;
+    double *orow = oz + (long long)(O * j0) * g.sY + (long long)(O * (i0 + ci)) * g.sX + vbase;
 
     // one step: source row k; target rows k, k-1, k-2 (accumulator sets are indexed by row mod 3, static
     // because the step loop is unrolled by 3)
@@ -351,14 +368,25 @@ __global__ void __launch_bounds__(32 * (STREAM_TX * VSPLIT + 1), 1) xy_apply_str
                     const int set = (u - d + NACC) % NACC;
                     if (k - d < 0 || k - d >= rows) continue;
                     const int desc = d == 0 ? dsc[set].x : (d == 1 ? dsc[set].y : dsc[set].z);
-                    if (!(desc & 7)) continue;
-                    const double *Wp = wring + ((desc >> 3) & 0x1ff) * 16;
-                    const double *src = srow + (size_t)(2 * (desc >> 12)) * VL;
+                    if (!(desc & 7) || !wlive) continue;
+                    const double *Wp = wring + ((desc >> 3) & 0x1ff) * WB;
+                    const double *src = srow + (size_t)(O * (desc >> 12)) * VL;
+                    if (O == 2) {
 #pragma unroll
-                    for (int dx = 0; dx < 3; ++dx) {
-                        if ((desc >> dx) & 1) {
-                            fma_block_o2<NP>(acc[set], src + (size_t)(2 * dx) * VL, kq_stride, VL, Wp);
-                            Wp += 16;
+                        for (int dx = 0; dx < 3; ++dx) {
+                            if ((desc >> dx) & 1) {
+                                fma_block<O, NP>(acc[set], src + (size_t)(O * dx) * VL, kq_stride, VL, Wp);
+                                Wp += WB;
+                            }
+                        }
+                    } else {
+                        // o = 3: one copy of the 162-FMA block per (set, d), or the code outgrows the I-cache
+#pragma unroll 1
+                        for (int dx = 0; dx < 3; ++dx) {
+                            if ((desc >> dx) & 1) {
+                                fma_block<O, NP>(acc[set], src + (size_t)(O * dx) * VL, kq_stride, VL, Wp);
+                                Wp += WB;
+                            }
                         }
                     }
                 }
@@ -373,8 +401,8 @@ __global__ void __launch_bounds__(32 * (STREAM_TX * VSPLIT + 1), 1) xy_apply_str
                 if (dsc[set].w >> 8) {
                     double *o = orow;
 #pragma unroll
-                    for (int m = 0; m < 4; ++m) {
-                        double *om = o + (m >> 1) * g.sY + (m & 1) * g.sX;
+                    for (int m = 0; m < O2; ++m) {
+                        double *om = o + (m / O) * g.sY + (m % O) * g.sX;
 #pragma unroll
                         for (int p = 0; p < NP; ++p)
                             if (vbase + 64 * p < VL)
@@ -382,9 +410,9 @@ __global__ void __launch_bounds__(32 * (STREAM_TX * VSPLIT + 1), 1) xy_apply_str
                                        make_double2(acc[set][m][2 * p], acc[set][m][2 * p + 1]));
                     }
                 }
-                orow += 2 * g.sY;
+                orow += O * g.sY;
 #pragma unroll
-                for (int m = 0; m < 4; ++m)
+                for (int m = 0; m < O2; ++m)
 #pragma unroll
                     for (int e = 0; e < 2 * NP; ++e) acc[set][m][e] = 0.0;
                 __syncwarp();
@@ -402,23 +430,28 @@ __global__ void __launch_bounds__(32 * (STREAM_TX * VSPLIT + 1), 1) xy_apply_str
 // contiguous in m) each feeding NV FMAs -- o^2 NV accumulators per lane, o^2 + NV loads per o^2 NV FMAs.
 // Inputs and weights through L1/L2.  At o = 3 the step is bound by the fp64 pipe (2*9*c FMA per DOF).
 // --------------------------------------------------------------------------------------------------
-// stage_ok != nullptr: only the tiles whose streaming block (strip = the tile's 8 columns, segment of L rows, z
-// node) is NOT stageable are done here (the streaming kernel does the others).
+// stage_ok != nullptr: only the cells whose streaming block (strip of stx columns, segment of L rows, z node) is
+// NOT stageable are done here (the streaming kernel does the others).
 template <int O, int NV>
 __global__ void __launch_bounds__(256, 2) xy_apply_direct_kernel(const double *__restrict__ fin,
                                                               double *__restrict__ fout,
                                                               const int4 *__restrict__ hdrg,
                                                               const double *__restrict__ W, GridDev g,
-                                                              const int32_t *__restrict__ stage_ok, int L)
+                                                              const int32_t *__restrict__ stage_ok, int L, int stx)
 {
     constexpr int O2 = O * O, TX = 8, TY = 4;
     const int nx = g.n[0], ny = g.n[1];
     const int tiles_x = (nx + TX - 1) / TX;
     const int tile_i = (blockIdx.x % tiles_x) * TX, tile_j = (blockIdx.x / tiles_x) * TY;
     const int z = blockIdx.z;
+    const int segs = stage_ok ? (ny + L - 1) / L : 0, strips = stage_ok ? (nx + stx - 1) / stx : 0;
     if (stage_ok) {
-        const int segs = (ny + L - 1) / L;
-        if (stage_ok[(z * segs + tile_j / L) * tiles_x + tile_i / TX]) return;
+        // the tile's rows lie in one segment (L is a multiple of TY or the only segment); its columns in TX / stx
+        // strips: nothing to do here if all of them stream
+        bool all_stream = true;
+        for (int i = tile_i; i < min(tile_i + TX, nx); i += stx)
+            all_stream = all_stream && stage_ok[(z * segs + tile_j / L) * strips + i / stx];
+        if (all_stream) return;
     }
     const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
     const int v = blockIdx.y * 32 * NV + lane;
@@ -433,6 +466,7 @@ __global__ void __launch_bounds__(256, 2) xy_apply_direct_kernel(const double *_
     for (int c = warp; c < TX * TY; c += 8) {
         const int i = tile_i + (c % TX), j = tile_j + (c / TX);
         if (i >= nx || j >= ny) continue;
+        if (stage_ok && stage_ok[(z * segs + j / L) * strips + i / stx]) continue;  // the streaming kernel's
         const long long cellid = (long long)z * ncell + (long long)j * nx + i;
         const int4 h = __ldcg(hdrg + cellid);
         const int ax = wrap_idx(i + h.x, nx);
@@ -450,7 +484,7 @@ __global__ void __launch_bounds__(256, 2) xy_apply_direct_kernel(const double *_
             int r = ax + slot % 3, s = ay + slot / 3;
             if (r >= nx) r -= nx;
             if (s >= ny) s -= ny;
-            const double *Wp = W + ((size_t)cellid * 9 + nb++) * (O2 * O2);
+            const double *Wp = W + ((size_t)cellid * 9 + nb++) * sldg_w_block_doubles(O);
 #pragma unroll
             for (int kq = 0; kq < O; ++kq)
 #pragma unroll
@@ -481,13 +515,13 @@ __global__ void __launch_bounds__(256, 2) xy_apply_direct_kernel(const double *_
     }
 }
 
-static bool xy_apply_streams(const GridDev &g) { return g.o[0] == 2 && !getenv("SLDG_APPLY_DIRECT"); }
+static bool xy_apply_streams(int O) { return (O == 2 || O == 3) && !getenv("SLDG_APPLY_DIRECT"); }
 static int stream_segment_rows(int ny) { return ny < STREAM_LMAX ? ny : STREAM_LMAX; }
 
 size_t xy_apply_stage_flags(const sldg_params *p)
 {
-    const int L = stream_segment_rows(p->n[1]);
-    const size_t strips = (p->n[0] + STREAM_TX - 1) / STREAM_TX, segs = (p->n[1] + L - 1) / L;
+    const int L = stream_segment_rows(p->n[1]), tx = stream_tx(p->order[0]);
+    const size_t strips = (p->n[0] + tx - 1) / tx, segs = (p->n[1] + L - 1) / L;
     return strips * segs * (size_t)p->n[2] * p->order[2];
 }
 
@@ -503,30 +537,39 @@ cudaError_t launch_xy_apply(sldg_ctx *c, const double *fin, double *fout)
     dim3 dgrid((unsigned)tiles, (unsigned)vchunks, (unsigned)g.N[2]);
     const int32_t *flags = nullptr;
     int L = 0;
+    const int stx = stream_tx(O);
 #define LAUNCH_A(OO, NN) \
-    xy_apply_direct_kernel<OO, NN><<<dgrid, 256, 0, c->stream>>>(fin, fout, c->hdr, c->W, g, flags, L)
+    xy_apply_direct_kernel<OO, NN><<<dgrid, 256, 0, c->stream>>>(fin, fout, c->hdr, c->W, g, flags, L, stx)
 #define LAUNCH_AN(OO)                                                                                         \
     do {                                                                                                      \
         if (nv == 1) LAUNCH_A(OO, 1); else if (nv == 2) LAUNCH_A(OO, 2); else if (nv == 3) LAUNCH_A(OO, 3);   \
         else if (nv == 4) LAUNCH_A(OO, 4); else LAUNCH_A(OO, 5);                                              \
     } while (0)
-    if (xy_apply_streams(g)) {
-        // o = 2: which blocks can stream is decided on the device (scan of the headers); the streaming kernel does
+    if (xy_apply_streams(O)) {
+        // Which blocks can stream is decided on the device (scan of the headers); the streaming kernel does
         // those, the direct kernel the others (none in an ITG step; most of them in a solid-body rotation, where the
         // anchors change by many cells along a strip).  No host synchronisation.
         static const int vsplit = getenv("SLDG_APPLY_VSPLIT") ? atoi(getenv("SLDG_APPLY_VSPLIT")) : 1;
-        auto kern = vsplit == 1 ? xy_apply_stream_kernel<1> : xy_apply_stream_kernel<2>;
-        const int STREAM_THREADS = 32 * (STREAM_TX * (vsplit == 1 ? 1 : 2) + 1);
-        cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)STREAM_SMEM);
         L = stream_segment_rows(g.n[1]);
-        const int strips = (g.n[0] + STREAM_TX - 1) / STREAM_TX, segs = (g.n[1] + L - 1) / L;
+        const int strips = (g.n[0] + stx - 1) / stx, segs = (g.n[1] + L - 1) / L;
         const int VL = g.Pv < STREAM_VMAX ? g.Pv : STREAM_VMAX;
+        const size_t ring = O == 3 ? StreamCfg<3>::RING : StreamCfg<2>::RING;
         xy_stageable_kernel<<<dim3((unsigned)(strips * segs), (unsigned)g.N[2]), 128, 0, c->stream>>>(
-            c->hdr, g, L, VL, c->stage_ok, c->err);
+            c->hdr, g, L, VL, stx, ring, c->stage_ok, c->err);
         dim3 grid((unsigned)(strips * segs), (unsigned)((g.Pv + STREAM_VMAX - 1) / STREAM_VMAX), (unsigned)g.N[2]);
-        kern<<<grid, STREAM_THREADS, STREAM_SMEM, c->stream>>>(fin, fout, c->hdr, c->W, g, L, c->stage_ok);
+#define LAUNCH_S(OO, VS)                                                                                      \
+    do {                                                                                                      \
+        auto kern = xy_apply_stream_kernel<OO, VS>;                                                           \
+        cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)stream_smem_bytes<OO>()); \
+        kern<<<grid, 32 * (StreamCfg<OO>::TX * VS + 1), stream_smem_bytes<OO>(), c->stream>>>(                \
+            fin, fout, c->hdr, c->W, g, L, c->stage_ok);                                                      \
+    } while (0)
+        if (O == 3) LAUNCH_S(3, 2);
+        else if (vsplit == 1) LAUNCH_S(2, 1);
+        else LAUNCH_S(2, 2);
+#undef LAUNCH_S
         flags = c->stage_ok;
-        LAUNCH_AN(2);
+        if (O == 3) LAUNCH_AN(3); else LAUNCH_AN(2);
         c->launches += 3;
         return cudaGetLastError();
     }

@@ -50,6 +50,7 @@ __global__ void __launch_bounds__(GeomShared<O>::CELLS) xy_geometry_kernel(const
 
 // debug/test helper: expand the packed weight blocks of one z plane to the dense [cell][slot] form
 __global__ void geometry_expand_kernel(const int4 *__restrict__ hdr, const double *__restrict__ W, int ncell, int o4,
+                                       int wbs,
                                        int32_t *__restrict__ anchor, int32_t *__restrict__ mask,
                                        double *__restrict__ Wd)
 {
@@ -67,7 +68,7 @@ __global__ void geometry_expand_kernel(const int4 *__restrict__ hdr, const doubl
     for (int slot = 0; slot < 9; ++slot) {
         if (!((h.z >> slot) & 1)) continue;
         for (int e = threadIdx.x; e < o4; e += blockDim.x)
-            Wd[((size_t)t * 9 + slot) * o4 + e] = W[((size_t)t * 9 + n) * o4 + e];
+            Wd[((size_t)t * 9 + slot) * o4 + e] = W[((size_t)t * 9 + n) * wbs + e];
         ++n;
     }
 }
@@ -105,8 +106,9 @@ cudaError_t launch_geometry_expand(sldg_ctx *c, int z, int32_t *anchor, int32_t 
     const GridDev &g = c->g;
     const int ncell = g.n[0] * g.n[1];
     const int o4 = g.o[0] * g.o[0] * g.o[0] * g.o[0];
-    geometry_expand_kernel<<<ncell, 32, 0, c->stream>>>(c->hdr + (size_t)z * ncell, c->W + (size_t)z * ncell * 9 * o4,
-                                                        ncell, o4, anchor, mask, Wd);
+    const int wbs = sldg_w_block_doubles(g.o[0]);
+    geometry_expand_kernel<<<ncell, 32, 0, c->stream>>>(c->hdr + (size_t)z * ncell, c->W + (size_t)z * ncell * 9 * wbs,
+                                                        ncell, o4, wbs, anchor, mask, Wd);
     c->launches++;
     return cudaGetLastError();
 }

@@ -404,7 +404,7 @@ __device__ __forceinline__ void geometry_piece(const SH &sh, bool valid, int c, 
 #pragma unroll
     for (int m = 0; m < O2; ++m) iw[m] = 1.0 / (bs.w[O][m % O] * bs.w[O][m / O]);
     const int slot = dr + 3 * ds;
-    double *Wout = Wcell + (size_t)rank * (O2 * O2);
+    double *Wout = Wcell + (size_t)rank * sldg_w_block_doubles(O);
     // o = 3: the two loops over the source node stay rolled -- unrolled, the kernel's code no longer fits the
     // instruction cache (`no_instruction` was its largest stall) and T, cf spill anyway
 #pragma unroll(O == 3 ? 1 : O)
@@ -490,7 +490,7 @@ __device__ __forceinline__ void geometry_block(GeomShared<O, CELLS> &sh, int tid
         const int w = sh.nr[cc] + 1;
         const int ds = k / w, dr = k - ds * w;
         const long long cellid = (long long)z * ncell + cell_of(cc);
-        geometry_piece<O>(sh, valid, cc, k, dr, ds, bs, W + (size_t)cellid * 9 * O4, &sh.mask[cc]);
+        geometry_piece<O>(sh, valid, cc, k, dr, ds, bs, W + (size_t)cellid * 9 * sldg_w_block_doubles(O), &sh.mask[cc]);
     }
     __syncthreads();
     if (t >= 0) {
