@@ -282,10 +282,14 @@ int sldg_create(const sldg_params *p, double *f_a_dev, double *f_b_dev, void *wo
             return SLDG_ECUDA;
         }
     for (int k = 0; k < 2; ++k)
-        if (cudaEventCreate(&c->gev[k]) != cudaSuccess) {
+        if (cudaEventCreate(&c->gev[k]) != cudaSuccess || cudaEventCreate(&c->cev[k]) != cudaSuccess) {
             sldg_destroy(c);
             return SLDG_ECUDA;
         }
+    if (cudaStreamCreateWithFlags(&c->cstream, cudaStreamNonBlocking) != cudaSuccess) {
+        sldg_destroy(c);
+        return SLDG_ECUDA;
+    }
     // fields default to zero, error word cleared
     cudaError_t e = cudaMemsetAsync(ws + m.Ez, 0, m.hdr - m.Ez, c->stream);
     if (e == cudaSuccess) e = cudaMemsetAsync(c->err, 0, 256, c->stream);
@@ -302,8 +306,14 @@ int sldg_destroy(sldg_ctx *c)
     if (!c) return SLDG_EINVAL;
     for (int k = 0; k < 8; ++k)
         if (c->ev[k]) cudaEventDestroy(c->ev[k]);
-    for (int k = 0; k < 2; ++k)
+    if (c->cstream) {
+        cudaStreamSynchronize(c->cstream);
+        cudaStreamDestroy(c->cstream);
+    }
+    for (int k = 0; k < 2; ++k) {
         if (c->gev[k]) cudaEventDestroy(c->gev[k]);
+        if (c->cev[k]) cudaEventDestroy(c->cev[k]);
+    }
     delete c;
     return SLDG_OK;
 }
@@ -410,6 +420,10 @@ static int do_pair(sldg_ctx *c, double tau, bool z_first, cudaEvent_t mid, int *
 // stream with per-z counters, or as a prologue of every apply block -- was built and measured slower: DESIGN.md 6.3.)
 static int do_xy(sldg_ctx *c, double tau, int trace_order)
 {
+    if (c->ab_pending) {  // a, b uploaded on the copy stream by sldg_strang_step_host
+        cudaStreamWaitEvent(c->stream, c->cev[1], 0);
+        c->ab_pending = 0;
+    }
     cudaEventRecord(c->gev[0], c->stream);
     if (launch_xy_geometry(c, tau, trace_order) != cudaSuccess) return SLDG_ECUDA;
     cudaEventRecord(c->gev[1], c->stream);
@@ -491,8 +505,13 @@ int sldg_strang_step_host(sldg_ctx *c, double dt, const double *Ez_host, const d
     if (a_host) {
         size_t bytes = (size_t)g.N[2] * (g.n[0] + 1) * (g.n[1] + 1) * 8;
         c->vel_periodic = periodic ? 1 : 0;
-        if (cudaMemcpyAsync(c->va, a_host, bytes, cudaMemcpyHostToDevice, c->stream) != cudaSuccess) return SLDG_ECUDA;
-        if (cudaMemcpyAsync(c->vb, b_host, bytes, cudaMemcpyHostToDevice, c->stream) != cudaSuccess) return SLDG_ECUDA;
+        // a, b are first needed by the 2d step: their upload runs on the copy stream under the z and v sweeps
+        cudaEventRecord(c->cev[0], c->stream);
+        cudaStreamWaitEvent(c->cstream, c->cev[0], 0);
+        if (cudaMemcpyAsync(c->va, a_host, bytes, cudaMemcpyHostToDevice, c->cstream) != cudaSuccess) return SLDG_ECUDA;
+        if (cudaMemcpyAsync(c->vb, b_host, bytes, cudaMemcpyHostToDevice, c->cstream) != cudaSuccess) return SLDG_ECUDA;
+        cudaEventRecord(c->cev[1], c->cstream);
+        c->ab_pending = 1;
     }
     int rc = sldg_strang_step(c, dt);
     if (rc) return rc;

@@ -63,6 +63,9 @@ struct sldg_ctx {
     int32_t *err;           // sticky device error word
     int32_t *stage_ok;      // [Nz][strips*segments] 1: that block of the streaming 2d apply can stage its rows
     cudaEvent_t gev[2];     // start / end of the geometry kernel of the last 2d step
+    cudaStream_t cstream;   // copy stream: sldg_strang_step_host uploads a, b under the first sweeps
+    cudaEvent_t cev[2];     // fork / join of that upload
+    int ab_pending;         // an upload of a, b is in flight on cstream: the next 2d step waits for it
     int fuse, last_fused;   // fuse: sldg_strang_step runs each pair of adjacent sweeps in one pass
     size_t n_partials;
     int trace_order, vel_periodic;
