@@ -56,7 +56,7 @@ __device__ __forceinline__ void trace_point(const double *__restrict__ a, const 
     fy = eta - ty * ub;
 }
 
-// Gauss-Jordan with partial pivoting on [V | X], fully unrolled so that everything stays in registers.
+// Gauss-Jordan with partial pivoting on [V | X], fully unrolled so that everything stays in registers (o <= 2).
 // On exit X = V^{-1}.  Returns the smallest pivot magnitude.
 template <int N>
 __device__ __forceinline__ double gauss_jordan(double (&V)[N][N], double (&X)[N][N])
@@ -100,6 +100,70 @@ __device__ __forceinline__ double gauss_jordan(double (&V)[N][N], double (&X)[N]
                     V[r][k] = fma(-fct, V[c][k], V[r][k]);
                     X[r][k] = fma(-fct, X[c][k], X[r][k]);
                 }
+            }
+        }
+    }
+    return minpiv;
+}
+
+// In-place Gauss-Jordan inversion with partial pivoting of the N x N matrix whose element (r, k) lives at
+// a[(r * N + k) * stride] (one thread's column of a shared-memory array: conflict-free).  For o = 3 (N = 9): two
+// 9 x 9 matrices in registers are 324 registers' worth and spill; in local memory they thrash L1 (measured: 2x
+// slower).  Returns the smallest pivot magnitude.
+template <int N>
+__device__ __forceinline__ double invert_in_place(double *a, int stride)
+{
+    double minpiv = 1e300;
+    unsigned long long perm = 0;  // 4 bits per column: the row it was swapped with
+#pragma unroll 1
+    for (int c = 0; c < N; ++c) {
+        int p = c;
+        double best = fabs(a[(c * N + c) * stride]);
+#pragma unroll 1
+        for (int r = c + 1; r < N; ++r) {
+            const double v = fabs(a[(r * N + c) * stride]);
+            if (v > best) {
+                best = v;
+                p = r;
+            }
+        }
+        perm |= (unsigned long long)p << (4 * c);
+        if (p != c) {
+#pragma unroll
+            for (int k = 0; k < N; ++k) {
+                const double t = a[(c * N + k) * stride];
+                a[(c * N + k) * stride] = a[(p * N + k) * stride];
+                a[(p * N + k) * stride] = t;
+            }
+        }
+        minpiv = dmin(minpiv, best);
+        const double inv = 1.0 / a[(c * N + c) * stride];
+        a[(c * N + c) * stride] = 1.0;
+        double rowc[N];
+#pragma unroll
+        for (int k = 0; k < N; ++k) {
+            rowc[k] = a[(c * N + k) * stride] * inv;
+            a[(c * N + k) * stride] = rowc[k];
+        }
+#pragma unroll 1
+        for (int r = 0; r < N; ++r) {
+            if (r == c) continue;
+            const double fct = a[(r * N + c) * stride];
+            a[(r * N + c) * stride] = 0.0;
+#pragma unroll
+            for (int k = 0; k < N; ++k) a[(r * N + k) * stride] = fma(-fct, rowc[k], a[(r * N + k) * stride]);
+        }
+    }
+    // the row swaps of the elimination become column swaps of the inverse, undone in reverse order
+#pragma unroll 1
+    for (int c = N - 1; c >= 0; --c) {
+        const int p = (int)((perm >> (4 * c)) & 15);
+        if (p != c) {
+#pragma unroll 1
+            for (int r = 0; r < N; ++r) {
+                const double t = a[(r * N + c) * stride];
+                a[(r * N + c) * stride] = a[(r * N + p) * stride];
+                a[(r * N + p) * stride] = t;
             }
         }
     }
@@ -293,6 +357,28 @@ __device__ __forceinline__ int geometry_setup(const double *__restrict__ va, con
             }
         xc *= 1.0 / O2;
         yc *= 1.0 / O2;
+        if (O == 3) {
+            // Vandermonde matrix straight into this cell's column of sh.Vi, inverted there in place
+#pragma unroll
+            for (int m = 0; m < O2; ++m) {
+                double py = 1.0;
+#pragma unroll
+                for (int bq = 0; bq < O; ++bq) {
+                    double px = 1.0;
+#pragma unroll
+                    for (int bp = 0; bp < O; ++bp) {
+                        sh.Vi[m * O2 + bp + O * bq][c] = px * py;
+                        px *= fx[m] - xc;
+                    }
+                    py *= fy[m] - yc;
+                }
+            }
+            const double minpiv = invert_in_place<O2>(&sh.Vi[0][c], SH::CELLS);  // Vi[ab][m] = (V^-1)[ab][m]
+            if (!(minpiv > 1e-10)) atomicMin(err, SLDG_EGEOM);
+            sh.xc[c] = xc;
+            sh.yc[c] = yc;
+            return (nr + 1) * (ns + 1);
+        }
         double V[O2][O2];
 #pragma unroll
         for (int m = 0; m < O2; ++m) {
