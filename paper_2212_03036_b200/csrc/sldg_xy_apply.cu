@@ -430,8 +430,8 @@ __global__ void __launch_bounds__(32 * (StreamCfg<O>::TX * VSPLIT + 1), 1) xy_ap
 // contiguous in m) each feeding NV FMAs -- o^2 NV accumulators per lane, o^2 + NV loads per o^2 NV FMAs.
 // Inputs and weights through L1/L2.  At o = 3 the step is bound by the fp64 pipe (2*9*c FMA per DOF).
 // --------------------------------------------------------------------------------------------------
-// stage_ok != nullptr: only the cells whose streaming block (strip of stx columns, segment of L rows, z node) is
-// NOT stageable are done here (the streaming kernel does the others).
+// stage_ok != nullptr (filtered): the grid is that of the streaming kernel, a block does the cells of one streaming
+// block (strip of stx columns, segment of L rows, z node) if that block is NOT stageable, and nothing otherwise.
 template <int O, int NV>
 __global__ void __launch_bounds__(256, 2) xy_apply_direct_kernel(const double *__restrict__ fin,
                                                               double *__restrict__ fout,
@@ -441,17 +441,22 @@ __global__ void __launch_bounds__(256, 2) xy_apply_direct_kernel(const double *_
 {
     constexpr int O2 = O * O, TX = 8, TY = 4;
     const int nx = g.n[0], ny = g.n[1];
-    const int tiles_x = (nx + TX - 1) / TX;
-    const int tile_i = (blockIdx.x % tiles_x) * TX, tile_j = (blockIdx.x / tiles_x) * TY;
     const int z = blockIdx.z;
-    const int segs = stage_ok ? (ny + L - 1) / L : 0, strips = stage_ok ? (nx + stx - 1) / stx : 0;
+    // the block's cells: a tile of 8 x 4, or -- filtered -- one whole block of the streaming kernel (strip x segment)
+    int ri0, rj0, rw, rh;
     if (stage_ok) {
-        // the tile's rows lie in one segment (L is a multiple of TY or the only segment); its columns in TX / stx
-        // strips: nothing to do here if all of them stream
-        bool all_stream = true;
-        for (int i = tile_i; i < min(tile_i + TX, nx); i += stx)
-            all_stream = all_stream && stage_ok[(z * segs + tile_j / L) * strips + i / stx];
-        if (all_stream) return;
+        if (stage_ok[z * gridDim.x + blockIdx.x]) return;  // streamed
+        const int strips = (nx + stx - 1) / stx;
+        ri0 = (blockIdx.x % strips) * stx;
+        rj0 = (blockIdx.x / strips) * L;
+        rw = min(stx, nx - ri0);
+        rh = min(L, ny - rj0);
+    } else {
+        const int tiles_x = (nx + TX - 1) / TX;
+        ri0 = (blockIdx.x % tiles_x) * TX;
+        rj0 = (blockIdx.x / tiles_x) * TY;
+        rw = min(TX, nx - ri0);
+        rh = min(TY, ny - rj0);
     }
     const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
     const int v = blockIdx.y * 32 * NV + lane;
@@ -463,10 +468,8 @@ __global__ void __launch_bounds__(256, 2) xy_apply_direct_kernel(const double *_
     const double *fz = fin + z * g.sZ + v;
     double *oz = fout + z * g.sZ + v;
 
-    for (int c = warp; c < TX * TY; c += 8) {
-        const int i = tile_i + (c % TX), j = tile_j + (c / TX);
-        if (i >= nx || j >= ny) continue;
-        if (stage_ok && stage_ok[(z * segs + j / L) * strips + i / stx]) continue;  // the streaming kernel's
+    for (int c = warp; c < rw * rh; c += 8) {
+        const int i = ri0 + (c % rw), j = rj0 + (c / rw);
         const long long cellid = (long long)z * ncell + (long long)j * nx + i;
         const int4 h = __ldcg(hdrg + cellid);
         const int ax = wrap_idx(i + h.x, nx);
@@ -569,6 +572,7 @@ cudaError_t launch_xy_apply(sldg_ctx *c, const double *fin, double *fout)
         else LAUNCH_S(2, 2);
 #undef LAUNCH_S
         flags = c->stage_ok;
+        dgrid = dim3((unsigned)(strips * segs), (unsigned)vchunks, (unsigned)g.N[2]);
         if (O == 3) LAUNCH_AN(3); else LAUNCH_AN(2);
         c->launches += 3;
         return cudaGetLastError();

@@ -536,7 +536,6 @@ __device__ __forceinline__ void geometry_block(GeomShared<O, CELLS> &sh, int tid
                                                int4 *hdr, double *W, int32_t *err, const GridDev &g, const Basis &bs,
                                                double tau, int order, int periodic)
 {
-    constexpr int O4 = O * O * O * O;
     const int lane = tid & 31, warp = tid >> 5;
     const int ncell = g.n[0] * g.n[1];
     const int t = tid < CELLS ? cell_of(tid) : -1;
