@@ -6,8 +6,8 @@
 // warp-uniform, the control flow over the (up to 3x3) non-empty source cells is warp-uniform, and empty
 // source cells cost nothing.
 //
-//   xy_apply_stream_kernel (o = 2, the default): a streaming stencil in SOURCE-row order.  A block owns a
-//     strip of TX = 8 target cells in x, a segment of up to 128 target rows in y, one z node and one chunk
+//   xy_apply_stream_kernel (o = 2 and 3; the numbers below are o = 2): a streaming stencil in SOURCE-row order.
+//     A block owns a strip of TX = 8 target cells in x (o = 3: 4), a segment of up to 128 target rows in y, one z node and one chunk
 //     of <= 128 v values.  The prologue reads the segment's headers and takes the bounds of the anchors;
 //     they fix a static schedule: target row j uses source rows j+aymin .. j+aymin+2 and the x window
 //     [axmin, TX-1+axmax].  A producer warp streams the source rows (each row = the window's lines, all v
@@ -17,8 +17,9 @@
 //     use it -- their partial sums live in registers -- release the row at once, and store a target row
 //     when its last source row has been applied.  Because a source row is never held while others arrive,
 //     all but one ring slot are in flight.  Every input line is fetched once per strip (x halo:
-//     window/TX = 10/8), weights once.  Segments whose anchors vary too much fall back to direct loads.
-//   xy_apply_direct_kernel (any o): warp <-> target cell, inputs through L1.
+//     window/TX = 10/8), weights once.
+//   xy_stageable_kernel: decides per block (strip, segment, z node) whether its anchors allow that schedule.
+//   xy_apply_direct_kernel (any o): warp <-> target cell, inputs through L1; does the blocks that cannot stream.
 #include <stdlib.h>
 
 #include "sldg_internal.cuh"
