@@ -15,8 +15,9 @@
 //           remaining NH lines as soon as the current plane is done (NL = 80 of 128 at 128 x 128, o = 2);
 //   ZV      phase A  z sweep in place, thread <-> (v, slice of z): the result for target cell i is written over
 //                    its left source cell (i+s) mod nz, which is dead by then -- column v ends up rotated by s(v);
-//           phase B  v sweep line by line, warp <-> line, gathering through the per-column rotation, results
-//                    straight to global memory;
+//           phase B  v sweep line by line, warp <-> line, lane <-> source cells (the rotation offsets of a lane's
+//                    columns sit in registers; the other source cell of a target comes from the next lane by
+//                    shuffle), results straight to global memory;
 //   VZ      phase A  v sweep in place, warp <-> line (all sources of a warp's line are in registers before the
 //                    first write);
 //           phase B  z sweep, thread <-> (v, slice of z), results straight to global memory.
@@ -157,6 +158,14 @@ __global__ void __launch_bounds__(FUSED_BLOCK, 1) fused_sweep_kernel(const doubl
         return;
     }
 
+    int rreg[CPL][O];  // z,v pair: rotation offsets of this lane's columns in the line-wise phase
+#pragma unroll
+    for (int k = 0; k < CPL; ++k)
+#pragma unroll
+        for (int m = 0; m < O; ++m) {
+            const int cell = lane + 32 * k;
+            rreg[k][m] = (ZFIRST && cell < nv) ? rotoff[cell * O + m] : 0;
+        }
     double ez_next = 0.0;
     int col = blockIdx.x, par = 0;
     uint32_t phL[2] = {0, 0}, phH = 0;
@@ -247,7 +256,9 @@ __global__ void __launch_bounds__(FUSED_BLOCK, 1) fused_sweep_kernel(const doubl
                 step(last);  // the last target of the slice: its right source cell was read before the sweep
             }
             compute_sync();
-            // ---- phase B: v sweep of every line, gathering through the rotation, to global memory ---------
+            // ---- phase B: v sweep of every line, to global memory.  lane <-> SOURCE cells (fixed columns, so the
+            //      rotation offsets of a lane's columns sit in registers); the right source cell of a target comes
+            //      from the neighbouring lane by shuffle; the lane stores target cell (source cell - s) ---------------
 #pragma unroll 1
             for (int zr = warp; zr < Nz; zr += FUSED_THREADS / 32) {
                 const int s = vs[zr];
@@ -261,54 +272,47 @@ __global__ void __launch_bounds__(FUSED_BLOCK, 1) fused_sweep_kernel(const doubl
                     }
                 double *w = dst + zr * g.sZ;
                 const int zoff = zr * Pv;
-                auto at = [&](int vcol) {  // value of line zr at column vcol: the column is rotated by whole cells
-                    int t = rotoff[vcol] + zoff;
-                    if (t >= NzPv) t -= NzPv;
-                    return tile[t + vcol];
-                };
-                auto load_cell = [&](int cc, double (&u)[O]) {
-                    if (O == 2) {
-                        const int2 ro = *reinterpret_cast<const int2 *>(rotoff + 2 * cc);
-                        int t0 = ro.x + zoff, t1 = ro.y + zoff;
-                        if (t0 >= NzPv) t0 -= NzPv;
-                        if (t1 >= NzPv) t1 -= NzPv;
-                        u[0] = tile[t0 + 2 * cc];
-                        u[O - 1] = tile[t1 + 2 * cc + 1];
-                    } else {
+                double u0[CPL][O];
 #pragma unroll
-                        for (int m = 0; m < O; ++m) u[m] = at(cc * O + m);
+                for (int k = 0; k < CPL; ++k) {
+                    const int cell = lane + 32 * k;
+#pragma unroll
+                    for (int m = 0; m < O; ++m) {
+                        int t = rreg[k][m] + zoff;  // the column is rotated by whole cells
+                        if (t >= NzPv) t -= NzPv;
+                        u0[k][m] = cell < nv ? tile[t + cell * O + m] : 0.0;
                     }
-                };
-                for (int cell0 = 0; cell0 < nv; cell0 += 32) {
-                    const int cell = cell0 + lane;
-                    const bool valid = cell < nv;
-                    int c0 = cell + s;
-                    if (c0 >= nv) c0 -= nv;
-                    int c1 = c0 + 1;
-                    if (c1 >= nv) c1 -= nv;
-                    double u0[O], u1[O], r[O];
+                }
 #pragma unroll
-                    for (int m = 0; m < O; ++m) u0[m] = 0.0;
-                    if (valid) load_cell(c0, u0);
-                    // the right source cell of this lane's target is the left source cell of the next lane's
+                for (int k = 0; k < CPL; ++k) {
+                    const int cell = lane + 32 * k;
+                    double u1[O];
 #pragma unroll
-                    for (int m = 0; m < O; ++m) u1[m] = __shfl_down_sync(0xffffffffu, u0[m], 1);
-                    if (valid && (lane == 31 || cell + 1 >= nv)) load_cell(c1, u1);
-                    if (!valid) continue;
-#pragma unroll
-                    for (int j = 0; j < O; ++j) {
-                        double acc = 0.0;
-#pragma unroll
-                        for (int m = 0; m < O; ++m) acc = fma(A[j][m], u0[m], acc);
-#pragma unroll
-                        for (int m = 0; m < O; ++m) acc = fma(B[j][m], u1[m], acc);
-                        r[j] = acc;
+                    for (int m = 0; m < O; ++m) {
+                        const double dn = __shfl_down_sync(0xffffffffu, u0[k][m], 1);
+                        const double fnext = __shfl_sync(0xffffffffu, u0[(k + 1) % CPL][m], 0);
+                        const double fzero = __shfl_sync(0xffffffffu, u0[0][m], 0);
+                        u1[m] = (cell + 1 == nv) ? fzero : (lane == 31 ? fnext : dn);
                     }
-                    if (O == 2) {
-                        __stcs(reinterpret_cast<double2 *>(w + 2 * cell), make_double2(r[0], r[O - 1]));
-                    } else {
+                    if (cell < nv) {
+                        int c = cell - s;  // the target whose left source cell this is
+                        if (c < 0) c += nv;
+                        double r[O];
 #pragma unroll
-                        for (int j = 0; j < O; ++j) __stcs(w + cell * O + j, r[j]);
+                        for (int j = 0; j < O; ++j) {
+                            double acc = 0.0;
+#pragma unroll
+                            for (int m = 0; m < O; ++m) acc = fma(A[j][m], u0[k][m], acc);
+#pragma unroll
+                            for (int m = 0; m < O; ++m) acc = fma(B[j][m], u1[m], acc);
+                            r[j] = acc;
+                        }
+                        if (O == 2) {
+                            __stcs(reinterpret_cast<double2 *>(w + 2 * c), make_double2(r[0], r[O - 1]));
+                        } else {
+#pragma unroll
+                            for (int j = 0; j < O; ++j) __stcs(w + c * O + j, r[j]);
+                        }
                     }
                 }
             }
