@@ -341,7 +341,7 @@ __device__ __forceinline__ int geometry_setup(const double *__restrict__ va, con
     sh.mask[c] = 0;
 
     // step 4: node feet and adjoint polynomials in centred coordinates (relative to the anchor cell)
-    double Vi[O2][O2], xc = 0.0, yc = 0.0;
+    double xc = 0.0, yc = 0.0;
     {
         double fx[O2], fy[O2];
 #pragma unroll
@@ -357,7 +357,7 @@ __device__ __forceinline__ int geometry_setup(const double *__restrict__ va, con
             }
         xc *= 1.0 / O2;
         yc *= 1.0 / O2;
-        if (O == 3) {
+        if constexpr (O == 3) {
             // Vandermonde matrix straight into this cell's column of sh.Vi, inverted there in place
 #pragma unroll
             for (int m = 0; m < O2; ++m) {
@@ -375,11 +375,8 @@ __device__ __forceinline__ int geometry_setup(const double *__restrict__ va, con
             }
             const double minpiv = invert_in_place<O2>(&sh.Vi[0][c], SH::CELLS);  // Vi[ab][m] = (V^-1)[ab][m]
             if (!(minpiv > 1e-10)) atomicMin(err, SLDG_EGEOM);
-            sh.xc[c] = xc;
-            sh.yc[c] = yc;
-            return (nr + 1) * (ns + 1);
-        }
-        double V[O2][O2];
+        } else {
+        double V[O2][O2], Vi[O2][O2];
 #pragma unroll
         for (int m = 0; m < O2; ++m) {
             double py = 1.0;
@@ -398,13 +395,14 @@ __device__ __forceinline__ int geometry_setup(const double *__restrict__ va, con
         }
         const double minpiv = gauss_jordan<O2>(V, Vi);  // phi*_m = sum_ab Vi[ab][m] (x-xc)^a (y-yc)^b
         if (!(minpiv > 1e-10)) atomicMin(err, SLDG_EGEOM);
+#pragma unroll
+        for (int ab = 0; ab < O2; ++ab)
+#pragma unroll
+            for (int m = 0; m < O2; ++m) sh.Vi[ab * O2 + m][c] = Vi[ab][m];
+        }
     }
     sh.xc[c] = xc;
     sh.yc[c] = yc;
-#pragma unroll
-    for (int ab = 0; ab < O2; ++ab)
-#pragma unroll
-        for (int m = 0; m < O2; ++m) sh.Vi[ab * O2 + m][c] = Vi[ab][m];
     return (nr + 1) * (ns + 1);
 }
 
