@@ -71,7 +71,9 @@ __host__ __device__ inline size_t fused_table_bytes(int Nz, int Pv, int O)
     return (size_t)Nz * 2 * O * O * 8 + (size_t)Pv * 2 * O * O * 8 + (size_t)Nz * 4 + (size_t)Pv * 8 + 64;
 }
 
-template <int O, int CPL, bool ZFIRST>
+// ZONLY (with ZFIRST = false): the z sweep alone through the same planes -- for Courant numbers so different from
+// one v node to the next that the column walk of advect_z_kernel reads a different z row in almost every lane.
+template <int O, int CPL, bool ZFIRST, bool ZONLY>
 __global__ void __launch_bounds__(FUSED_BLOCK, 1) fused_sweep_kernel(const double *__restrict__ fin,
                                                                        double *__restrict__ fout,
                                                                        const double *__restrict__ Ez, GridDev g,
@@ -121,7 +123,7 @@ __global__ void __launch_bounds__(FUSED_BLOCK, 1) fused_sweep_kernel(const doubl
 
     // staging by bulk copies (TMA), issued by the producer warp, completing on mbarriers: line l of a plane ->
     // tile + l * Pv.  bars: full_L[2], full_H, done (all compute warps are through with a plane)
-    uint64_t *bars = reinterpret_cast<uint64_t *>(zs + Pv + (Pv & 1));  // 8-byte aligned
+    uint64_t *bars = reinterpret_cast<uint64_t *>((reinterpret_cast<uintptr_t>(zs + Pv) + 7) & ~(uintptr_t)7);  // 8-byte aligned (Nz, Pv may be odd)
     if (tid == 0) {
         for (int k = 0; k < 3; ++k) mbar_init(&bars[k], 1);
         mbar_init(&bars[3], FUSED_THREADS / 32);
@@ -169,14 +171,14 @@ __global__ void __launch_bounds__(FUSED_BLOCK, 1) fused_sweep_kernel(const doubl
     double ez_next = 0.0;
     int col = blockIdx.x, par = 0;
     uint32_t phL[2] = {0, 0}, phH = 0;
-    if (col < ncol && tid < Nz) ez_next = __ldg(Ez + tid * plane_nodes + col);
+    if (!ZONLY && col < ncol && tid < Nz) ez_next = __ldg(Ez + tid * plane_nodes + col);
     for (; col < ncol; col += gridDim.x, par ^= 1) {
         double *tile = buf + (par ? NL * Pv : 0);
         const int ncolx = col + (int)gridDim.x;
         const double ez_cur = ez_next;
-        if (ncolx < ncol && tid < Nz) ez_next = __ldg(Ez + tid * plane_nodes + ncolx);
+        if (!ZONLY && ncolx < ncol && tid < Nz) ez_next = __ldg(Ez + tid * plane_nodes + ncolx);
         // ---- per line the (s, A, B) of its v shift (under the copies) ------------------------------------------
-        if (tid < Nz) {
+        if (!ZONLY && tid < Nz) {
             int s;
             double alpha, A[O][O], B[O][O];
             shift_of(ez_cur, tau_v, g.h[3], s, alpha);
@@ -194,7 +196,7 @@ __global__ void __launch_bounds__(FUSED_BLOCK, 1) fused_sweep_kernel(const doubl
             mbar_wait(&bars[par], phL[par]);
             phL[par] ^= 1;
         }
-        if (ZFIRST && NH > 0) {  // the z sweep needs every line; the v sweep (VZ) starts on the L lines
+        if ((ZFIRST || ZONLY) && NH > 0) {  // the z sweep needs every line; the v sweep (VZ) starts on the L lines
             mbar_wait(&bars[2], phH);
             phH ^= 1;
         }
@@ -320,7 +322,7 @@ __global__ void __launch_bounds__(FUSED_BLOCK, 1) fused_sweep_kernel(const doubl
             // ---- phase A: v sweep in place, warp <-> line; first the L lines (fetched one plane ahead), then,
             //      once they have arrived, the H lines ---------------------------------------------------------
 #pragma unroll 1
-            for (int pass = 0; pass < 2; ++pass) {
+            for (int pass = 0; pass < (ZONLY ? 0 : 2); ++pass) {
             const int cnt = pass ? NH : NL;
             const int base = pass ? (par ? 0 : NL) : (par ? NH : 0);
             if (pass && NH > 0) {
@@ -440,12 +442,14 @@ __global__ void __launch_bounds__(FUSED_BLOCK, 1) fused_sweep_kernel(const doubl
 
 // The pair (z then v, or v then z) in one pass; returns cudaErrorNotSupported when the (z,v) plane does not fit
 // (the caller then runs the two separate kernels).
-cudaError_t launch_fused_sweeps(sldg_ctx *c, const double *fin, double *fout, double tau_z, double tau_v, bool z_first)
+cudaError_t launch_fused_sweeps(sldg_ctx *c, const double *fin, double *fout, double tau_z, double tau_v, bool z_first,
+                                bool z_only)
 {
+    if (z_only) z_first = false;
     const GridDev &g = c->g;
     const int O = g.o[2];
-    if (g.o[3] != O) return cudaErrorNotSupported;
-    if (g.Pv > FUSED_THREADS || g.n[3] > 32 * FUSED_MAXCPL) return cudaErrorNotSupported;
+    if (!z_only && g.o[3] != O) return cudaErrorNotSupported;
+    if (g.Pv > FUSED_THREADS || (!z_only && g.n[3] > 32 * FUSED_MAXCPL)) return cudaErrorNotSupported;
     const int Nz = g.N[2];
     const size_t tables = fused_table_bytes(Nz, g.Pv, O), row = (size_t)g.Pv * 8;
     const size_t budget = 227 * 1024 - 1024;
@@ -455,15 +459,16 @@ cudaError_t launch_fused_sweeps(sldg_ctx *c, const double *fin, double *fout, do
     // z first: the z sweep cannot start before the whole plane is there, so the lines that do not fit beside the
     // current plane (NH = Nz - NL, fetched only when it is done) are fully exposed; measured at 144 x 144 (o = 3,
     // NL = 0.28 Nz) the pair is then slower than the two separate kernels.  v first hides them under its L lines.
-    if (z_first && 2 * NL < Nz) return cudaErrorNotSupported;
+    if ((z_first || z_only) && 2 * NL < Nz) return cudaErrorNotSupported;
     const size_t smem = tables + row * (size_t)(2 * NL + (Nz - NL));
     const bool cpl2 = g.n[3] <= 64;
     const int ncol = g.N[0] * g.N[1];
     const int grid = ncol < c->sm_count ? ncol : c->sm_count;
 #define LAUNCH_F(OO)                                                                                              \
     do {                                                                                                          \
-        auto kern = z_first ? (cpl2 ? fused_sweep_kernel<OO, 2, true> : fused_sweep_kernel<OO, 4, true>)  \
-                            : (cpl2 ? fused_sweep_kernel<OO, 2, false> : fused_sweep_kernel<OO, 4, false>); \
+        auto kern = z_only ? fused_sweep_kernel<OO, 2, false, true>                                               \
+                  : z_first ? (cpl2 ? fused_sweep_kernel<OO, 2, true, false> : fused_sweep_kernel<OO, 4, true, false>) \
+                            : (cpl2 ? fused_sweep_kernel<OO, 2, false, false> : fused_sweep_kernel<OO, 4, false, false>); \
         cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);                       \
         kern<<<grid, FUSED_BLOCK, smem, c->stream>>>(fin, fout, c->Ez, g, c->sp_z, c->sp_v, c->basis, tau_z,    \
                                                        tau_v, NL);                                                \

@@ -3,6 +3,9 @@
 //
 // Internal layout: v fastest.  Element (z,Y,X,v) lives at z*sZ + Y*sY + X*sX + v; every (z,Y,X) "line"
 // of Nv doubles is contiguous and starts on a 128-byte boundary (pitch Pv).
+#include <math.h>
+#include <stdlib.h>
+
 #include "sldg_internal.cuh"
 #include "sldg_sweep_common.cuh"
 
@@ -262,6 +265,19 @@ cudaError_t launch_advect_z(sldg_ctx *c, const double *fin, double *fout, double
 {
     const GridDev &g = c->g;
     const int O = g.o[2];
+    {
+        // The Courant number grows linearly with the v node.  When it changes by more than ~2 cells across the 32 v
+        // nodes of a warp, the lanes of the column walk below read different z rows (scattered 8-24 byte runs:
+        // measured 7.1 ms instead of 2.6 ms at |CFL| = 20, configs[2]): the plane-tiled kernel of sldg_fused_sweeps.cu
+        // does the same sweep (same arithmetic, bit-identical) with every row read whole.
+        const double dv_warp = 32.0 * g.h[3] / g.o[3];
+        const double spread = fabs(dv_warp * tau / g.h[2]);
+        if (spread > 2.0 && !getenv("SLDG_ADVECT_Z_COLUMNS")) {
+            cudaError_t e = launch_fused_sweeps(c, fin, fout, tau, 0.0, false, true);
+            if (e != cudaErrorNotSupported) return e;
+            cudaGetLastError();
+        }
+    }
     const long long nthreads = (long long)g.N[1] * g.N[0] * g.Pv;
     const long long nblk = (nthreads + 255) / 256;
     if (nblk >= (1ll << 31)) return cudaErrorInvalidValue;

@@ -100,6 +100,32 @@ def test_advect_v_parity(torch, name, cfl):
         assert _rel(got, ref) <= TOL
 
 
+@pytest.mark.parametrize("name", list(SPECS))
+def test_advect_z_plane_kernel_is_bit_identical_to_the_column_walk(torch, monkeypatch, name):
+    """Large Courant numbers (configs[2]: |CFL| = 20) send sldg_advect_z through the plane-tiled kernel (every z row read
+    whole) instead of the per-column walk; same arithmetic, so the results must agree bit for bit."""
+    spec = SPECS[name]
+    rng = np.random.default_rng(17)
+    f = rng.random(spec.shape)
+    tau = 20.0 * spec.h[2] / max(abs(spec.lo[3]), abs(spec.hi[3]))
+    outs = []
+    for columns in (False, True):
+        if columns:
+            monkeypatch.setenv("SLDG_ADVECT_Z_COLUMNS", "1")
+        else:
+            monkeypatch.delenv("SLDG_ADVECT_Z_COLUMNS", raising=False)
+        s = _sldg(spec)
+        s.import_state(_dev(torch, f))
+        n0 = s.launch_count()
+        s.advect_z(tau)
+        s.advect_z(-0.37 * tau)
+        outs.append(s.export_state().cpu().numpy())
+        s.check()
+        s.close()
+    assert np.array_equal(outs[0], outs[1])
+    assert _rel(outs[0], oracle.advect_z(spec, oracle.advect_z(spec, f, tau), -0.37 * tau)) <= TOL
+
+
 def test_integer_courant_numbers_are_bit_exact(torch):
     """A(0) = I, B(0) = 0: integer shifts copy the data with wrap, bit for bit (both sweeps)."""
     spec = GridSpec(n=(3, 2, 6, 8), order=(2, 2, 2, 1), lo=(0, 0, 0.0, -4.0), hi=(1, 1, 6.0, 4.0))
