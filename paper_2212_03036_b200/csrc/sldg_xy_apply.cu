@@ -170,7 +170,7 @@ __global__ void __launch_bounds__(128) xy_stageable_kernel(const int4 *__restric
 template <int O, int VSPLIT>
 __global__ void __launch_bounds__(32 * (StreamCfg<O>::TX * VSPLIT + 1), 1) xy_apply_stream_kernel(
     const double *__restrict__ fin, double *__restrict__ fout, const int4 *__restrict__ hdrg,
-    const double *__restrict__ W, GridDev g, int L, const int32_t *__restrict__ stage_ok)
+    const double *__restrict__ W, GridDev g, int L, const int32_t *__restrict__ stage_ok, int vend)
 {
     if (!stage_ok[blockIdx.z * gridDim.x + blockIdx.x]) return;  // the direct kernel handles this block
     using Cfg = StreamCfg<O>;
@@ -193,7 +193,7 @@ __global__ void __launch_bounds__(32 * (StreamCfg<O>::TX * VSPLIT + 1), 1) xy_ap
     const int rows = min(L, ny - j0);
     const int z = blockIdx.z;
     const int v0 = blockIdx.y * STREAM_VMAX;
-    const int VL = min(STREAM_VMAX, g.Pv - v0);  // multiple of 16
+    const int VL = min(STREAM_VMAX, vend - v0);  // multiple of 16; this kernel covers the v values [0, vend)
     const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
     const long long ncell = (long long)nx * ny;
     const long long zc = (long long)z * ncell;
@@ -438,7 +438,8 @@ __global__ void __launch_bounds__(256, 2) xy_apply_direct_kernel(const double *_
                                                               double *__restrict__ fout,
                                                               const int4 *__restrict__ hdrg,
                                                               const double *__restrict__ W, GridDev g,
-                                                              const int32_t *__restrict__ stage_ok, int L, int stx)
+                                                              const int32_t *__restrict__ stage_ok, int L, int stx,
+                                                              int vbeg, int vend)
 {
     constexpr int O2 = O * O, TX = 8, TY = 4;
     const int nx = g.n[0], ny = g.n[1];
@@ -460,11 +461,11 @@ __global__ void __launch_bounds__(256, 2) xy_apply_direct_kernel(const double *_
         rh = min(TY, ny - rj0);
     }
     const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
-    const int v = blockIdx.y * 32 * NV + lane;
-    if (v >= g.Pv) return;
+    const int v = vbeg + blockIdx.y * 32 * NV + lane;  // this launch covers the v values [vbeg, vend)
+    if (v >= vend) return;
     int nve = 0;  // values of this lane inside the line
 #pragma unroll
-    for (int e = 0; e < NV; ++e) nve += (v + 32 * e < g.Pv) ? 1 : 0;
+    for (int e = 0; e < NV; ++e) nve += (v + 32 * e < vend) ? 1 : 0;
     const long long ncell = (long long)nx * ny;
     const double *fz = fin + z * g.sZ + v;
     double *oz = fout + z * g.sZ + v;
@@ -529,58 +530,70 @@ size_t xy_apply_stage_flags(const sldg_params *p)
     return strips * segs * (size_t)p->n[2] * p->order[2];
 }
 
-cudaError_t launch_xy_apply(sldg_ctx *c, const double *fin, double *fout)
+// one launch of the direct kernel over the v values [vbeg, vend): all cells (flags == nullptr, grid of 8 x 4 tiles) or
+// only the cells of the non-stageable streaming blocks (grid of the streaming kernel)
+static void launch_direct(sldg_ctx *c, const double *fin, double *fout, const int32_t *flags, int L, int nblk_x, int vbeg,
+                          int vend)
 {
     const GridDev &g = c->g;
-    const int O = g.o[0];
-    const int tiles = ((g.n[0] + 7) / 8) * ((g.n[1] + 3) / 4);
-    // direct kernel, values per lane: as many as cover the line in one chunk, at most 5 (45 accumulators at o = 3)
-    int nv = (g.Pv + 31) / 32;
+    const int O = g.o[0], stx = stream_tx(O), span = vend - vbeg;
+    // values per lane: as many as cover the range in one chunk, at most 5 (45 accumulators at o = 3)
+    int nv = (span + 31) / 32;
     if (nv > 5) nv = 4;
-    const int vchunks = (g.Pv + 32 * nv - 1) / (32 * nv);
-    dim3 dgrid((unsigned)tiles, (unsigned)vchunks, (unsigned)g.N[2]);
-    const int32_t *flags = nullptr;
-    int L = 0;
-    const int stx = stream_tx(O);
+    const int vchunks = (span + 32 * nv - 1) / (32 * nv);
+    dim3 dgrid((unsigned)nblk_x, (unsigned)vchunks, (unsigned)g.N[2]);
 #define LAUNCH_A(OO, NN) \
-    xy_apply_direct_kernel<OO, NN><<<dgrid, 256, 0, c->stream>>>(fin, fout, c->hdr, c->W, g, flags, L, stx)
+    xy_apply_direct_kernel<OO, NN><<<dgrid, 256, 0, c->stream>>>(fin, fout, c->hdr, c->W, g, flags, L, stx, vbeg, vend)
 #define LAUNCH_AN(OO)                                                                                         \
     do {                                                                                                      \
         if (nv == 1) LAUNCH_A(OO, 1); else if (nv == 2) LAUNCH_A(OO, 2); else if (nv == 3) LAUNCH_A(OO, 3);   \
         else if (nv == 4) LAUNCH_A(OO, 4); else LAUNCH_A(OO, 5);                                              \
     } while (0)
+    if (O == 1) LAUNCH_AN(1); else if (O == 2) LAUNCH_AN(2); else LAUNCH_AN(3);
+#undef LAUNCH_AN
+#undef LAUNCH_A
+    c->launches++;
+}
+
+cudaError_t launch_xy_apply(sldg_ctx *c, const double *fin, double *fout)
+{
+    const GridDev &g = c->g;
+    const int O = g.o[0];
+    const int tiles = ((g.n[0] + 7) / 8) * ((g.n[1] + 3) / 4);
     if (xy_apply_streams(O)) {
         // Which blocks can stream is decided on the device (scan of the headers); the streaming kernel does
         // those, the direct kernel the others (none in an ITG step; most of them in a solid-body rotation, where the
         // anchors change by many cells along a strip).  No host synchronisation.
         static const int vsplit = getenv("SLDG_APPLY_VSPLIT") ? atoi(getenv("SLDG_APPLY_VSPLIT")) : 1;
-        L = stream_segment_rows(g.n[1]);
+        const int stx = stream_tx(O);
+        const int L = stream_segment_rows(g.n[1]);
         const int strips = (g.n[0] + stx - 1) / stx, segs = (g.n[1] + L - 1) / L;
-        const int VL = g.Pv < STREAM_VMAX ? g.Pv : STREAM_VMAX;
+        // v chunks of the streaming kernel.  A last chunk with fewer than 64 values (Pv = 144 at o = 3: 128 + 16) would
+        // keep a whole block busy for as long as a full chunk -- its lanes are mostly idle, its FMAs are not fewer --
+        // and double the kernel's time: that remainder goes to the direct kernel instead.
+        int vstream = g.Pv;
+        if (g.Pv > STREAM_VMAX && g.Pv % STREAM_VMAX != 0 && g.Pv % STREAM_VMAX < 64) vstream = g.Pv - g.Pv % STREAM_VMAX;
+        const int VL = vstream < STREAM_VMAX ? vstream : STREAM_VMAX;
         const size_t ring = O == 3 ? StreamCfg<3>::RING : StreamCfg<2>::RING;
         xy_stageable_kernel<<<dim3((unsigned)(strips * segs), (unsigned)g.N[2]), 128, 0, c->stream>>>(
             c->hdr, g, L, VL, stx, ring, c->stage_ok, c->err);
-        dim3 grid((unsigned)(strips * segs), (unsigned)((g.Pv + STREAM_VMAX - 1) / STREAM_VMAX), (unsigned)g.N[2]);
+        dim3 grid((unsigned)(strips * segs), (unsigned)((vstream + STREAM_VMAX - 1) / STREAM_VMAX), (unsigned)g.N[2]);
 #define LAUNCH_S(OO, VS)                                                                                      \
     do {                                                                                                      \
         auto kern = xy_apply_stream_kernel<OO, VS>;                                                           \
         cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)stream_smem_bytes<OO>()); \
         kern<<<grid, 32 * (StreamCfg<OO>::TX * VS + 1), stream_smem_bytes<OO>(), c->stream>>>(                \
-            fin, fout, c->hdr, c->W, g, L, c->stage_ok);                                                      \
+            fin, fout, c->hdr, c->W, g, L, c->stage_ok, vstream);                                             \
     } while (0)
         if (O == 3) LAUNCH_S(3, 2);
         else if (vsplit == 1) LAUNCH_S(2, 1);
         else LAUNCH_S(2, 2);
 #undef LAUNCH_S
-        flags = c->stage_ok;
-        dgrid = dim3((unsigned)(strips * segs), (unsigned)vchunks, (unsigned)g.N[2]);
-        if (O == 3) LAUNCH_AN(3); else LAUNCH_AN(2);
-        c->launches += 3;
+        c->launches += 2;
+        launch_direct(c, fin, fout, c->stage_ok, L, strips * segs, 0, vstream);  // the non-stageable blocks
+        if (vstream < g.Pv) launch_direct(c, fin, fout, nullptr, 0, tiles, vstream, g.Pv);  // the short last chunk
         return cudaGetLastError();
     }
-    if (O == 1) LAUNCH_AN(1); else if (O == 2) LAUNCH_AN(2); else LAUNCH_AN(3);
-#undef LAUNCH_AN
-#undef LAUNCH_A
-    c->launches++;
+    launch_direct(c, fin, fout, nullptr, 0, tiles, 0, g.Pv);
     return cudaGetLastError();
 }
