@@ -433,7 +433,8 @@ __global__ void __launch_bounds__(32 * (StreamCfg<O>::TX * VSPLIT + 1), 1) xy_ap
 // --------------------------------------------------------------------------------------------------
 // stage_ok != nullptr (filtered): the grid is that of the streaming kernel, a block does the cells of one streaming
 // block (strip of stx columns, segment of L rows, z node) if that block is NOT stageable, and nothing otherwise.
-template <int O, int NV>
+// HALF (NV = 1, at most 16 v values): the two half-warps take two different cells.
+template <int O, int NV, bool HALF = false>
 __global__ void __launch_bounds__(256, 2) xy_apply_direct_kernel(const double *__restrict__ fin,
                                                               double *__restrict__ fout,
                                                               const int4 *__restrict__ hdrg,
@@ -461,7 +462,7 @@ __global__ void __launch_bounds__(256, 2) xy_apply_direct_kernel(const double *_
         rh = min(TY, ny - rj0);
     }
     const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
-    const int v = vbeg + blockIdx.y * 32 * NV + lane;  // this launch covers the v values [vbeg, vend)
+    const int v = vbeg + (HALF ? (lane & 15) : blockIdx.y * 32 * NV + lane);  // this launch covers [vbeg, vend)
     if (v >= vend) return;
     int nve = 0;  // values of this lane inside the line
 #pragma unroll
@@ -470,7 +471,7 @@ __global__ void __launch_bounds__(256, 2) xy_apply_direct_kernel(const double *_
     const double *fz = fin + z * g.sZ + v;
     double *oz = fout + z * g.sZ + v;
 
-    for (int c = warp; c < rw * rh; c += 8) {
+    for (int c = HALF ? 2 * warp + (lane >> 4) : warp; c < rw * rh; c += HALF ? 16 : 8) {
         const int i = ri0 + (c % rw), j = rj0 + (c / rw);
         const long long cellid = (long long)z * ncell + (long long)j * nx + i;
         const int4 h = __ldcg(hdrg + cellid);
@@ -549,7 +550,10 @@ static void launch_direct(sldg_ctx *c, const double *fin, double *fout, const in
         if (nv == 1) LAUNCH_A(OO, 1); else if (nv == 2) LAUNCH_A(OO, 2); else if (nv == 3) LAUNCH_A(OO, 3);   \
         else if (nv == 4) LAUNCH_A(OO, 4); else LAUNCH_A(OO, 5);                                              \
     } while (0)
-    if (O == 1) LAUNCH_AN(1); else if (O == 2) LAUNCH_AN(2); else LAUNCH_AN(3);
+    if (span <= 16 && O == 3) {
+        xy_apply_direct_kernel<3, 1, true><<<dgrid, 256, 0, c->stream>>>(fin, fout, c->hdr, c->W, g, flags, L, stx, vbeg,
+                                                                         vend);
+    } else if (O == 1) LAUNCH_AN(1); else if (O == 2) LAUNCH_AN(2); else LAUNCH_AN(3);
 #undef LAUNCH_AN
 #undef LAUNCH_A
     c->launches++;
