@@ -433,8 +433,9 @@ __global__ void __launch_bounds__(32 * (StreamCfg<O>::TX * VSPLIT + 1), 1) xy_ap
 // --------------------------------------------------------------------------------------------------
 // stage_ok != nullptr (filtered): the grid is that of the streaming kernel, a block does the cells of one streaming
 // block (strip of stx columns, segment of L rows, z node) if that block is NOT stageable, and nothing otherwise.
-// HALF (NV = 1, at most 16 v values): the two half-warps take two different cells.
-template <int O, int NV, bool HALF = false>
+// CPW > 1 (a remainder of at most 16 v values): CPW cells per warp, 32 / CPW lanes per cell, the lane's values at
+// stride 32 / CPW.
+template <int O, int NV, int CPW = 1>
 __global__ void __launch_bounds__(256, 2) xy_apply_direct_kernel(const double *__restrict__ fin,
                                                               double *__restrict__ fout,
                                                               const int4 *__restrict__ hdrg,
@@ -462,16 +463,17 @@ __global__ void __launch_bounds__(256, 2) xy_apply_direct_kernel(const double *_
         rh = min(TY, ny - rj0);
     }
     const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
-    const int v = vbeg + (HALF ? (lane & 15) : blockIdx.y * 32 * NV + lane);  // this launch covers [vbeg, vend)
+    constexpr int LPC = 32 / CPW;  // lanes per cell
+    const int v = vbeg + blockIdx.y * LPC * NV + lane % LPC;  // this launch covers [vbeg, vend)
     if (v >= vend) return;
     int nve = 0;  // values of this lane inside the line
 #pragma unroll
-    for (int e = 0; e < NV; ++e) nve += (v + 32 * e < vend) ? 1 : 0;
+    for (int e = 0; e < NV; ++e) nve += (v + LPC * e < vend) ? 1 : 0;
     const long long ncell = (long long)nx * ny;
     const double *fz = fin + z * g.sZ + v;
     double *oz = fout + z * g.sZ + v;
 
-    for (int c = HALF ? 2 * warp + (lane >> 4) : warp; c < rw * rh; c += HALF ? 16 : 8) {
+    for (int c = CPW * warp + lane / LPC; c < rw * rh; c += 8 * CPW) {
         const int i = ri0 + (c % rw), j = rj0 + (c / rw);
         const long long cellid = (long long)z * ncell + (long long)j * nx + i;
         const int4 h = __ldcg(hdrg + cellid);
@@ -498,7 +500,7 @@ __global__ void __launch_bounds__(256, 2) xy_apply_direct_kernel(const double *_
                     const double *src = fz + (long long)(s * O + kq) * g.sY + (long long)(r * O + kp) * g.sX;
                     double in[NV];
 #pragma unroll
-                    for (int e = 0; e < NV; ++e) in[e] = e < nve ? __ldg(src + 32 * e) : 0.0;
+                    for (int e = 0; e < NV; ++e) in[e] = e < nve ? __ldg(src + LPC * e) : 0.0;
                     const int k = kp + O * kq;
 #pragma unroll
                     for (int m = 0; m < O2; ++m) {
@@ -516,7 +518,7 @@ __global__ void __launch_bounds__(256, 2) xy_apply_direct_kernel(const double *_
                 const int m = mp + O * mq;
 #pragma unroll
                 for (int e = 0; e < NV; ++e)
-                    if (e < nve) __stcs(dst + 32 * e, acc[m][e]);
+                    if (e < nve) __stcs(dst + LPC * e, acc[m][e]);
             }
     }
 }
@@ -551,8 +553,8 @@ static void launch_direct(sldg_ctx *c, const double *fin, double *fout, const in
         else if (nv == 4) LAUNCH_A(OO, 4); else LAUNCH_A(OO, 5);                                              \
     } while (0)
     if (span <= 16 && O == 3) {
-        xy_apply_direct_kernel<3, 1, true><<<dgrid, 256, 0, c->stream>>>(fin, fout, c->hdr, c->W, g, flags, L, stx, vbeg,
-                                                                         vend);
+        dgrid.y = 1;
+        xy_apply_direct_kernel<3, 2, 4><<<dgrid, 256, 0, c->stream>>>(fin, fout, c->hdr, c->W, g, flags, L, stx, vbeg, vend);
     } else if (O == 1) LAUNCH_AN(1); else if (O == 2) LAUNCH_AN(2); else LAUNCH_AN(3);
 #undef LAUNCH_AN
 #undef LAUNCH_A
