@@ -21,43 +21,10 @@
 //   VZ      phase A  v sweep in place, warp <-> line (all sources of a warp's line are in registers before the
 //                    first write);
 //           phase B  z sweep, thread <-> (v, slice of z), results straight to global memory.
+#include "sldg_async.cuh"
 #include "sldg_sweep_common.cuh"
 
 namespace {
-
-// ---- mbarrier / bulk-copy primitives (PTX) --------------------------------------------------------
-__device__ __forceinline__ uint32_t smem_u32(const void *p) { return (uint32_t)__cvta_generic_to_shared(p); }
-__device__ __forceinline__ void mbar_init(uint64_t *bar, uint32_t count)
-{
-    asm volatile("mbarrier.init.shared::cta.b64 [%0], %1;" ::"r"(smem_u32(bar)), "r"(count) : "memory");
-}
-__device__ __forceinline__ void mbar_fence_init() { asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory"); }
-__device__ __forceinline__ void mbar_arrive(uint64_t *bar)
-{
-    asm volatile("mbarrier.arrive.shared::cta.b64 _, [%0];" ::"r"(smem_u32(bar)) : "memory");
-}
-__device__ __forceinline__ void mbar_arrive_expect_tx(uint64_t *bar, uint32_t bytes)
-{
-    asm volatile("mbarrier.arrive.expect_tx.shared::cta.b64 _, [%0], %1;" ::"r"(smem_u32(bar)), "r"(bytes) : "memory");
-}
-__device__ __forceinline__ void bulk_g2s(void *dst, const void *src, uint32_t bytes, uint64_t *bar)
-{
-    asm volatile("cp.async.bulk.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1], %2, [%3];" ::"r"(
-                     smem_u32(dst)),
-                 "l"(src), "r"(bytes), "r"(smem_u32(bar))
-                 : "memory");
-}
-__device__ __forceinline__ void mbar_wait(uint64_t *bar, uint32_t parity)
-{
-    uint32_t ok;
-    do {
-        asm volatile(
-            "{\n.reg .pred p;\nmbarrier.try_wait.parity.shared::cta.b64 p, [%1], %2;\nselp.u32 %0, 1, 0, p;\n}"
-            : "=r"(ok)
-            : "r"(smem_u32(bar)), "r"(parity)
-            : "memory");
-    } while (!ok);
-}
 
 constexpr int FUSED_THREADS = 512;          // compute threads (16 warps)
 constexpr int FUSED_BLOCK = FUSED_THREADS + 32;  // + one producer warp
@@ -431,7 +398,7 @@ __global__ void __launch_bounds__(FUSED_BLOCK, 1) fused_sweep_kernel(const doubl
                 }
             }
         }
-        asm volatile("fence.proxy.async.shared::cta;" ::: "memory");  // generic writes before the next bulk copies
+        fence_proxy_async();  // generic writes before the next bulk copies
         __syncwarp();
         if (lane == 0) mbar_arrive(&bars[3]);
         compute_sync();  // the per-line tables are free for the next plane
@@ -451,6 +418,8 @@ cudaError_t launch_fused_sweeps(sldg_ctx *c, const double *fin, double *fout, do
     if (!z_only && g.o[3] != O) return cudaErrorNotSupported;
     if (g.Pv > FUSED_THREADS || (!z_only && g.n[3] > 32 * FUSED_MAXCPL)) return cudaErrorNotSupported;
     const int Nz = g.N[2];
+    // the per-line tables of the v shift (vs, vAB, the E_z prefetch) are filled by thread <-> line
+    if (!z_only && Nz > FUSED_THREADS) return cudaErrorNotSupported;
     const size_t tables = fused_table_bytes(Nz, g.Pv, O), row = (size_t)g.Pv * 8;
     const size_t budget = 227 * 1024 - 1024;
     if (tables + row * Nz > budget) return cudaErrorNotSupported;

@@ -22,47 +22,13 @@
 //   xy_apply_direct_kernel (any o): warp <-> target cell, inputs through L1; does the blocks that cannot stream.
 #include <stdlib.h>
 
+#include "sldg_async.cuh"
 #include "sldg_internal.cuh"
-#include "sldg_xy_geometry.cuh"
 
 __device__ __forceinline__ int wrap_idx(int i, int n)
 {
     int r = i % n;
     return r < 0 ? r + n : r;
-}
-
-// ---- mbarrier / bulk-copy primitives (PTX) --------------------------------------------------------
-__device__ __forceinline__ uint32_t smem_u32(const void *p) { return (uint32_t)__cvta_generic_to_shared(p); }
-__device__ __forceinline__ void mbar_init(uint64_t *bar, uint32_t count)
-{
-    asm volatile("mbarrier.init.shared::cta.b64 [%0], %1;" ::"r"(smem_u32(bar)), "r"(count) : "memory");
-}
-__device__ __forceinline__ void mbar_fence_init() { asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory"); }
-__device__ __forceinline__ void mbar_arrive(uint64_t *bar)
-{
-    asm volatile("mbarrier.arrive.shared::cta.b64 _, [%0];" ::"r"(smem_u32(bar)) : "memory");
-}
-__device__ __forceinline__ void mbar_arrive_expect_tx(uint64_t *bar, uint32_t bytes)
-{
-    asm volatile("mbarrier.arrive.expect_tx.shared::cta.b64 _, [%0], %1;" ::"r"(smem_u32(bar)), "r"(bytes) : "memory");
-}
-__device__ __forceinline__ void bulk_g2s(void *dst, const void *src, uint32_t bytes, uint64_t *bar)
-{
-    asm volatile("cp.async.bulk.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1], %2, [%3];" ::"r"(
-                     smem_u32(dst)),
-                 "l"(src), "r"(bytes), "r"(smem_u32(bar))
-                 : "memory");
-}
-__device__ __forceinline__ void mbar_wait(uint64_t *bar, uint32_t parity)
-{
-    uint32_t ok;
-    do {
-        asm volatile(
-            "{\n.reg .pred p;\nmbarrier.try_wait.parity.shared::cta.b64 p, [%1], %2;\nselp.u32 %0, 1, 0, p;\n}"
-            : "=r"(ok)
-            : "r"(smem_u32(bar)), "r"(parity)
-            : "memory");
-    } while (!ok);
 }
 
 // One source cell's contribution for NP v pairs per lane (pair p at v = 64 p + 2 lane): o^2 inputs (k), o^4
@@ -489,9 +455,7 @@ __global__ void __launch_bounds__(256, 2) xy_apply_direct_kernel(const double *_
 #pragma unroll 1
         for (int slot = 0; slot < 9; ++slot) {
             if (!((msk >> slot) & 1)) continue;
-            int r = ax + slot % 3, s = ay + slot / 3;
-            if (r >= nx) r -= nx;
-            if (s >= ny) s -= ny;
+            const int r = wrap_idx(ax + slot % 3, nx), s = wrap_idx(ay + slot / 3, ny);  // nx, ny may be < 3
             const double *Wp = W + ((size_t)cellid * 9 + nb++) * sldg_w_block_doubles(O);
 #pragma unroll
             for (int kq = 0; kq < O; ++kq)

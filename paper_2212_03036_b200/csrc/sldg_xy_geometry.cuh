@@ -1,5 +1,5 @@
-// sldg_xy_geometry.cuh -- device code of the 2d geometry (eq. 14-18), shared by the stand-alone geometry kernel
-// (sldg_xy_geometry.cu) and the apply kernel that computes the geometry of its own strip (sldg_xy_apply.cu).
+// sldg_xy_geometry.cuh -- device code of the 2d geometry (eq. 14-18) used by the geometry kernel
+// of sldg_xy_geometry.cu: tracing, adjoint polynomials, clipping, Green's-theorem moments, contraction.
 #pragma once
 #include "sldg_internal.cuh"
 

@@ -1,0 +1,278 @@
+"""Parity of the CUDA path against the CPU oracle at every BASELINE.json config's OWN step count (north_star:
+"relative L-infinity error <= 1e-11 after each config's step count"), on the same seeded inputs, through the C-ABI.
+
+  configs[0]  16x16x8x16 cells, 20 Strang steps                      -> tests/test_gpu_parity.py::test_config0_...
+  configs[1]  256x256 cells, o = 2 and 3, a seeded subset of 256 of the 4096 planes (the planes are independent and
+              share one velocity field): solid-body rotation for the full 40 steps (clamped
+              half-step lookup) and the swirling deformation flow for the full 30 steps with the field re-evaluated
+              at t^{n+1/2} every step
+  configs[2]  128x128x64x64 cells at full size: sampled z lines after advect_z at max |CFL| 20 and sampled v lines
+              after advect_v at max |CFL| 2.5 with the seeded Fourier E_z, against oracle.shift_line; and all 50
+              sweeps of each on a reduced (x,y) grid (16x16x64x64 cells) against the full oracle
+  configs[3]  200 Strang steps at dt = 4 on 64x64 (x,y) cells with fewer z and v cells (64x64x4x16), state compared
+              after 50, 100 and 200 steps, mass every 10 steps.  (The full 64x64x32x64 grid over 200 steps is run once
+              by tests/full_config_parity.py through gpurun; its error curve is profiles/r02_c3_parity.md.)
+  configs[4]  50 Strang steps at dt = 4, o = 2 on 128x128 (x,y) cells and o = 3 on 96x96 cells, with fewer z and v
+              cells (the full-size single step on sampled outputs is tests/test_gpu_full_size.py)
+
+The reduced grids keep the (x,y) resolution, the box, the profiles, dt and the prescribed fields of the config: the
+2d step (whose oracle costs seconds per step) sees exactly the config's geometry; only the number of z and v cells
+shrinks, so that the oracle finishes inside the driver's time limit for the GPU tests.
+"""
+import math
+
+import numpy as np
+import pytest
+
+import oracle
+from paper_2212_03036_b200 import inputs
+
+pytestmark = pytest.mark.gpu
+
+TOL = 1e-11
+
+
+@pytest.fixture(scope="module")
+def torch():
+    import torch as t
+    if not t.cuda.is_available():
+        pytest.skip("needs a CUDA device")
+    return t
+
+
+def _sldg(spec):
+    from paper_2212_03036_b200.binding import Sldg
+    return Sldg(spec)
+
+
+def _dev(torch, x):
+    return torch.from_numpy(np.ascontiguousarray(x)).cuda()
+
+
+def _rel(got, ref):
+    return float(np.abs(got - ref).max() / np.abs(ref).max())
+
+
+# ------------------------------------------------------------------------------------------------ configs[1]
+C1_PLANES = 256
+
+
+def _c1_inputs(o):
+    full = inputs.bumps_grid(256, 4096, o)
+    sel = np.sort(np.random.default_rng(101).choice(4096, size=C1_PLANES, replace=False))
+    f = inputs.bumps_initial_f(full, seed=1, plane_slice=sel)
+    spec = inputs.bumps_grid(256, C1_PLANES, o)
+    assert f.shape == spec.shape
+    return spec, f
+
+
+@pytest.mark.parametrize("o", [2, 3])
+def test_config1_rotation_full_period_40_steps(torch, o):
+    spec, f = _c1_inputs(o)
+    a, b = inputs.rotation_velocity(spec)
+    tau = 2.0 * math.pi / 40
+    s = _sldg(spec)
+    s.import_state(_dev(torch, f))
+    s.set_vxy(_dev(torch, a), _dev(torch, b), 0)
+    ref = f
+    worst = 0.0
+    for n in range(40):
+        s.advect_xy(tau, 2)
+        ref = oracle.advect_xy(spec, ref, a, b, tau, 2, 0)
+        if n in (0, 9, 19, 29, 39):
+            worst = max(worst, _rel(s.export_state().cpu().numpy(), ref))
+            assert worst <= TOL, (n, worst)
+    s.check()
+    # one period of a solid-body rotation returns the bumps to where they started, to discretisation accuracy
+    # (each step projects; SURVEY.md 8(c)-2 pin (vi)) -- the GPU path itself, not only the oracle
+    got = s.export_state().cpu().numpy()
+    assert np.abs(got - f).max() < (0.08 if o == 2 else 0.02)
+    m0, m1 = oracle.mass(spec, f), float(s.mass().cpu()[0])
+    assert abs(m1 - oracle.mass(spec, ref)) <= 1e-13 * abs(m0)
+    s.close()
+
+
+@pytest.mark.parametrize("o", [2, 3])
+def test_config1_swirl_30_steps_field_at_half_steps(torch, o):
+    spec, f = _c1_inputs(o)
+    tau = 0.05
+    s = _sldg(spec)
+    s.import_state(_dev(torch, f))
+    ref = f
+    m0 = oracle.mass(spec, f)
+    for n in range(30):
+        a, b = inputs.swirl_velocity(spec, (n + 0.5) * tau)  # the caller evaluates the field at t^{n+1/2} (R8)
+        s.set_vxy(_dev(torch, a), _dev(torch, b), 1)
+        s.advect_xy(tau, 2)
+        ref = oracle.advect_xy(spec, ref, a, b, tau, 2, 1)
+        if n in (0, 9, 19, 29):
+            err = _rel(s.export_state().cpu().numpy(), ref)
+            assert err <= TOL, (n, err)
+    s.check()
+    m1 = float(s.mass().cpu()[0])
+    assert abs(m1 - m0) <= 1e-13 * abs(m0)  # periodic field: the upstream mesh tiles, mass to round-off
+    s.close()
+
+
+# ------------------------------------------------------------------------------------------------ configs[2]
+def test_config2_full_size_sampled_lines(torch):
+    """128x128x64x64 cells: z sweep at max |CFL| = 20 (plane-tiled kernel), v sweep with the Fourier E_z at max
+    |CFL| = 2.5 (multi-cell shifts), each checked on 64 whole lines the oracle computes one by one."""
+    if torch.cuda.get_device_properties(0).total_memory < 60e9:
+        pytest.skip("needs 60 GB of device memory")
+    spec = inputs.itg_grid(128, 128, 64, 64, 2)
+    Nz, Nv, Ny, Nx = spec.shape
+    f0 = inputs.sweeps_initial_f(spec, seed=3)
+    Ez = inputs.fourier_Ez(spec, seed=2)
+    dtz, dtv = inputs.sweeps_dt_z(spec, 20.0), inputs.sweeps_dt_v(spec, Ez, 2.5)
+    s = _sldg(spec)
+    s.import_state_host(f0)
+    s.set_Ez(_dev(torch, Ez))
+    o = 2
+    xi, _ = oracle.gl(o)
+    rng = np.random.default_rng(12)
+    scale = np.abs(f0).max()
+
+    def view():
+        cur = s.f_a if s.current_ptr() == s.f_a.data_ptr() else s.f_b
+        Pv = s.state_bytes // 8 // (Nz * Ny * Nx)
+        return cur.view(Nz, Ny, Nx, Pv)
+
+    m0 = float(s.mass().cpu()[0])
+    n0 = s.launch_count()
+    s.advect_z(dtz)
+    s.check()
+    V = view()
+    shifts = set()
+    for k in range(64):
+        v = (0, Nv - 1, 1, Nv // 2)[k] if k < 4 else int(rng.integers(Nv))  # the extreme Courant numbers included
+        y, x = int(rng.integers(Ny)), int(rng.integers(Nx))
+        vq = spec.lo[3] + (v // o + xi[v % o]) * spec.h[3]
+        delta = vq * dtz / spec.h[2]
+        shifts.add(int(math.floor(-delta)))
+        ref = oracle.shift_line(f0[:, v, y, x].copy(), o, delta)
+        got = V[:, y, x, v].cpu().numpy()
+        assert np.abs(got - ref).max() <= TOL * scale, ("z", v, y, x)
+    assert min(shifts) <= -20 and max(shifts) >= 19  # |CFL| = 20 really reached, in both directions
+    samples = [(int(rng.integers(Nz)), int(rng.integers(Ny)), int(rng.integers(Nx))) for _ in range(60)]
+    flat = np.argsort(np.abs(Ez).ravel())[-4:]  # plus the four lines with the largest |E_z| (|CFL| ~ 2.5)
+    samples += [tuple(int(c) for c in np.unravel_index(i, Ez.shape)) for i in flat]
+    lines_in = [V[z, y, x, :Nv].cpu().numpy().copy() for (z, y, x) in samples]
+    s.advect_v(dtv)
+    s.check()
+    V = view()
+    big = 0
+    for (z, y, x), u in zip(samples, lines_in):
+        delta = Ez[z, y, x] * dtv / spec.h[3]
+        big += abs(delta) > 1.0
+        ref = oracle.shift_line(u, o, delta)
+        got = V[z, y, x, :Nv].cpu().numpy()
+        assert np.abs(got - ref).max() <= TOL * scale, ("v", z, y, x)
+    assert big >= 4
+    m1 = float(s.mass().cpu()[0])
+    assert abs(m1 - m0) <= 1e-13 * abs(m0)
+    assert s.launch_count() - n0 >= 2
+    s.close()
+
+
+def test_config2_50_sweeps_each_on_reduced_xy(torch):
+    """All 50 z sweeps (max |CFL| 20) and 50 v sweeps (Fourier E_z, max |CFL| 2.5) of configs[2] with its 64x64 (z,v)
+    cells, on 16x16 (x,y) cells so that the oracle finishes in seconds."""
+    spec = inputs.itg_grid(16, 16, 64, 64, 2)
+    f = inputs.sweeps_initial_f(spec, seed=3)
+    Ez = inputs.fourier_Ez(spec, seed=2)
+    dtz, dtv = inputs.sweeps_dt_z(spec, 20.0), inputs.sweeps_dt_v(spec, Ez, 2.5)
+    s = _sldg(spec)
+    s.import_state(_dev(torch, f))
+    s.set_Ez(_dev(torch, Ez))
+    ref = f
+    m0 = oracle.mass(spec, f)
+    for n in range(50):
+        s.advect_z(dtz)
+        s.advect_v(dtv)
+        ref = oracle.advect_v(spec, oracle.advect_z(spec, ref, dtz), Ez, dtv)
+        if n in (0, 24, 49):
+            err = _rel(s.export_state().cpu().numpy(), ref)
+            assert err <= TOL, (n, err)
+    s.check()
+    assert abs(float(s.mass().cpu()[0]) - m0) <= 1e-13 * abs(m0)
+    s.close()
+
+
+# ------------------------------------------------------------------------------------- configs[3], configs[4]
+def _itg_run(torch, cells, o, dt, steps, checkpoints):
+    spec = inputs.itg_grid(*cells, o)
+    f = inputs.itg_initial_f(spec)
+    a, b, Ez, _ = inputs.itg_fields(spec, dt, 0.8)
+    s = _sldg(spec)
+    s.import_state(_dev(torch, f))
+    s.set_Ez(_dev(torch, Ez))
+    s.set_vxy(_dev(torch, a), _dev(torch, b), 1)
+    ref = f.copy()
+    tmp = np.empty_like(ref)
+    m0 = oracle.mass(spec, f)
+    errs, drift = {}, 0.0
+    for n in range(1, steps + 1):
+        s.strang_step(dt)
+        oracle.strang_step(spec, ref, Ez, a, b, dt, 2, 1, tmp=tmp)
+        if n % 10 == 0:
+            drift = max(drift, abs(float(s.mass().cpu()[0]) - m0) / abs(m0))
+        if n in checkpoints:
+            errs[n] = _rel(s.export_state().cpu().numpy(), ref)
+    s.check()
+    rho = s.charge_density().cpu().numpy()
+    err_rho = _rel(rho, oracle.charge_density(spec, ref))
+    s.close()
+    return errs, drift, err_rho
+
+
+def test_config3_200_strang_steps_state_parity(torch):
+    errs, drift, err_rho = _itg_run(torch, (64, 64, 4, 16), 2, 4.0, 200, (50, 100, 200))
+    assert set(errs) == {50, 100, 200}
+    assert max(errs.values()) <= TOL, errs
+    assert err_rho <= TOL
+    assert drift <= 1e-13, drift
+
+
+@pytest.mark.parametrize("o,cells", [(2, (128, 128, 2, 4)), (3, (96, 96, 1, 2))])
+def test_config4_50_strang_steps_state_parity(torch, o, cells):
+    errs, drift, err_rho = _itg_run(torch, cells, o, 4.0, 50, (10, 25, 50))
+    assert max(errs.values()) <= TOL, errs
+    assert err_rho <= TOL
+    assert drift <= 1e-13, drift
+
+
+def test_fused_pairs_with_more_than_512_z_lines_equal_separate_sweeps(torch, monkeypatch):
+    """Nz = 600 z lines with a short v axis still fits the shared-memory budget of the fused sweep pairs; their
+    per-line tables are filled by thread <-> line over 512 threads.  Whatever path sldg_strang_step
+    takes, the state must equal the five separate calls bit for bit, and match the oracle."""
+    spec = inputs.itg_grid(2, 2, 300, 8, 2)
+    rng = np.random.default_rng(31)
+    f = rng.random(spec.shape)
+    dt = 2.0
+    a, b, Ez, _ = inputs.itg_fields(spec, dt, 0.6)
+    Ez = Ez * (1.7 * spec.h[3] / (0.5 * dt) / max(np.abs(Ez).max(), 1e-300))
+    outs = []
+    for fuse in (True, False):
+        if fuse:
+            monkeypatch.delenv("SLDG_NO_FUSE", raising=False)
+        else:
+            monkeypatch.setenv("SLDG_NO_FUSE", "1")
+        s = _sldg(spec)
+        s.import_state(_dev(torch, f))
+        s.set_Ez(_dev(torch, Ez))
+        s.set_vxy(_dev(torch, a), _dev(torch, b), 1)
+        if fuse:
+            s.strang_step(dt)
+        else:
+            s.advect_z(0.5 * dt)
+            s.advect_v(0.5 * dt)
+            s.advect_xy(dt, 2)
+            s.advect_v(0.5 * dt)
+            s.advect_z(0.5 * dt)
+        s.check()
+        outs.append(s.export_state().cpu().numpy())
+        s.close()
+    assert np.array_equal(outs[0], outs[1])
+    ref = oracle.strang_step(spec, f.copy(), Ez, a, b, dt, 2, 1)
+    assert _rel(outs[0], ref) <= TOL

@@ -498,3 +498,37 @@ def test_geometry_error_words(torch):
         s.check()
     assert ei.value.code == SLDG_ESTENCIL
     s.check()  # cleared
+
+
+def test_geometry_error_egeom_both_ways(torch):
+    """SLDG_EGEOM, provoked both ways, and the oracle raises on the same
+    input: (i) crossed characteristics -- a field converging so strongly that Euler's foot map (1 - tau k) x flips the
+    orientation of every upstream cell; (ii) a singular Vandermonde system -- one Euler step of the solid rotation
+    with tau = 1 turns the Q^1 node feet by 45 degrees onto the axes through their centre, where the monomial xy
+    vanishes at all four of them.  A slightly smaller step (tau = 0.9) is fine on both sides."""
+    from paper_2212_03036_b200.binding import SLDG_EGEOM, SldgError
+    spec = GridSpec(n=(8, 8, 1, 2), order=(2, 2, 1, 1), lo=(-1, -1, 0, 0), hi=(1, 1, 1, 1))
+    XV, YV = np.meshgrid(spec.vertex_coords(0), spec.vertex_coords(1), indexing="xy")
+    rng = np.random.default_rng(13)
+    f = rng.random(spec.shape)
+    cases = [((1.5 * XV)[None], np.zeros((1, 9, 9)), 1.0), ((-YV)[None], XV[None].copy(), 1.0)]
+    for a, b, tau in cases:
+        with pytest.raises(oracle.OracleError):
+            oracle.advect_xy(spec, f, a, b, tau, 1, 0)
+        s = _sldg(spec)
+        s.import_state(_dev(torch, f))
+        s.set_vxy(_dev(torch, a), _dev(torch, b), 0)
+        s.advect_xy(tau, 1)
+        with pytest.raises(SldgError) as ei:
+            s.check()
+        assert ei.value.code == SLDG_EGEOM
+        s.check()  # cleared
+        s.close()
+    a, b, _ = cases[1]
+    s = _sldg(spec)
+    s.import_state(_dev(torch, f))
+    s.set_vxy(_dev(torch, a), _dev(torch, b), 0)
+    s.advect_xy(0.9, 1)
+    s.check()
+    assert _rel(s.export_state().cpu().numpy(), oracle.advect_xy(spec, f, a, b, 0.9, 1, 0)) <= TOL
+    s.close()

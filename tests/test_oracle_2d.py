@@ -237,6 +237,98 @@ def test_trace_periodic_images_agree():
             assert np.abs(bot - (top - np.array([0.0, 1.0]))).max() < 3e-16
 
 
+def _np_bilinear(a, b, ci, cj, xi, eta):
+    """Velocity of the bilinear patch of cell (ci, cj) at local (xi, eta) -- also OUTSIDE [0,1]^2 (extrapolation)."""
+    w = np.array([(1 - xi) * (1 - eta), xi * (1 - eta), (1 - xi) * eta, xi * eta])
+    va = np.array([a[cj, ci], a[cj, ci + 1], a[cj + 1, ci], a[cj + 1, ci + 1]])
+    vb = np.array([b[cj, ci], b[cj, ci + 1], b[cj + 1, ci], b[cj + 1, ci + 1]])
+    return float(w @ va), float(w @ vb)
+
+
+def _np_midpoint_foot_clamped(spec, a, b, i, j, xi, eta, tau):
+    """eq. (15) as explicit midpoint, written out: half-step point -> the grid cell that contains
+    it, its index CLAMPED to the box, the local coordinates taken relative to that clamped
+    cell (so the patch is extrapolated when the point lies outside the box) -> foot.  Returns (foot relative to cell
+    (i,j) in cell units, whether the clamp was active)."""
+    nx, ny = spec.n[0], spec.n[1]
+    hx, hy = spec.h[0], spec.h[1]
+    ua, ub = _np_bilinear(a, b, i, j, xi, eta)
+    mx, my = xi - 0.5 * tau * ua / hx, eta - 0.5 * tau * ub / hy  # half-step point, relative to cell (i,j)
+    gi, gj = i + math.floor(mx), j + math.floor(my)              # the cell that contains it (unclamped)
+    ci, cj = min(max(gi, 0), nx - 1), min(max(gj, 0), ny - 1)
+    ua, ub = _np_bilinear(a, b, ci, cj, (i + mx) - ci, (j + my) - cj)
+    return np.array([xi - tau * ua / hx, eta - tau * ub / hy]), (ci != gi or cj != gj)
+
+
+def test_trace_clamped_half_step_lookup_outside_the_box():
+    """The vel_periodic = 0 branch of the tracing (the path of config 1's rotation) when the half-step point LEAVES
+    the box: the cell index is clamped and the boundary cell's bilinear patch is extrapolated.
+    (i) Solid rotation: every patch reproduces u = (-y, x) exactly, also extrapolated, so the foot is the closed form
+        (I - tau J + tau^2 J^2 / 2) X even though the half-step point is outside.
+    (ii) A random non-periodic field (no patch reproduces it): the foot equals the definition written out in numpy;
+        a wrong clamp offset, or local coordinates not re-based on the clamped cell, fail this.
+    Points are boundary cells on all four sides and the four corner cells, tau large enough to leave the box."""
+    spec = inputs.bumps_grid(12, 1, 2)
+    nx = ny = 12
+    hx, hy = spec.h[0], spec.h[1]
+    J = np.array([[0.0, -1.0], [1.0, 0.0]])
+    a, b = inputs.rotation_velocity(spec)
+    tau = 0.9  # a boundary point at |X| ~ pi moves by ~1.4 = 2.7 cells in the half step
+    pts = [(0, 5, 0.0, 0.3), (11, 6, 1.0, 0.7), (4, 0, 0.2, 0.0), (7, 11, 0.6, 1.0), (0, 0, 0.0, 0.0), (11, 11, 1.0, 1.0),
+           (0, 11, 0.1, 0.9), (11, 0, 0.9, 0.1)]
+    left = 0
+    for (i, j, xi, eta) in pts:
+        X = np.array([spec.lo[0] + (i + xi) * hx, spec.lo[1] + (j + eta) * hy])
+        foot = oracle.trace(spec, a[0], b[0], i, j, xi, eta, tau, 2, 0)
+        phys = np.array([spec.lo[0] + (i + foot[0]) * hx, spec.lo[1] + (j + foot[1]) * hy])
+        assert np.abs(phys - (np.eye(2) - tau * J + 0.5 * tau ** 2 * J @ J) @ X).max() < 2e-14
+        _, clamped = _np_midpoint_foot_clamped(spec, a[0], b[0], i, j, xi, eta, tau)
+        left += clamped
+    assert left >= 6  # the half-step point really left the box
+    rng = np.random.default_rng(44)
+    a = rng.uniform(-1.0, 1.0, size=(ny + 1, nx + 1))
+    b = rng.uniform(-1.0, 1.0, size=(ny + 1, nx + 1))
+    left = 0
+    for tau in (0.4, 1.3, 2.6):
+        for i in range(nx):
+            for j in range(ny):
+                if 1 < i < nx - 2 and 1 < j < ny - 2:
+                    continue  # boundary cells (two layers) only
+                for (xi, eta) in ((0.0, 0.0), (1.0, 1.0), (0.2113, 0.7887)):
+                    ref, clamped = _np_midpoint_foot_clamped(spec, a, b, i, j, xi, eta, tau)
+                    got = oracle.trace(spec, a, b, i, j, xi, eta, tau, 2, 0)
+                    assert np.abs(got - ref).max() < 1e-13, (tau, i, j, xi, eta)
+                    left += clamped
+    assert left > 50
+
+
+def test_trace_linear_field_closed_form_midpoint():
+    """Any affine field u = M X + c is reproduced exactly by the bilinear patches, so the explicit-midpoint foot is
+    X - tau (M (X - tau/2 (M X + c)) + c) in closed form and Euler's is X - tau (M X + c): pins eq. (14)/(15)
+    independently of the solid rotation (shear, strain, non-zero divergence), periodic lookup off and on where
+    the point stays inside the box."""
+    spec = inputs.bumps_grid(10, 1, 3)
+    hx, hy = spec.h[0], spec.h[1]
+    xv, yv = spec.vertex_coords(0), spec.vertex_coords(1)
+    XV, YV = np.meshgrid(xv, yv, indexing="xy")
+    rng = np.random.default_rng(45)
+    for _ in range(4):
+        M = rng.uniform(-0.6, 0.6, size=(2, 2))
+        c = rng.uniform(-0.3, 0.3, size=2)
+        a = M[0, 0] * XV + M[0, 1] * YV + c[0]
+        b = M[1, 0] * XV + M[1, 1] * YV + c[1]
+        tau = 0.2
+        for (i, j, xi, eta) in [(4, 5, 0.0, 1.0), (3, 6, 0.1127, 0.5), (6, 2, 0.8873, 0.8873), (5, 5, 1.0, 0.0)]:
+            X = np.array([spec.lo[0] + (i + xi) * hx, spec.lo[1] + (j + eta) * hy])
+            euler = X - tau * (M @ X + c)
+            mid = X - tau * (M @ (X - 0.5 * tau * (M @ X + c)) + c)
+            for order, exact in ((1, euler), (2, mid)):
+                for periodic in (0, 1):
+                    foot = oracle.trace(spec, a, b, i, j, xi, eta, tau, order, periodic)
+                    phys = np.array([spec.lo[0] + (i + foot[0]) * hx, spec.lo[1] + (j + foot[1]) * hy])
+                    assert np.abs(phys - exact).max() < 1e-14, (order, periodic, i, j)
+
+
 # ----------------------------------------------------------------------------- plane geometry
 def _periodic_random_velocity(spec, seed, amp):
     nx, ny = spec.n[0], spec.n[1]
