@@ -144,7 +144,13 @@ int sldg_debug_geometry(sldg_ctx *ctx, int z, int32_t *anchor_dev, int32_t *mask
  *   0: blocks (strip x segment x z node) of the 2d apply whose source window does not fit the streaming kernel's
  *      shared-memory ring (anchors varying by many cells inside the block, more than 3 source rows per target
  *      row) and were handed to the direct kernel instead. */
+/*   1: non-empty weight blocks (target cell, source cell) of the last sldg_advect_xy, summed over all z nodes: the 2d
+ *      apply does 2 o^4 flops per block and v node (eq. 17; PAPER.md:378-382 counts the dense 3x3 case). */
 int sldg_debug_counter(sldg_ctx *ctx, int which, long long *value_host);
+/* Measures the device's fp64 FMA throughput (independent FMA chains, every SM busy), best of `repeats` launches, in
+ * TFLOP/s: the roof of the ALU-bound kernels (the paper's intensity argument).
+ * Synchronises. */
+int sldg_debug_fp64_peak(sldg_ctx *ctx, int repeats, double *tflops_host);
 const char *sldg_strerror(int code);
 
 #ifdef __cplusplus

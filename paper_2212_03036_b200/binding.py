@@ -21,7 +21,7 @@ EXPORTS = [
     "sldg_set_Ez", "sldg_set_vxy", "sldg_advect_z", "sldg_advect_v", "sldg_advect_xy",
     "sldg_charge_density", "sldg_mass", "sldg_strang_step", "sldg_set_trace_order",
     "sldg_strang_step_host", "sldg_check", "sldg_last_timing_ms", "sldg_launch_count",
-    "sldg_debug_geometry", "sldg_debug_counter", "sldg_strerror",
+    "sldg_debug_geometry", "sldg_debug_counter", "sldg_debug_fp64_peak", "sldg_strerror",
 ]
 
 
@@ -79,6 +79,7 @@ def load_library():
     L.sldg_launch_count.restype = C.c_longlong
     L.sldg_debug_geometry.argtypes = [vp, C.c_int, ip, ip, dp]
     L.sldg_debug_counter.argtypes = [vp, C.c_int, C.POINTER(C.c_longlong)]
+    L.sldg_debug_fp64_peak.argtypes = [vp, C.c_int, C.POINTER(C.c_double)]
     L.sldg_strerror.argtypes = [C.c_int]
     L.sldg_strerror.restype = C.c_char_p
     _lib = L
@@ -232,6 +233,12 @@ class Sldg:
         v = C.c_longlong(0)
         self._chk(self.L.sldg_debug_counter(self.h, int(which), C.byref(v)), "sldg_debug_counter")
         return int(v.value)
+
+    def debug_fp64_peak(self, repeats=5):
+        """Measured fp64 FMA throughput of the device in TFLOP/s (the roof of the ALU-bound kernels)."""
+        v = C.c_double(0.0)
+        self._chk(self.L.sldg_debug_fp64_peak(self.h, int(repeats), C.byref(v)), "sldg_debug_fp64_peak")
+        return float(v.value)
 
     def debug_geometry(self, z):
         t = self.torch

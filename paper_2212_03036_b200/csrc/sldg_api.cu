@@ -583,7 +583,8 @@ int sldg_debug_geometry(sldg_ctx *c, int z, int32_t *anchor_dev, int32_t *mask_d
 
 int sldg_debug_counter(sldg_ctx *c, int which, long long *value_host)
 {
-    if (!c || !value_host || which != 0) return SLDG_EINVAL;
+    if (!c || !value_host || which < 0 || which > 1) return SLDG_EINVAL;
+    if (which == 1) return cuda_fail(count_weight_blocks(c, value_host));
     int32_t word = 0;
     if (cudaMemcpyAsync(&word, c->err + 1 + which, 4, cudaMemcpyDeviceToHost, c->stream) != cudaSuccess) return SLDG_ECUDA;
     if (cudaStreamSynchronize(c->stream) != cudaSuccess) return SLDG_ECUDA;

@@ -87,5 +87,6 @@ cudaError_t launch_xy_geometry(sldg_ctx *c, double tau, int trace_order);
 size_t xy_apply_stage_flags(const sldg_params *p);  // number of stage_ok entries
 cudaError_t launch_geometry_expand(sldg_ctx *c, int z, int32_t *anchor, int32_t *mask, double *Wd);
 cudaError_t launch_xy_apply(sldg_ctx *c, const double *fin, double *fout);
+cudaError_t count_weight_blocks(sldg_ctx *c, long long *total_host);
 cudaError_t launch_fused_sweeps(sldg_ctx *c, const double *fin, double *fout, double tau_z, double tau_v, bool z_first,
                                 bool z_only = false);
