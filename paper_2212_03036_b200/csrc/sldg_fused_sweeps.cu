@@ -32,15 +32,16 @@ constexpr int FUSED_MAXCPL = 4;  // v cells per lane in the line-wise phases (nv
 
 // dynamic shared memory: planes [2 NL + NH][Pv] doubles | per line: A, B of its v shift [Nz][2 O^2] doubles |
 // per column: A, B of its z shift [2 O^2][Pv] doubles | per line: s [Nz] ints | per column: rotation offset
-// [Pv] ints, z shift [Pv] ints
+// [Pv] ints, z shift [Pv] ints | barriers | z,v pair: line order per plane parity [2][Nz] shorts, marks [2][Nz] bytes
 __host__ __device__ inline size_t fused_table_bytes(int Nz, int Pv, int O)
 {
-    return (size_t)Nz * 2 * O * O * 8 + (size_t)Pv * 2 * O * O * 8 + (size_t)Nz * 4 + (size_t)Pv * 8 + 64;
+    return (size_t)Nz * 2 * O * O * 8 + (size_t)Pv * 2 * O * O * 8 + (size_t)Nz * 4 + (size_t)Pv * 8 + 64 +
+           (size_t)Nz * 6 + 16;  // + line order of the z,v pair's line-wise phase [2][Nz] shorts, marks [2][Nz] bytes
 }
 
 // ZONLY (with ZFIRST = false): the z sweep alone through the same planes -- for Courant numbers so different from
 // one v node to the next that the column walk of advect_z_kernel reads a different z row in almost every lane.
-template <int O, int CPL, bool ZFIRST, bool ZONLY>
+template <int O, int CPL, bool ZFIRST, bool ZONLY, bool FULLV>
 __global__ void __launch_bounds__(FUSED_BLOCK, 1) fused_sweep_kernel(const double *__restrict__ fin,
                                                                        double *__restrict__ fout,
                                                                        const double *__restrict__ Ez, GridDev g,
@@ -94,9 +95,41 @@ __global__ void __launch_bounds__(FUSED_BLOCK, 1) fused_sweep_kernel(const doubl
     if (tid == 0) {
         for (int k = 0; k < 3; ++k) mbar_init(&bars[k], 1);
         mbar_init(&bars[3], FUSED_THREADS / 32);
+        mbar_init(&bars[4], FUSED_THREADS / 32);  // z,v pair: the H rows of the current plane are no longer read
         mbar_fence_init();
     }
     __syncthreads();
+    // z,v pair: the line-wise phase reads line zr of column v from physical row (zr + s_z(v) O) mod Nz.  The lines that
+    // touch the H rows (the part of the tile the NEXT plane's late lines go to) are done first; once they are through,
+    // the producer fetches those late lines under the rest of the phase instead of after the plane.  order[p] = the
+    // lines of a plane of parity p in that order, n_early[p] = how many of them touch H.
+    short *order = reinterpret_cast<short *>(bars + 6);
+    unsigned char *mark = reinterpret_cast<unsigned char *>(order + 2 * Nz);
+    int *n_early = reinterpret_cast<int *>(bars + 5);
+    if (ZFIRST) {
+        for (int i = tid; i < 2 * Nz; i += FUSED_BLOCK) mark[i] = 0;
+        __syncthreads();
+        if (tid < Nv) {
+            const int rot = zs[tid] * O;
+            for (int r = 0; r < NH; ++r) {  // physical rows of H: NL + r in an even plane's tile, r in an odd plane's
+                int l0 = NL + r - rot, l1 = r - rot;
+                if (l0 < 0) l0 += Nz;
+                if (l1 < 0) l1 += Nz;
+                mark[l0] = 1;
+                mark[Nz + l1] = 1;
+            }
+        }
+        __syncthreads();
+        if (tid < 2) {
+            int n = 0;
+            for (int zr = 0; zr < Nz; ++zr)
+                if (mark[tid * Nz + zr]) order[tid * Nz + n++] = (short)zr;
+            n_early[tid] = n;
+            for (int zr = 0; zr < Nz; ++zr)
+                if (!mark[tid * Nz + zr]) order[tid * Nz + n++] = (short)zr;
+        }
+        __syncthreads();
+    }
     auto compute_sync = [&]() { asm volatile("bar.sync 1, %0;" ::"n"(FUSED_THREADS) : "memory"); };
     const uint32_t line_bytes = (uint32_t)Pv * 8;
     auto issue_lines = [&](int col, double *tl, int first, int count, uint64_t *bar) {  // producer warp only
@@ -109,31 +142,44 @@ __global__ void __launch_bounds__(FUSED_BLOCK, 1) fused_sweep_kernel(const doubl
     };
     if (warp == FUSED_THREADS / 32) {
         // ---------------- producer warp ------------------------------------------------------------------------
-        uint32_t phD = 0;
+        uint32_t phD = 0, phF = 0;
         int col = blockIdx.x, par = 0;
         if (col < ncol) issue_lines(col, buf, 0, NL, &bars[0]);  // L lines of the first (even) plane
+        if (ZFIRST && col < ncol) issue_lines(col, buf, NL, NH, &bars[2]);  // z,v: and its H lines
         for (bool first = true; col < ncol; col += gridDim.x, par ^= 1, first = false) {
             if (!first) {
-                mbar_wait(&bars[3], phD);  // the previous plane is done: H and the other L are free
+                mbar_wait(&bars[3], phD);  // the previous plane is done: (H and) the other L are free
                 phD ^= 1;
             }
             double *tile = buf + (par ? NL * Pv : 0);
             const int ncolx = col + (int)gridDim.x;
             // H lines of this plane: [NL,Nz) of an even plane, [0,NH) of an odd one
-            issue_lines(col, tile, par ? 0 : NL, NH, &bars[2]);
+            if (!ZFIRST) issue_lines(col, tile, par ? 0 : NL, NH, &bars[2]);
             // L lines of the next plane into the other L: [0,NL) of an even plane, [NH,Nz) of an odd one
             if (ncolx < ncol) issue_lines(ncolx, buf + (par ? 0 : NL * Pv), par ? 0 : NH, NL, &bars[par ^ 1]);
+            if (ZFIRST && NH > 0 && ncolx < ncol) {
+                // z,v: the H lines of the NEXT plane as soon as this plane's line-wise phase is through with the H rows
+                mbar_wait(&bars[4], phF);
+                issue_lines(ncolx, buf + (par ? 0 : NL * Pv), par ? NL : 0, NH, &bars[2]);
+            }
+            phF ^= 1;
         }
         return;
     }
 
-    int rreg[CPL][O];  // z,v pair: rotation offsets of this lane's columns in the line-wise phase
+    // z,v pair, line-wise phase: byte offset inside the plane tile of row 0 of this lane's columns after the in-place z
+    // sweep (column v ends up rotated by s_z(v) cells), for the lane's own source cell (left source of its target)
+    // and for the next cell (right source); the columns of a cell rotate independently (s_z depends on the v NODE)
+    uint32_t off0[CPL][O], off1[CPL][O];
 #pragma unroll
     for (int k = 0; k < CPL; ++k)
 #pragma unroll
         for (int m = 0; m < O; ++m) {
             const int cell = lane + 32 * k;
-            rreg[k][m] = (ZFIRST && cell < nv) ? rotoff[cell * O + m] : 0;
+            const int c0 = (ZFIRST && cell < nv) ? cell : 0;
+            const int c1 = (c0 + 1 == nv) ? 0 : c0 + 1;
+            off0[k][m] = ZFIRST ? (uint32_t)(rotoff[c0 * O + m] + c0 * O + m) * 8u : 0u;
+            off1[k][m] = ZFIRST ? (uint32_t)(rotoff[c1 * O + m] + c1 * O + m) * 8u : 0u;
         }
     double ez_next = 0.0;
     int col = blockIdx.x, par = 0;
@@ -225,45 +271,58 @@ __global__ void __launch_bounds__(FUSED_BLOCK, 1) fused_sweep_kernel(const doubl
                 step(last);  // the last target of the slice: its right source cell was read before the sweep
             }
             compute_sync();
-            // ---- phase B: v sweep of every line, to global memory.  lane <-> SOURCE cells (fixed columns, so the
-            //      rotation offsets of a lane's columns sit in registers); the right source cell of a target comes
-            //      from the neighbouring lane by shuffle; the lane stores target cell (source cell - s) ---------------
+            // ---- phase B: v sweep of every line, to global memory.  warp <-> line, lane <-> SOURCE cell c0 of the
+            //      target cell (c0 - s): its two source cells c0, c0 + 1 are read straight from the rotated columns
+            //      (explicit 32-bit shared addresses; the wrap of a rotated column is one unsigned min), no shuffles,
+            //      so lanes beyond nv simply skip ---------------------------------------------------------------------
+            const uint32_t tile_b = smem_u32(tile), vab_b = smem_u32(vAB), vs_b = smem_u32(vs);
+            const uint32_t plane_b = (uint32_t)NzPv * 8u, row_b = (uint32_t)Pv * 8u;
+            const uint32_t ord_b = smem_u32(order + par * Nz);
+            const int ne = n_early[par];
+            bool told = false;
 #pragma unroll 1
-            for (int zr = warp; zr < Nz; zr += FUSED_THREADS / 32) {
-                const int s = vs[zr];
-                double A[O][O], B[O][O];
-#pragma unroll
-                for (int j = 0; j < O; ++j)
-#pragma unroll
-                    for (int m = 0; m < O; ++m) {
-                        A[j][m] = vAB[(zr * 2) * O * O + j * O + m];
-                        B[j][m] = vAB[(zr * 2 + 1) * O * O + j * O + m];
-                    }
-                double *w = dst + zr * g.sZ;
-                const int zoff = zr * Pv;
-                double u0[CPL][O];
-#pragma unroll
-                for (int k = 0; k < CPL; ++k) {
-                    const int cell = lane + 32 * k;
-#pragma unroll
-                    for (int m = 0; m < O; ++m) {
-                        int t = rreg[k][m] + zoff;  // the column is rotated by whole cells
-                        if (t >= NzPv) t -= NzPv;
-                        u0[k][m] = cell < nv ? tile[t + cell * O + m] : 0.0;
-                    }
+            for (int idx = warp; idx < Nz; idx += FUSED_THREADS / 32) {
+                if (!told && idx >= ne) {  // this warp has read its last line that touches the H rows
+                    told = true;
+                    fence_proxy_async();
+                    __syncwarp();
+                    if (lane == 0) mbar_arrive(&bars[4]);
                 }
+                const int zr = lds_s16(ord_b + 2u * idx);
+                const int s = lds_s32(vs_b + 4u * zr);
+                double A[O][O], B[O][O];
+                {
+                    double ab[2 * O * O];
+                    const uint32_t at = vab_b + (uint32_t)zr * (2 * O * O * 8);
+#pragma unroll
+                    for (int e = 0; e < O * O; ++e) {
+                        const double2 t = lds_v2f64(at + 16u * e);
+                        ab[2 * e] = t.x;
+                        ab[2 * e + 1] = t.y;
+                    }
+#pragma unroll
+                    for (int j = 0; j < O; ++j)
+#pragma unroll
+                        for (int m = 0; m < O; ++m) {
+                            A[j][m] = ab[j * O + m];
+                            B[j][m] = ab[O * O + j * O + m];
+                        }
+                }
+                double *w = dst + zr * g.sZ;
+                const uint32_t zb = (uint32_t)zr * row_b;
 #pragma unroll
                 for (int k = 0; k < CPL; ++k) {
                     const int cell = lane + 32 * k;
-                    double u1[O];
+                    if (FULLV || cell < nv) {
+                        double u0[O], u1[O];
 #pragma unroll
-                    for (int m = 0; m < O; ++m) {
-                        const double dn = __shfl_down_sync(0xffffffffu, u0[k][m], 1);
-                        const double fnext = __shfl_sync(0xffffffffu, u0[(k + 1) % CPL][m], 0);
-                        const double fzero = __shfl_sync(0xffffffffu, u0[0][m], 0);
-                        u1[m] = (cell + 1 == nv) ? fzero : (lane == 31 ? fnext : dn);
-                    }
-                    if (cell < nv) {
+                        for (int m = 0; m < O; ++m) {
+                            uint32_t t0 = off0[k][m] + zb, t1 = off1[k][m] + zb;
+                            t0 = min(t0, t0 - plane_b);  // unsigned: subtracts the plane size exactly when t >= it
+                            t1 = min(t1, t1 - plane_b);
+                            u0[m] = lds_f64(tile_b + t0);
+                            u1[m] = lds_f64(tile_b + t1);
+                        }
                         int c = cell - s;  // the target whose left source cell this is
                         if (c < 0) c += nv;
                         double r[O];
@@ -271,7 +330,7 @@ __global__ void __launch_bounds__(FUSED_BLOCK, 1) fused_sweep_kernel(const doubl
                         for (int j = 0; j < O; ++j) {
                             double acc = 0.0;
 #pragma unroll
-                            for (int m = 0; m < O; ++m) acc = fma(A[j][m], u0[k][m], acc);
+                            for (int m = 0; m < O; ++m) acc = fma(A[j][m], u0[m], acc);
 #pragma unroll
                             for (int m = 0; m < O; ++m) acc = fma(B[j][m], u1[m], acc);
                             r[j] = acc;
@@ -284,6 +343,11 @@ __global__ void __launch_bounds__(FUSED_BLOCK, 1) fused_sweep_kernel(const doubl
                         }
                     }
                 }
+            }
+            if (!told) {
+                fence_proxy_async();
+                __syncwarp();
+                if (lane == 0) mbar_arrive(&bars[4]);
             }
         } else {
             // ---- phase A: v sweep in place, warp <-> line; first the L lines (fetched one plane ahead), then,
@@ -431,13 +495,18 @@ cudaError_t launch_fused_sweeps(sldg_ctx *c, const double *fin, double *fout, do
     if ((z_first || z_only) && 2 * NL < Nz) return cudaErrorNotSupported;
     const size_t smem = tables + row * (size_t)(2 * NL + (Nz - NL));
     const bool cpl2 = g.n[3] <= 64;
+    const bool fullv = g.n[3] == (cpl2 ? 64 : 128);  // every lane of the line-wise phase has all its cells
     const int ncol = g.N[0] * g.N[1];
     const int grid = ncol < c->sm_count ? ncol : c->sm_count;
 #define LAUNCH_F(OO)                                                                                              \
     do {                                                                                                          \
-        auto kern = z_only ? fused_sweep_kernel<OO, 2, false, true>                                               \
-                  : z_first ? (cpl2 ? fused_sweep_kernel<OO, 2, true, false> : fused_sweep_kernel<OO, 4, true, false>) \
-                            : (cpl2 ? fused_sweep_kernel<OO, 2, false, false> : fused_sweep_kernel<OO, 4, false, false>); \
+        auto kern = z_only ? fused_sweep_kernel<OO, 2, false, true, false>                                        \
+                  : z_first ? (cpl2 ? (fullv ? fused_sweep_kernel<OO, 2, true, false, true>                       \
+                                             : fused_sweep_kernel<OO, 2, true, false, false>)                     \
+                                    : (fullv ? fused_sweep_kernel<OO, 4, true, false, true>                       \
+                                             : fused_sweep_kernel<OO, 4, true, false, false>))                    \
+                            : (cpl2 ? fused_sweep_kernel<OO, 2, false, false, false>                              \
+                                    : fused_sweep_kernel<OO, 4, false, false, false>);                            \
         cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);                       \
         kern<<<grid, FUSED_BLOCK, smem, c->stream>>>(fin, fout, c->Ez, g, c->sp_z, c->sp_v, c->basis, tau_z,    \
                                                        tau_v, NL);                                                \

@@ -269,3 +269,36 @@ def fourier_Ez(spec: GridSpec, seed=2, modes=8, amplitude=0.5):
 
 def sweeps_dt_v(spec: GridSpec, Ez, cfl=2.5):
     return cfl * spec.h[3] / np.abs(Ez).max()
+
+
+# --------------------------------------------------------------------------------------------------
+# Swirling-deformation validation of the 2d step (Table 1)
+# --------------------------------------------------------------------------------------------------
+
+def paper_swirl_velocity(spec: GridSpec, t, period=1.5):
+    """The paper's swirling deformation flow on [-pi,pi]^2 at the cell vertices:
+    d_t u - d_x(cos^2(x/2) sin(y) g u) + d_y(sin(x) cos^2(y/2) g u) = 0,  g(t) = pi cos(pi t / T), i.e. the velocity
+    (a, b) = (-cos^2(x/2) sin y, sin x cos^2(y/2)) g(t).  Divergence free, no flow through the box boundary, reverses
+    at t = T/2 so that the exact solution at t = T is the initial condition."""
+    xv = spec.vertex_coords(0)
+    yv = spec.vertex_coords(1)
+    XV, YV = np.meshgrid(xv, yv, indexing="xy")
+    g = math.pi * math.cos(math.pi * t / period)
+    a = -np.cos(0.5 * XV) ** 2 * np.sin(YV) * g
+    b = np.sin(XV) * np.cos(0.5 * YV) ** 2 * g
+    for u in (a, b):  # 2 pi periodic: the wrap row/column bitwise equal (SURVEY.md 8(c) A15)
+        u[-1, :] = u[0, :]
+        u[:, -1] = u[:, 0]
+    return np.ascontiguousarray(a[None]), np.ascontiguousarray(b[None])
+
+
+def cosine_bell(spec: GridSpec, centre=(0.2 * math.pi, 0.3 * math.pi), radius=0.3 * math.pi):
+    """A C^5 cosine bell cos^6(pi r / 2R) for r < R (PAPER.md:303 names the regularity; centre and radius are in the
+    paper's ref. [2], which is not available: these are this build's choice).  Shape [1][Nv][Ny][Nx], every v plane
+    the same bell."""
+    x = spec.node_coords(0)
+    y = spec.node_coords(1)
+    X, Y = np.meshgrid(x, y, indexing="xy")
+    r = np.sqrt((X - centre[0]) ** 2 + (Y - centre[1]) ** 2)
+    bell = np.where(r < radius, np.cos(0.5 * math.pi * np.minimum(r, radius) / radius) ** 6, 0.0)
+    return np.ascontiguousarray(np.broadcast_to(bell[None, None], (1, spec.N[3], spec.N[1], spec.N[0])))
