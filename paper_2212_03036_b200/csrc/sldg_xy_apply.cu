@@ -69,9 +69,15 @@ __device__ __forceinline__ void fma_block(double (&acc)[O * O][2 * NP], const do
 // Per order: target cells per strip, weight stages (target rows), weight blocks per stage (TX cells x <= 9 blocks),
 // doubles per weight block in memory (o = 3: 81 padded to 82, bulk copies move multiples of 16 bytes), ring bytes.
 template <int O> struct StreamCfg;
+#ifndef SLDG_RING2_KB
+#define SLDG_RING2_KB 160
+#endif
+#ifndef SLDG_NW2
+#define SLDG_NW2 5
+#endif
 template <> struct StreamCfg<2> {
-    static constexpr int TX = 8, NW = 5, WROW = 72, WB = 16;
-    static constexpr size_t RING = 160 * 1024;
+    static constexpr int TX = 8, NW = SLDG_NW2, WROW = 72, WB = 16;
+    static constexpr size_t RING = SLDG_RING2_KB * 1024;
 };
 template <> struct StreamCfg<3> {
     static constexpr int TX = 4, NW = 4, WROW = 36, WB = 82;
