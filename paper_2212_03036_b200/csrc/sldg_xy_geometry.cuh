@@ -5,8 +5,10 @@
 
 namespace sldg_geom {
 
+// i modulo n in [0, n); the division (some 25 instructions) only when i is outside the box
 __device__ __forceinline__ int wrap_idx(int i, int n)
 {
+    if ((unsigned)i < (unsigned)n) return i;
     int r = i % n;
     return r < 0 ? r + n : r;
 }
@@ -170,17 +172,13 @@ __device__ __forceinline__ double invert_in_place(double *a, int stride)
     return minpiv;
 }
 
-// Per-cell description of the upstream quadrilateral's edges (corners counter-clockwise, target-cell
-// units): start point, direction and the reciprocals of the direction components (0 when the component is 0).
-struct QuadEdges {
-    double x0[4], y0[4], dx[4], dy[4], idx[4], idy[4];
-};
-
 // Monomial moments M[p][q] = int x^p y^q over (upstream quadrilateral) cap (source cell (r,s)), in that
-// cell's local coordinates, by Green's theorem.  inner_right: the grid line x_local = 1 lies inside the
-// quadrilateral's bounding box (r < r1).
-template <int O>
-__device__ __forceinline__ void piece_moments(const QuadEdges &q, double offx, double offy, bool inner_right,
+// cell's local coordinates, by Green's theorem.  The quadrilateral of the block's cell c comes from shared memory
+// (corners counter-clockwise in anchor-cell units sh.cx/sh.cy, reciprocals of the edge direction components sh.idx/
+// sh.idy, 0 when the component is 0); the loop over its four edges stays rolled (code size).  inner_right: the grid line
+// x_local = 1 lies inside the quadrilateral's bounding box (r < r1).
+template <int O, class SH>
+__device__ __forceinline__ void piece_moments(const SH &sh, int c, double offx, double offy, bool inner_right,
                                               const Basis &bs, double (&M)[2 * O - 1][2 * O - 1])
 {
     constexpr int NM = 2 * O - 1;
@@ -189,14 +187,19 @@ __device__ __forceinline__ void piece_moments(const QuadEdges &q, double offx, d
 #pragma unroll
         for (int qq = 0; qq < NM; ++qq) M[p][qq] = 0.0;
     double ylo = 1e300, yhi = -1e300;
-#pragma unroll
+    double xn = sh.cx[0][c], yn = sh.cy[0][c];  // start of the next edge
+#pragma unroll 1
     for (int e = 0; e < 4; ++e) {
-        const double x0 = q.x0[e] - offx, y0 = q.y0[e] - offy;
-        const double dx = q.dx[e], dy = q.dy[e];
+        const double xs = xn, ys = yn;
+        xn = sh.cx[(e + 1) & 3][c];
+        yn = sh.cy[(e + 1) & 3][c];
+        const double x0 = xs - offx, y0 = ys - offy;
+        const double dx = xn - xs, dy = yn - ys;
+        const double idx = sh.idx[e][c], idy = sh.idy[e][c];
         // crossing with the line x = 1 (for the inner segment); decided from the actual end points
-        const double x1 = q.x0[(e + 1) & 3] - offx;
+        const double x1 = xn - offx;
         if (inner_right && dx != 0.0 && (x0 - 1.0) * (x1 - 1.0) <= 0.0) {
-            const double yc = fma(dmin(dmax((1.0 - x0) * q.idx[e], 0.0), 1.0), dy, y0);
+            const double yc = fma(dmin(dmax((1.0 - x0) * idx, 0.0), 1.0), dy, y0);
             ylo = dmin(ylo, yc);
             yhi = dmax(yhi, yc);
         }
@@ -206,12 +209,12 @@ __device__ __forceinline__ void piece_moments(const QuadEdges &q, double offx, d
         if (dx == 0.0) {
             ok = ok && x0 >= 0.0 && x0 <= 1.0;
         } else {
-            const double ta = -x0 * q.idx[e], tb = (1.0 - x0) * q.idx[e];
+            const double ta = -x0 * idx, tb = (1.0 - x0) * idx;
             t0 = dmax(t0, dmin(ta, tb));
             t1 = dmin(t1, dmax(ta, tb));
         }
         {
-            const double ta = -y0 * q.idy[e], tb = (1.0 - y0) * q.idy[e];
+            const double ta = -y0 * idy, tb = (1.0 - y0) * idy;
             t0 = dmax(t0, dmin(ta, tb));
             t1 = dmin(t1, dmax(ta, tb));
         }
@@ -271,7 +274,9 @@ struct GeomShared {
     // structure of arrays, [field][cell]: phase 1 writes with consecutive lanes on consecutive words
     double cx[4][CELLS], cy[4][CELLS];     // corner feet relative to the anchor cell, cell units
     double idx[4][CELLS], idy[4][CELLS];   // reciprocals of the edge direction components (0 if the component is 0)
-    double Vi[O2 * O2][CELLS];             // inverse Vandermonde, Vi[ab * O2 + m]
+    // inverse Vandermonde, Vi[ab * O2 + m]; phase 1 first parks the 4 + O2 traced feet (x, then y) here
+    static constexpr int NVI = O2 * O2 > 2 * (4 + O2) ? O2 * O2 : 2 * (4 + O2);
+    double Vi[NVI][CELLS];
     double xc[CELLS], yc[CELLS];           // centre of the node feet
     int r0[CELLS], s0[CELLS], nr[CELLS], ns[CELLS], mask[CELLS];
     unsigned short item[CELLS * 11];       // work item -> cell | candidate index << 8, 0xffff = padding
@@ -290,12 +295,32 @@ __device__ __forceinline__ int geometry_setup(const double *__restrict__ va, con
     const double *a = va + z * vplane, *b = vb + z * vplane;
     const double tx = tau / g.h[0], ty = tau / g.h[1];
 
-    // step 1: corner feet -> upstream quadrilateral (counter-clockwise from lower-left)
+    // steps 1 and 4, tracing: the four corners (counter-clockwise from lower-left) and the O2 Gauss-Legendre nodes.
+    // One rolled loop over the 4 + O2 points -- unrolled, eight copies of the two bilinear look-ups were a quarter of the
+    // kernel's code --, feet parked in this cell's column of sh.Vi (x at [pt], y at [4 + O2 + pt]).
+    constexpr int NPT = 4 + O2;
+#pragma unroll 1
+    for (int pt = 0; pt < NPT; ++pt) {
+        double xi, eta;
+        if (pt < 4) {
+            xi = (pt == 1 || pt == 2) ? 1.0 : 0.0;
+            eta = pt >= 2 ? 1.0 : 0.0;
+        } else {
+            xi = bs.xi[O][(pt - 4) % O];
+            eta = bs.xi[O][(pt - 4) / O];
+        }
+        double px, py;
+        trace_point(a, b, nx, ny, tx, ty, i, j, xi, eta, order, periodic, px, py);
+        sh.Vi[pt][c] = px;
+        sh.Vi[NPT + pt][c] = py;
+    }
+    // step 1: upstream quadrilateral
     double cx[4], cy[4];
-    trace_point(a, b, nx, ny, tx, ty, i, j, 0.0, 0.0, order, periodic, cx[0], cy[0]);
-    trace_point(a, b, nx, ny, tx, ty, i, j, 1.0, 0.0, order, periodic, cx[1], cy[1]);
-    trace_point(a, b, nx, ny, tx, ty, i, j, 1.0, 1.0, order, periodic, cx[2], cy[2]);
-    trace_point(a, b, nx, ny, tx, ty, i, j, 0.0, 1.0, order, periodic, cx[3], cy[3]);
+#pragma unroll
+    for (int e = 0; e < 4; ++e) {
+        cx[e] = sh.Vi[e][c];
+        cy[e] = sh.Vi[NPT + e][c];
+    }
     const double xmin = dmin(dmin(cx[0], cx[1]), dmin(cx[2], cx[3]));
     const double ymin = dmin(dmin(cy[0], cy[1]), dmin(cy[2], cy[3]));
     const int r0 = (int)floor(xmin), s0 = (int)floor(ymin);
@@ -345,16 +370,13 @@ __device__ __forceinline__ int geometry_setup(const double *__restrict__ va, con
     {
         double fx[O2], fy[O2];
 #pragma unroll
-        for (int qn = 0; qn < O; ++qn)
-#pragma unroll
-            for (int p = 0; p < O; ++p) {
-                double px, py;
-                trace_point(a, b, nx, ny, tx, ty, i, j, bs.xi[O][p], bs.xi[O][qn], order, periodic, px, py);
-                fx[p + O * qn] = px - r0;
-                fy[p + O * qn] = py - s0;
-                xc += px - r0;
-                yc += py - s0;
-            }
+        for (int m = 0; m < O2; ++m) {  // node m = p + O * qn
+            const double px = sh.Vi[4 + m][c], py = sh.Vi[NPT + 4 + m][c];
+            fx[m] = px - r0;
+            fy[m] = py - s0;
+            xc += px - r0;
+            yc += py - s0;
+        }
         xc *= 1.0 / O2;
         yc *= 1.0 / O2;
         if constexpr (O == 3) {
@@ -417,21 +439,8 @@ __device__ __forceinline__ void geometry_piece(const SH &sh, bool valid, int c, 
     constexpr int O2 = O * O, NM = 2 * O - 1;
     const int lane = threadIdx.x & 31;
     if (!valid) c = 0;
-    QuadEdges q;
-#pragma unroll
-    for (int e = 0; e < 4; ++e) {
-        q.x0[e] = sh.cx[e][c];
-        q.y0[e] = sh.cy[e][c];
-        q.idx[e] = sh.idx[e][c];
-        q.idy[e] = sh.idy[e][c];
-    }
-#pragma unroll
-    for (int e = 0; e < 4; ++e) {
-        q.dx[e] = q.x0[(e + 1) & 3] - q.x0[e];
-        q.dy[e] = q.y0[(e + 1) & 3] - q.y0[e];
-    }
     double M[NM][NM];
-    piece_moments<O>(q, (double)dr, (double)ds, dr < sh.nr[c], bs, M);
+    piece_moments<O>(sh, c, (double)dr, (double)ds, dr < sh.nr[c], bs, M);
     const bool nonempty = valid && M[0][0] > 0.0;
     const unsigned ballot = __ballot_sync(0xffffffffu, nonempty);
     if (!nonempty) return;  // empty intersection
@@ -528,12 +537,18 @@ __device__ __forceinline__ void geometry_piece(const SH &sh, bool valid, int c, 
 // The geometry of up to CELLS target cells of one z node by one thread block (see the two phases above).
 // cell_of(c) -> index t = j * nx + i of the block's c-th cell, or -1.  Threads 0 .. CELLS-1 do phase 1, all
 // `nthreads` (a multiple of 32, >= CELLS) phase 2.  Every thread of the block must call this (block barriers).
-template <int O, int CELLS, class CellOf>
+// WARP: the "block" is ONE warp (CELLS = nthreads = 32, tid = lane) that synchronises with __syncwarp only -- the
+// geometry warps of the persistent 2d kernel (sldg_xy_apply.cu), which must not touch the block-wide barrier.
+template <int O, int CELLS, bool WARP = false, class CellOf>
 __device__ __forceinline__ void geometry_block(GeomShared<O, CELLS> &sh, int tid, int nthreads, CellOf cell_of, int z,
                                                const double *__restrict__ va, const double *__restrict__ vb,
                                                int4 *hdr, double *W, int32_t *err, const GridDev &g, const Basis &bs,
                                                double tau, int order, int periodic)
 {
+    static_assert(!WARP || CELLS == 32, "a geometry warp does 32 cells at a time");
+    auto sync = [] {
+        if constexpr (WARP) __syncwarp(); else __syncthreads();
+    };
     const int lane = tid & 31, warp = tid >> 5;
     const int ncell = g.n[0] * g.n[1];
     const int t = tid < CELLS ? cell_of(tid) : -1;
@@ -554,16 +569,16 @@ __device__ __forceinline__ void geometry_block(GeomShared<O, CELLS> &sh, int tid
         pos = (pos + 31) & ~31;
         if (lane == 0) sh.warp_tot[warp] = pos;
     }
-    __syncthreads();
+    sync();
     int base = 0, total = 0;
     for (int w = 0; w < CELLS / 32; ++w) {
         if (w < warp) base += sh.warp_tot[w];
         total += sh.warp_tot[w];
     }
     for (int it = tid; it < total; it += nthreads) sh.item[it] = 0xffff;
-    __syncthreads();
+    sync();
     for (int k = 0; k < n; ++k) sh.item[base + first + k] = (unsigned short)(tid | (k << 8));
-    __syncthreads();
+    sync();
 
     // phase 2: one piece per thread and pass (whole warps: total is a multiple of 32)
     for (int it = tid; it < total; it += nthreads) {
@@ -575,12 +590,12 @@ __device__ __forceinline__ void geometry_block(GeomShared<O, CELLS> &sh, int tid
         const long long cellid = (long long)z * ncell + cell_of(cc);
         geometry_piece<O>(sh, valid, cc, k, dr, ds, bs, W + (size_t)cellid * 9 * sldg_w_block_doubles(O), &sh.mask[cc]);
     }
-    __syncthreads();
+    sync();
     if (t >= 0) {
         const int m = sh.mask[tid];
         hdr[(long long)z * ncell + t] = make_int4(sh.r0[tid], sh.s0[tid], m, __popc(m));
     }
-    __syncthreads();
+    sync();
 }
 
 }  // namespace sldg_geom
