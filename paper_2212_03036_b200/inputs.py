@@ -166,6 +166,16 @@ def itg_fields(spec: GridSpec, dt, cfl_xy=0.8):
     return a, b, np.ascontiguousarray(Ez), phi0
 
 
+def itg_vertex_profiles(spec: GridSpec):
+    """n0(r) and T_e(r) = T_i(r) (C_Ti = C_Te, kappa_Ti = kappa_Te) of BASELINE.json configs[0] on the
+    periodic nx x ny vertex grid, [ny][nx]: the coefficients of the quasi-neutrality equation (eq. 2)."""
+    xv = spec.vertex_coords(0)[:-1]
+    yv = spec.vertex_coords(1)[:-1]
+    XV, YV = np.meshgrid(xv, yv, indexing="xy")
+    T, n0 = _itg_profiles(np.sqrt(XV * XV + YV * YV))
+    return np.ascontiguousarray(n0), np.ascontiguousarray(T)
+
+
 # --------------------------------------------------------------------------------------------------
 # 2d-only workload (config 1): batched Gaussian bumps sharing one velocity field
 # --------------------------------------------------------------------------------------------------
