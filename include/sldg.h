@@ -151,6 +151,42 @@ int sldg_debug_counter(sldg_ctx *ctx, int which, long long *value_host);
  * TFLOP/s: the roof of the ALU-bound kernels (the paper's intensity argument).
  * Synchronises. */
 int sldg_debug_fp64_peak(sldg_ctx *ctx, int repeats, double *tflops_host);
+
+/* ---- Field step, invariants and the two time-stepping algorithms ----------------
+ * Outside the timed hot path (1/Nv of the volume).  Field grid: the nx x ny cell vertices (periodic) x Nz equidistant
+ * z points at (m + 1/2) h_z / o_z ("inside the cell"); arrays on it are double [Nz][ny][nx].
+ *
+ * sldg_set_profiles: n0 and T_e of the quasi-neutrality equation (eq. 2) at the vertices, [ny][nx], and
+ * the magnetic field strength B of the drift (eq. 1); copied into the workspace. */
+int sldg_set_profiles(sldg_ctx *ctx, const double *n0_dev, const double *Te_dev, double B);
+/* Algorithm 1 step 1 / 5 (section 3.6): charge density of the current state ->
+ * resampled to the field grid (vertex value = mean of the four adjacent cells' polynomials) ->
+ *   -(1/n0) div(n0 grad phi) + (phi - <phi>)/Te = rho/n0 - 1,  <phi> = z average (R20-R22),
+ * second-order differences, Jacobi-preconditioned conjugate gradients to |r| <= tol |b| or max_iter iterations ->
+ * a = -d_y phi/B, b = d_x phi/B, E_z = -d_z phi by centred differences, interpolated to where the advection steps
+ * read them (as after sldg_set_vxy(.., periodic = 1) and sldg_set_Ez).  SLDG_EINVAL before sldg_set_profiles. */
+int sldg_field_step(sldg_ctx *ctx, double tol, int max_iter);
+/* Largest iteration count and relative residual over the systems of the last field step.  Synchronises. */
+int sldg_field_info(sldg_ctx *ctx, int *max_iters_host, double *max_relres_host);
+/* Copies of the last field step's results: phi on the field grid; E_z [Nz][Ny][Nx], a, b [Nz][ny+1][nx+1] as the
+ * advection steps see them (any pointer may be NULL).  Asynchronous. */
+int sldg_get_phi(sldg_ctx *ctx, double *phi_dev);
+int sldg_get_fields(sldg_ctx *ctx, double *Ez_dev, double *a_dev, double *b_dev);
+/* The quantities of PAPER.md:332-346 for the current state and the potential of the last field step:
+ * out[0] electric energy sqrt(int phi^2(r_p, theta, z) dtheta dz) on the circle of radius r_p around the box centre
+ * (bilinear samples at 4 max(nx, ny) angles), out[1] mass, out[2] L2 norm, out[3] kinetic energy int v^2/2 f,
+ * out[4] potential energy int phi f (total energy = out[3] + out[4]).  Synchronises. */
+int sldg_diagnostics(sldg_ctx *ctx, double r_p, double out_host[5]);
+/* One time step of Algorithm 1 (the source terms vanish for the Cartesian full-f formulation):
+ * field step, z(dt/2), v(dt/2), field step, xy(dt), v(dt/2), z(dt/2). */
+int sldg_step_algorithm1(sldg_ctx *ctx, double dt, double tol, int max_iter);
+/* A third state buffer (sldg_state_bytes, 256-byte aligned, borrowed until sldg_destroy) for Algorithm 2, which
+ * restarts its corrector from the state of time level n ("three copies"). */
+int sldg_set_third_buffer(sldg_ctx *ctx, double *f_c_dev);
+/* One time step of Algorithm 2: field step; predictor z(dt/2), v(dt/2), xy(dt/2) with first-order
+ * tracing (eq. 14); field step on the predicted state; corrector from the state of level n: z(dt/2), v(dt/2), xy(dt)
+ * with second-order tracing (eq. 15), v(dt/2), z(dt/2).  No state is copied: the three buffers rotate. */
+int sldg_step_algorithm2(sldg_ctx *ctx, double dt, double tol, int max_iter);
 const char *sldg_strerror(int code);
 
 #ifdef __cplusplus

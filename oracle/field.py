@@ -230,3 +230,38 @@ def diagnostics(spec, f, phi, phi_nodes, r_p):
     kinetic = float((fw * (0.5 * v * v)[None, :, None, None]).sum())
     potential = float((fw * phi_nodes[:, None, :, :]).sum())
     return {"electric": float(electric), "mass": mass, "l2": l2, "kinetic": kinetic, "potential": potential}
+
+
+def algorithm1_step(spec, f, n0, Te, dt, B=1.0):
+    """One step of Algorithm 1 for the Cartesian full-f state (no source terms, R0), in the paper's
+    order: 1 field, 3 z(dt/2), 4 v(dt/2), 5 field from the intermediate state, 6 xy(dt) second-order tracing,
+    7 v(dt/2), 8 z(dt/2).  Returns the new f and the fields of step 5."""
+    import oracle
+
+    fs = field_step(spec, oracle.charge_density(spec, f), n0, Te, B)                # 1
+    f = oracle.advect_z(spec, f, 0.5 * dt)                                          # 3
+    f = oracle.advect_v(spec, f, fs["Ez"], 0.5 * dt)                                # 4
+    fs = field_step(spec, oracle.charge_density(spec, f), n0, Te, B)                # 5
+    f = oracle.advect_xy(spec, f, fs["a"], fs["b"], dt, 2, 1)                       # 6
+    f = oracle.advect_v(spec, f, fs["Ez"], 0.5 * dt)                                # 7
+    f = oracle.advect_z(spec, f, 0.5 * dt)                                          # 8
+    return f, fs
+
+
+def algorithm2_step(spec, f, n0, Te, dt, B=1.0):
+    """One step of Algorithm 2, predictor-corrector: 1 field phi^n; predictor 3 z(dt/2), 4 v(dt/2),
+    5 xy(dt/2) with first-order tracing (eq. 14) -> f^{n+1/2}; 6 field phi^{n+1/2}; corrector from f^n: 8 z(dt/2),
+    9 v(dt/2), 10 xy(dt) with second-order tracing (eq. 15), 11 v(dt/2), 12 z(dt/2)."""
+    import oracle
+
+    fs = field_step(spec, oracle.charge_density(spec, f), n0, Te, B)                # 1
+    g = oracle.advect_z(spec, f, 0.5 * dt)                                          # 3
+    g = oracle.advect_v(spec, g, fs["Ez"], 0.5 * dt)                                # 4
+    g = oracle.advect_xy(spec, g, fs["a"], fs["b"], 0.5 * dt, 1, 1)                 # 5
+    fs = field_step(spec, oracle.charge_density(spec, g), n0, Te, B)                # 6
+    f = oracle.advect_z(spec, f, 0.5 * dt)                                          # 8
+    f = oracle.advect_v(spec, f, fs["Ez"], 0.5 * dt)                                # 9
+    f = oracle.advect_xy(spec, f, fs["a"], fs["b"], dt, 2, 1)                       # 10
+    f = oracle.advect_v(spec, f, fs["Ez"], 0.5 * dt)                                # 11
+    f = oracle.advect_z(spec, f, 0.5 * dt)                                          # 12
+    return f, fs

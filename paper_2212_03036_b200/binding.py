@@ -22,6 +22,8 @@ EXPORTS = [
     "sldg_charge_density", "sldg_mass", "sldg_strang_step", "sldg_set_trace_order",
     "sldg_strang_step_host", "sldg_check", "sldg_last_timing_ms", "sldg_launch_count",
     "sldg_debug_geometry", "sldg_debug_counter", "sldg_debug_fp64_peak", "sldg_strerror",
+    "sldg_set_profiles", "sldg_field_step", "sldg_field_info", "sldg_get_phi", "sldg_get_fields", "sldg_diagnostics",
+    "sldg_step_algorithm1", "sldg_set_third_buffer", "sldg_step_algorithm2",
 ]
 
 
@@ -82,6 +84,15 @@ def load_library():
     L.sldg_debug_fp64_peak.argtypes = [vp, C.c_int, C.POINTER(C.c_double)]
     L.sldg_strerror.argtypes = [C.c_int]
     L.sldg_strerror.restype = C.c_char_p
+    L.sldg_set_profiles.argtypes = [vp, dp, dp, C.c_double]
+    L.sldg_field_step.argtypes = [vp, C.c_double, C.c_int]
+    L.sldg_field_info.argtypes = [vp, C.POINTER(C.c_int), C.POINTER(C.c_double)]
+    L.sldg_get_phi.argtypes = [vp, dp]
+    L.sldg_get_fields.argtypes = [vp, dp, dp, dp]
+    L.sldg_diagnostics.argtypes = [vp, C.c_double, C.POINTER(C.c_double * 5)]
+    L.sldg_step_algorithm1.argtypes = [vp, C.c_double, C.c_double, C.c_int]
+    L.sldg_set_third_buffer.argtypes = [vp, dp]
+    L.sldg_step_algorithm2.argtypes = [vp, C.c_double, C.c_double, C.c_int]
     _lib = L
     return L
 
@@ -215,6 +226,50 @@ class Sldg:
             out = self.torch.empty(1, dtype=self.torch.float64, device=self.device)
         self._chk(self.L.sldg_mass(self.h, out.data_ptr()), "sldg_mass")
         return out
+
+    # ---- field step, invariants, Algorithms 1 and 2 -------------------------------------------------
+    def set_profiles(self, n0, Te, B=1.0):
+        for u in (n0, Te):
+            assert u.is_cuda and u.dtype == self.torch.float64 and u.is_contiguous()
+        self._chk(self.L.sldg_set_profiles(self.h, n0.data_ptr(), Te.data_ptr(), float(B)), "sldg_set_profiles")
+
+    def field_step(self, tol=1e-13, max_iter=2000):
+        self._chk(self.L.sldg_field_step(self.h, float(tol), int(max_iter)), "sldg_field_step")
+
+    def field_info(self):
+        it, rr = C.c_int(0), C.c_double(0.0)
+        self._chk(self.L.sldg_field_info(self.h, C.byref(it), C.byref(rr)), "sldg_field_info")
+        return int(it.value), float(rr.value)
+
+    def get_phi(self):
+        nx, ny = self.spec.n[0], self.spec.n[1]
+        out = self.torch.empty((self.spec.N[2], ny, nx), dtype=self.torch.float64, device=self.device)
+        self._chk(self.L.sldg_get_phi(self.h, out.data_ptr()), "sldg_get_phi")
+        return out
+
+    def get_fields(self):
+        t = self.torch
+        Nx, Ny, Nz, _ = self.spec.N
+        nx, ny = self.spec.n[0], self.spec.n[1]
+        Ez = t.empty((Nz, Ny, Nx), dtype=t.float64, device=self.device)
+        a = t.empty((Nz, ny + 1, nx + 1), dtype=t.float64, device=self.device)
+        b = t.empty_like(a)
+        self._chk(self.L.sldg_get_fields(self.h, Ez.data_ptr(), a.data_ptr(), b.data_ptr()), "sldg_get_fields")
+        return Ez, a, b
+
+    def diagnostics(self, r_p):
+        out = (C.c_double * 5)()
+        self._chk(self.L.sldg_diagnostics(self.h, float(r_p), C.byref(out)), "sldg_diagnostics")
+        return dict(zip(("electric", "mass", "l2", "kinetic", "potential"), (float(x) for x in out)))
+
+    def step_algorithm1(self, dt, tol=1e-13, max_iter=2000):
+        self._chk(self.L.sldg_step_algorithm1(self.h, float(dt), float(tol), int(max_iter)), "sldg_step_algorithm1")
+
+    def step_algorithm2(self, dt, tol=1e-13, max_iter=2000):
+        if getattr(self, "f_c", None) is None:  # the third copy of f
+            self.f_c = self.torch.empty(self.state_bytes // 8, dtype=self.torch.float64, device=self.device)
+            self._chk(self.L.sldg_set_third_buffer(self.h, self.f_c.data_ptr()), "sldg_set_third_buffer")
+        self._chk(self.L.sldg_step_algorithm2(self.h, float(dt), float(tol), int(max_iter)), "sldg_step_algorithm2")
 
     # ---- diagnostics ---------------------------------------------------------------------------
     def check(self):

@@ -51,7 +51,7 @@ void fill_grid(const sldg_params *p, GridDev *g)
 }
 
 struct WorkspaceMap {
-    size_t Ez, va, vb, hdr, W, partials, rho, scalar, err, stage_ok, total;
+    size_t Ez, va, vb, hdr, W, partials, rho, scalar, err, stage_ok, field, total;
     size_t n_partials;
 };
 
@@ -75,6 +75,7 @@ WorkspaceMap map_workspace(const sldg_params *p)
     m.scalar = take(256);
     m.err = take(256);
     m.stage_ok = take(xy_apply_stage_flags(p) * 4);
+    m.field = take(field_workspace_bytes(p));
     m.total = off;
     return m;
 }
@@ -269,6 +270,7 @@ int sldg_create(const sldg_params *p, double *f_a_dev, double *f_b_dev, void *wo
     c->scalar_ws = (double *)(ws + m.scalar);
     c->err = (int32_t *)(ws + m.err);
     c->stage_ok = (int32_t *)(ws + m.stage_ok);
+    field_carve(c, ws + m.field);
     c->fuse = getenv("SLDG_NO_FUSE") ? 0 : 1;
     c->trace_order = 2;
     c->vel_periodic = 0;
@@ -574,6 +576,143 @@ int sldg_last_timing_ms(sldg_ctx *c, float ms[8])
 }
 
 long long sldg_launch_count(sldg_ctx *c) { return c ? c->launches : 0; }
+
+// ---- field step, invariants, Algorithms 1 and 2 --------------------------------------------------------------
+
+int sldg_set_profiles(sldg_ctx *c, const double *n0_dev, const double *Te_dev, double B)
+{
+    if (!c || !n0_dev || !Te_dev || !(B != 0.0)) return SLDG_EINVAL;
+    const size_t bytes = (size_t)c->g.n[0] * c->g.n[1] * 8;
+    if (cudaMemcpyAsync(c->fld.n0, n0_dev, bytes, cudaMemcpyDeviceToDevice, c->stream) != cudaSuccess) return SLDG_ECUDA;
+    if (cudaMemcpyAsync(c->fld.Te, Te_dev, bytes, cudaMemcpyDeviceToDevice, c->stream) != cudaSuccess) return SLDG_ECUDA;
+    c->fld.invB = 1.0 / B;
+    c->fld.have_profiles = 1;
+    return SLDG_OK;
+}
+
+int sldg_field_step(sldg_ctx *c, double tol, int max_iter)
+{
+    if (!c || !c->fld.have_profiles || !(tol > 0.0) || max_iter < 1) return SLDG_EINVAL;
+    return cuda_fail(launch_field_step(c, c->f[c->cur], tol, max_iter));
+}
+
+int sldg_field_info(sldg_ctx *c, int *max_iters_host, double *max_relres_host)
+{
+    if (!c || !c->fld.have_phi) return SLDG_EINVAL;
+    const int n = c->g.N[2] + 1;
+    std::vector<int> it(n);
+    std::vector<double> rr(n);
+    if (cudaMemcpyAsync(it.data(), c->fld.iters, n * 4, cudaMemcpyDeviceToHost, c->stream) != cudaSuccess) return SLDG_ECUDA;
+    if (cudaMemcpyAsync(rr.data(), c->fld.relres, n * 8, cudaMemcpyDeviceToHost, c->stream) != cudaSuccess) return SLDG_ECUDA;
+    if (cudaStreamSynchronize(c->stream) != cudaSuccess) return SLDG_ECUDA;
+    int mi = 0;
+    double mr = 0.0;
+    for (int k = 0; k < n; ++k) {
+        mi = it[k] > mi ? it[k] : mi;
+        mr = rr[k] > mr ? rr[k] : mr;
+    }
+    if (max_iters_host) *max_iters_host = mi;
+    if (max_relres_host) *max_relres_host = mr;
+    return SLDG_OK;
+}
+
+int sldg_get_phi(sldg_ctx *c, double *phi_dev)
+{
+    if (!c || !phi_dev || !c->fld.have_phi) return SLDG_EINVAL;
+    const size_t bytes = (size_t)c->g.N[2] * c->g.n[0] * c->g.n[1] * 8;
+    return cuda_fail(cudaMemcpyAsync(phi_dev, c->fld.phi, bytes, cudaMemcpyDeviceToDevice, c->stream));
+}
+
+int sldg_get_fields(sldg_ctx *c, double *Ez_dev, double *a_dev, double *b_dev)
+{
+    if (!c) return SLDG_EINVAL;
+    const GridDev &g = c->g;
+    const size_t vb = (size_t)g.N[2] * (g.n[0] + 1) * (g.n[1] + 1) * 8;
+    if (Ez_dev && cudaMemcpyAsync(Ez_dev, c->Ez, (size_t)g.lines * 8, cudaMemcpyDeviceToDevice, c->stream) != cudaSuccess)
+        return SLDG_ECUDA;
+    if (a_dev && cudaMemcpyAsync(a_dev, c->va, vb, cudaMemcpyDeviceToDevice, c->stream) != cudaSuccess) return SLDG_ECUDA;
+    if (b_dev && cudaMemcpyAsync(b_dev, c->vb, vb, cudaMemcpyDeviceToDevice, c->stream) != cudaSuccess) return SLDG_ECUDA;
+    return SLDG_OK;
+}
+
+int sldg_diagnostics(sldg_ctx *c, double r_p, double out_host[5])
+{
+    if (!c || !out_host || !c->fld.have_phi) return SLDG_EINVAL;
+    return cuda_fail(launch_diagnostics(c, c->f[c->cur], r_p, out_host));
+}
+
+int sldg_step_algorithm1(sldg_ctx *c, double dt, double tol, int max_iter)
+{
+    int rc, fused;
+    if ((rc = sldg_field_step(c, tol, max_iter))) return rc;
+    if ((rc = do_pair(c, 0.5 * dt, true, c->ev[1], &fused))) return rc;
+    if ((rc = sldg_field_step(c, tol, max_iter))) return rc;
+    if ((rc = do_xy(c, dt, 2))) return rc;
+    if ((rc = do_pair(c, 0.5 * dt, false, c->ev[4], &fused))) return rc;
+    c->ev_kind = 0;
+    return SLDG_OK;
+}
+
+int sldg_set_third_buffer(sldg_ctx *c, double *f_c_dev)
+{
+    if (!c || !f_c_dev || ((uintptr_t)f_c_dev & 255) || f_c_dev == c->f[0] || f_c_dev == c->f[1]) return SLDG_EINVAL;
+    c->f_c = f_c_dev;
+    return SLDG_OK;
+}
+
+// Algorithm 2 writes every substep into a buffer that is neither its source nor `keep` (the state of level n while the
+// corrector still needs it): the spare buffer takes the place of the context's idle ping-pong buffer when necessary.
+static void aim_away_from(sldg_ctx *c, const double *keep)
+{
+    if (c->f[c->cur ^ 1] == keep) {
+        double *t = c->f[c->cur ^ 1];
+        c->f[c->cur ^ 1] = c->f_c;
+        c->f_c = t;
+    }
+}
+
+static int pair_keeping(sldg_ctx *c, double tau, bool z_first, const double *keep)
+{
+    aim_away_from(c, keep);
+    if (c->fuse) {
+        cudaError_t e = launch_fused_sweeps(c, c->f[c->cur], c->f[c->cur ^ 1], tau, tau, z_first);
+        if (e == cudaSuccess) {
+            swap_state(c);
+            return SLDG_OK;
+        }
+        if (e != cudaErrorNotSupported) return SLDG_ECUDA;
+        cudaGetLastError();
+    }
+    int rc = z_first ? do_z(c, tau) : do_v(c, tau);
+    if (rc) return rc;
+    aim_away_from(c, keep);
+    return z_first ? do_v(c, tau) : do_z(c, tau);
+}
+
+int sldg_step_algorithm2(sldg_ctx *c, double dt, double tol, int max_iter)
+{
+    if (!c || !c->f_c) return SLDG_EINVAL;
+    int rc;
+    double *fn = c->f[c->cur];  // the state of time level n
+    if ((rc = sldg_field_step(c, tol, max_iter))) return rc;
+    // predictor with phi^n: first-order tracing over dt/2
+    if ((rc = pair_keeping(c, 0.5 * dt, true, fn))) return rc;
+    aim_away_from(c, fn);
+    if ((rc = do_xy(c, 0.5 * dt, 1))) return rc;
+    if ((rc = sldg_field_step(c, tol, max_iter))) return rc;  // phi^{n+1/2}
+    // corrector: start again from level n; the predicted state is dead, level n after its first read
+    if (c->f[0] == fn) c->cur = 0;
+    else if (c->f[1] == fn) c->cur = 1;
+    else {  // level n sits in the spare slot: exchange it with the predicted state
+        c->f_c = c->f[c->cur];
+        c->f[c->cur] = fn;
+    }
+    if ((rc = pair_keeping(c, 0.5 * dt, true, nullptr))) return rc;
+    if ((rc = do_xy(c, dt, 2))) return rc;
+    if ((rc = pair_keeping(c, 0.5 * dt, false, nullptr))) return rc;
+    c->ev_kind = 0;
+    return SLDG_OK;
+}
 
 int sldg_debug_geometry(sldg_ctx *c, int z, int32_t *anchor_dev, int32_t *mask_dev, double *W_dev)
 {

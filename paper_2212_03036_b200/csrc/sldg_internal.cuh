@@ -45,6 +45,15 @@ struct ShiftPoly {
     int o;
 };
 
+// Workspace of the field step (sldg_field.cu): profiles, the potential on the field grid [Nz][ny][nx], vectors of the
+// conjugate-gradient solves, the potential at the nodes (potential energy), scalars and per-system solver records.
+struct FieldWs {
+    double *n0, *Te, *phi, *rhs, *r, *p, *q, *bar[5], *phin, *scal, *relres;
+    int *iters;
+    double invB;
+    int have_profiles, have_phi;
+};
+
 struct sldg_ctx {
     sldg_params p;
     GridDev g;
@@ -73,6 +82,8 @@ struct sldg_ctx {
     int ev_kind;            // 0 none, 1 strang, 2 z, 3 v, 4 xy
     long long launches;
     int sm_count;
+    FieldWs fld;
+    double *f_c;            // optional third state buffer (Algorithm 2 keeps the state of time level n)
 };
 
 // ---- kernel launchers (each returns cudaGetLastError()) ------------------------------------------
@@ -90,3 +101,7 @@ cudaError_t launch_xy_apply(sldg_ctx *c, const double *fin, double *fout);
 cudaError_t count_weight_blocks(sldg_ctx *c, long long *total_host);
 cudaError_t launch_fused_sweeps(sldg_ctx *c, const double *fin, double *fout, double tau_z, double tau_v, bool z_first,
                                 bool z_only = false);
+size_t field_workspace_bytes(const sldg_params *p);
+void field_carve(sldg_ctx *c, char *base);
+cudaError_t launch_field_step(sldg_ctx *c, const double *fin, double tol, int max_iter);
+cudaError_t launch_diagnostics(sldg_ctx *c, const double *fin, double r_p, double *out_host);

@@ -103,8 +103,9 @@ def _itg_profiles(r):
     return T, n0
 
 
-def itg_initial_f(spec: GridSpec, out=None):
-    """BASELINE.json configs[0] initial condition sampled at the GL nodes (point values)."""
+def itg_initial_f(spec: GridSpec, out=None, eps=1e-6):
+    """BASELINE.json configs[0] initial condition sampled at the GL nodes (point values); eps is the
+    amplitude of the perturbation (1e-6 in the config; larger values exercise the self-consistent field in tests)."""
     x = spec.node_coords(0)
     y = spec.node_coords(1)
     z = spec.node_coords(2)
@@ -114,7 +115,7 @@ def itg_initial_f(spec: GridSpec, out=None):
     th = np.arctan2(Y, X)
     T, n0 = _itg_profiles(r)
     feq = (n0 / np.sqrt(2.0 * np.pi * T))[None, :, :] * np.exp(-(v * v)[:, None, None] / (2.0 * T)[None, :, :])
-    env = 1e-6 * np.exp(-((r - ITG_RP) ** 2) / 4.0)  # [Ny][Nx]
+    env = eps * np.exp(-((r - ITG_RP) ** 2) / 4.0)  # [Ny][Nx]
     if out is None:
         out = np.empty(spec.shape, dtype=np.float64)
     Lz = spec.hi[2] - spec.lo[2]

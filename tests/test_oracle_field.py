@@ -163,3 +163,45 @@ def test_diagnostics_closed_forms():
     assert abs(d["l2"] - math.sqrt(vol_yz * ix2 * (6.0 + 0.25 * 18.0))) < 1e-11
     assert abs(d["potential"] - 0.25 * d["mass"]) < 1e-11
     assert abs(d["electric"] - 0.25 * math.sqrt(2 * math.pi * 6.0)) < 1e-12
+
+
+def _small_itg():
+    spec = inputs.itg_grid(12, 12, 4, 12, 2)
+    n0, Te = inputs.itg_vertex_profiles(spec)
+    return spec, n0, Te, inputs.itg_initial_f(spec, eps=0.3)
+
+
+def test_algorithms_1_and_2_differ_by_a_local_second_order_term_and_conserve_mass():
+    # Algorithm 1 "fails to be second order because the electric field that is used to trace the
+    # characteristics is not a sufficiently accurate approximation at half the time step" -- its field phi* is an O(dt)
+    # approximation of phi^{n+1/2}, so one step of Algorithm 1 and one of Algorithm 2 differ by O(dt^2) (the spatial
+    # projection errors, identical substeps, cancel): halving dt divides the difference by 4
+    import oracle
+    spec, n0, Te, f0 = _small_itg()
+    m0 = oracle.mass(spec, f0)
+    d = []
+    for dt in (4.0, 2.0, 1.0):
+        f1, _ = field.algorithm1_step(spec, f0.copy(), n0, Te, dt)
+        f2, _ = field.algorithm2_step(spec, f0.copy(), n0, Te, dt)
+        d.append(np.abs(f1 - f2).max())
+        assert abs(oracle.mass(spec, f1) - m0) < 1e-13 * m0 and abs(oracle.mass(spec, f2) - m0) < 1e-13 * m0
+    assert 1.85 < math.log2(d[0] / d[1]) < 2.15 and 1.85 < math.log2(d[1] / d[2]) < 2.15, d
+
+
+def test_algorithm_steps_are_the_papers_sequences():
+    # the order of Algorithm 1 (steps 1, 3-8) and of Algorithm 2 (1, 3-6, 8-12) written out with the pinned substeps
+    import oracle
+    spec, n0, Te, f0 = _small_itg()
+    dt = 3.0
+    fs = field.field_step(spec, oracle.charge_density(spec, f0), n0, Te)
+    g = oracle.advect_v(spec, oracle.advect_z(spec, f0, dt / 2), fs["Ez"], dt / 2)
+    fs1 = field.field_step(spec, oracle.charge_density(spec, g), n0, Te)
+    w1 = oracle.advect_z(spec, oracle.advect_v(spec, oracle.advect_xy(spec, g, fs1["a"], fs1["b"], dt, 2, 1), fs1["Ez"], dt / 2), dt / 2)
+    got1, _ = field.algorithm1_step(spec, f0.copy(), n0, Te, dt)
+    assert np.array_equal(got1, w1)
+    half = oracle.advect_xy(spec, g, fs["a"], fs["b"], dt / 2, 1, 1)                # predictor: eq. (14), dt/2, phi^n
+    fs2 = field.field_step(spec, oracle.charge_density(spec, half), n0, Te)
+    h = oracle.advect_v(spec, oracle.advect_z(spec, f0, dt / 2), fs2["Ez"], dt / 2)  # corrector restarts from f^n
+    w2 = oracle.advect_z(spec, oracle.advect_v(spec, oracle.advect_xy(spec, h, fs2["a"], fs2["b"], dt, 2, 1), fs2["Ez"], dt / 2), dt / 2)
+    got2, _ = field.algorithm2_step(spec, f0.copy(), n0, Te, dt)
+    assert np.array_equal(got2, w2)
