@@ -84,7 +84,9 @@ double *sldg_current(sldg_ctx *ctx);
  * sldg_set_vxy: `periodic` != 0 declares a, b bitwise periodic (a[.., ny, :] == a[.., 0, :] and
  * a[.., :, nx] == a[.., :, 0]); the half-step point of the second-order tracing (eq. 15) is
  * then looked up modulo the box so that the upstream mesh tiles across the periodic seam; with
- * periodic == 0 the cell index is clamped to the box (reading A15). */
+ * periodic == 0 the cell index is clamped to the box (reading A15); periodic == 2: periodic
+ * along y only, clamped along x -- the polar plane with x = r, y = theta, where the radial velocity is zero at r_min and
+ * r_max and no upstream cell leaves the box through those edges. */
 int sldg_set_Ez(sldg_ctx *ctx, const double *Ez_dev);
 int sldg_set_vxy(sldg_ctx *ctx, const double *a_dev, const double *b_dev, int periodic);
 
@@ -187,6 +189,22 @@ int sldg_set_third_buffer(sldg_ctx *ctx, double *f_c_dev);
  * tracing (eq. 14); field step on the predicted state; corrector from the state of level n: z(dt/2), v(dt/2), xy(dt)
  * with second-order tracing (eq. 15), v(dt/2), z(dt/2).  No state is copied: the three buffers rotate. */
 int sldg_step_algorithm2(sldg_ctx *ctx, double dt, double tol, int max_iter);
+
+/* ---- Source term of the delta-g formulation in polar coordinates ------------------------
+ * The paper advects dg = g - g_eq, g = r f, in (r, theta, z, v) (eq. 3): axis 0 is r, axis 1 theta; the
+ * three advections are the calls above with the drift (-d_theta phi / r, d_r phi / r) at the vertices -- radial
+ * component zero at r_min and r_max, sldg_set_vxy(.., periodic = 2) -- and the equilibrium enters through
+ *     dg += tau ( d_z phi * d_v g_eq + d_theta phi * d_r(g_eq / r) )          (section 3.5)
+ * sldg_set_equilibrium: d_v g_eq and d_r(g_eq/r) as double [Nv][Nr] (r fastest).  sldg_set_source_fields: d_z phi and
+ * d_theta phi at the nodes, double [Nz][Ntheta][Nr].  Both are copied into the workspace. */
+int sldg_set_equilibrium(sldg_ctx *ctx, const double *dv_geq_dev, const double *dr_geq_dev);
+int sldg_set_source_fields(sldg_ctx *ctx, const double *dz_phi_dev, const double *dtheta_phi_dev);
+/* Forward-Euler source step of size tau, in place (one pass over f).  SLDG_EINVAL before the two setters.
+ * sldg_last_timing_ms()[7] holds its device time afterwards. */
+int sldg_source_step(sldg_ctx *ctx, double tau);
+/* Algorithm 1 steps 2-4, 6-9 with the fields currently set: source(dt/2), z(dt/2), v(dt/2), 2d(dt),
+ * v(dt/2), z(dt/2), source(dt/2). */
+int sldg_strang_step_sources(sldg_ctx *ctx, double dt);
 const char *sldg_strerror(int code);
 
 #ifdef __cplusplus

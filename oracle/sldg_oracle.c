@@ -307,14 +307,18 @@ static pt trace_point(const double *a, const double *b, int nx, int ny, double h
         return f;
     }
     double mx = xi - 0.5 * tau * ua / hx, my = eta - 0.5 * tau * ub / hy;
-    if (vel_periodic) {
-        /* bitwise-periodic field: the half-step point is looked up modulo the box, so that the two
-         * periodic images of a vertex get the same foot and the upstream mesh tiles (reading A15) */
+    {
+        /* Per axis: a bitwise-periodic field is looked up modulo the box, so that the two periodic images of a vertex get
+         * the same foot and the upstream mesh tiles (reading A15); otherwise the cell index is clamped to the box.
+         * vel_periodic 1: both axes periodic; 0: both clamped; 2: x clamped, y periodic -- the polar plane, x = r
+         * (bounded, radial velocity zero at r_min and r_max), y = theta (periodic). */
+        const int px = vel_periodic == 1, py = vel_periodic == 1 || vel_periodic == 2;
         int fi = (int)floor(mx), fj = (int)floor(my);
-        bilinear(a, b, nx, wrap(i + fi, nx), wrap(j + fj, ny), mx - fi, my - fj, &ua, &ub);
-    } else {
-        int ci = clampi(i + (int)floor(mx), 0, nx - 1), cj = clampi(j + (int)floor(my), 0, ny - 1);
-        bilinear(a, b, nx, ci, cj, mx - (ci - i), my - (cj - j), &ua, &ub);
+        const int ci = px ? wrap(i + fi, nx) : clampi(i + fi, 0, nx - 1);
+        const int cj = py ? wrap(j + fj, ny) : clampi(j + fj, 0, ny - 1);
+        if (!px) fi = ci - i;
+        if (!py) fj = cj - j;
+        bilinear(a, b, nx, ci, cj, mx - fi, my - fj, &ua, &ub);
     }
     f.x = xi - tau * ua / hx;
     f.y = eta - tau * ub / hy;

@@ -24,6 +24,7 @@ EXPORTS = [
     "sldg_debug_geometry", "sldg_debug_counter", "sldg_debug_fp64_peak", "sldg_strerror",
     "sldg_set_profiles", "sldg_field_step", "sldg_field_info", "sldg_get_phi", "sldg_get_fields", "sldg_diagnostics",
     "sldg_step_algorithm1", "sldg_set_third_buffer", "sldg_step_algorithm2",
+    "sldg_set_equilibrium", "sldg_set_source_fields", "sldg_source_step", "sldg_strang_step_sources",
 ]
 
 
@@ -93,6 +94,10 @@ def load_library():
     L.sldg_step_algorithm1.argtypes = [vp, C.c_double, C.c_double, C.c_int]
     L.sldg_set_third_buffer.argtypes = [vp, dp]
     L.sldg_step_algorithm2.argtypes = [vp, C.c_double, C.c_double, C.c_int]
+    L.sldg_set_equilibrium.argtypes = [vp, dp, dp]
+    L.sldg_set_source_fields.argtypes = [vp, dp, dp]
+    L.sldg_source_step.argtypes = [vp, C.c_double]
+    L.sldg_strang_step_sources.argtypes = [vp, C.c_double]
     _lib = L
     return L
 
@@ -270,6 +275,23 @@ class Sldg:
             self.f_c = self.torch.empty(self.state_bytes // 8, dtype=self.torch.float64, device=self.device)
             self._chk(self.L.sldg_set_third_buffer(self.h, self.f_c.data_ptr()), "sldg_set_third_buffer")
         self._chk(self.L.sldg_step_algorithm2(self.h, float(dt), float(tol), int(max_iter)), "sldg_step_algorithm2")
+
+    # ---- delta-g formulation: source term (polar coordinates, axis 0 = r, axis 1 = theta) ------------
+    def set_equilibrium(self, dv_geq, dr_geq):
+        for u in (dv_geq, dr_geq):
+            assert u.is_cuda and u.dtype == self.torch.float64 and u.is_contiguous()
+        self._chk(self.L.sldg_set_equilibrium(self.h, dv_geq.data_ptr(), dr_geq.data_ptr()), "sldg_set_equilibrium")
+
+    def set_source_fields(self, dz_phi, dtheta_phi):
+        for u in (dz_phi, dtheta_phi):
+            assert u.is_cuda and u.dtype == self.torch.float64 and u.is_contiguous()
+        self._chk(self.L.sldg_set_source_fields(self.h, dz_phi.data_ptr(), dtheta_phi.data_ptr()), "sldg_set_source_fields")
+
+    def source_step(self, tau):
+        self._chk(self.L.sldg_source_step(self.h, float(tau)), "sldg_source_step")
+
+    def strang_step_sources(self, dt):
+        self._chk(self.L.sldg_strang_step_sources(self.h, float(dt)), "sldg_strang_step_sources")
 
     # ---- diagnostics ---------------------------------------------------------------------------
     def check(self):

@@ -51,7 +51,7 @@ void fill_grid(const sldg_params *p, GridDev *g)
 }
 
 struct WorkspaceMap {
-    size_t Ez, va, vb, hdr, W, partials, rho, scalar, err, stage_ok, field, total;
+    size_t Ez, va, vb, hdr, W, partials, rho, scalar, err, stage_ok, field, source, total;
     size_t n_partials;
 };
 
@@ -76,6 +76,7 @@ WorkspaceMap map_workspace(const sldg_params *p)
     m.err = take(256);
     m.stage_ok = take(xy_apply_stage_flags(p) * 4);
     m.field = take(field_workspace_bytes(p));
+    m.source = take(source_workspace_bytes(p));
     m.total = off;
     return m;
 }
@@ -271,6 +272,7 @@ int sldg_create(const sldg_params *p, double *f_a_dev, double *f_b_dev, void *wo
     c->err = (int32_t *)(ws + m.err);
     c->stage_ok = (int32_t *)(ws + m.stage_ok);
     field_carve(c, ws + m.field);
+    source_carve(c, ws + m.source);
     c->fuse = getenv("SLDG_NO_FUSE") ? 0 : 1;
     c->trace_order = 2;
     c->vel_periodic = 0;
@@ -367,7 +369,7 @@ int sldg_set_vxy(sldg_ctx *c, const double *a_dev, const double *b_dev, int peri
     if (!c || !a_dev || !b_dev) return SLDG_EINVAL;
     const GridDev &g = c->g;
     size_t bytes = (size_t)g.N[2] * (g.n[0] + 1) * (g.n[1] + 1) * 8;
-    c->vel_periodic = periodic ? 1 : 0;
+    c->vel_periodic = periodic == 2 ? 2 : (periodic ? 1 : 0);
     if (cudaMemcpyAsync(c->va, a_dev, bytes, cudaMemcpyDeviceToDevice, c->stream) != cudaSuccess) return SLDG_ECUDA;
     return cuda_fail(cudaMemcpyAsync(c->vb, b_dev, bytes, cudaMemcpyDeviceToDevice, c->stream));
 }
@@ -506,7 +508,7 @@ int sldg_strang_step_host(sldg_ctx *c, double dt, const double *Ez_host, const d
         return SLDG_ECUDA;
     if (a_host) {
         size_t bytes = (size_t)g.N[2] * (g.n[0] + 1) * (g.n[1] + 1) * 8;
-        c->vel_periodic = periodic ? 1 : 0;
+        c->vel_periodic = periodic == 2 ? 2 : (periodic ? 1 : 0);
         // a, b are first needed by the 2d step: their upload runs on the copy stream under the z and v sweeps
         cudaEventRecord(c->cev[0], c->stream);
         cudaStreamWaitEvent(c->cstream, c->cev[0], 0);
@@ -571,6 +573,8 @@ int sldg_last_timing_ms(sldg_ctx *c, float ms[8])
     } else if (c->ev_kind == 4) {
         ms[2] = geom();
         ms[3] = ms[7] = el(0, 1);
+    } else if (c->ev_kind == 5) {
+        ms[7] = el(0, 1);
     }
     return SLDG_OK;
 }
@@ -651,6 +655,44 @@ int sldg_step_algorithm1(sldg_ctx *c, double dt, double tol, int max_iter)
     if ((rc = do_pair(c, 0.5 * dt, false, c->ev[4], &fused))) return rc;
     c->ev_kind = 0;
     return SLDG_OK;
+}
+
+// ---- source term of the delta-g formulation ----------------------------------------
+
+int sldg_set_equilibrium(sldg_ctx *c, const double *dv_geq_dev, const double *dr_geq_dev)
+{
+    if (!c || !dv_geq_dev || !dr_geq_dev) return SLDG_EINVAL;
+    c->src_ready |= 1;
+    return cuda_fail(launch_source_profiles(c, dv_geq_dev, dr_geq_dev));
+}
+
+int sldg_set_source_fields(sldg_ctx *c, const double *dz_phi_dev, const double *dtheta_phi_dev)
+{
+    if (!c || !dz_phi_dev || !dtheta_phi_dev) return SLDG_EINVAL;
+    const size_t bytes = (size_t)c->g.lines * 8;
+    if (cudaMemcpyAsync(c->src_dz, dz_phi_dev, bytes, cudaMemcpyDeviceToDevice, c->stream) != cudaSuccess) return SLDG_ECUDA;
+    if (cudaMemcpyAsync(c->src_dth, dtheta_phi_dev, bytes, cudaMemcpyDeviceToDevice, c->stream) != cudaSuccess) return SLDG_ECUDA;
+    c->src_ready |= 2;
+    return SLDG_OK;
+}
+
+int sldg_source_step(sldg_ctx *c, double tau)
+{
+    if (!c || c->src_ready != 3) return SLDG_EINVAL;
+    cudaEventRecord(c->ev[0], c->stream);
+    cudaError_t e = launch_source_step(c, c->f[c->cur], tau);
+    cudaEventRecord(c->ev[1], c->stream);
+    c->ev_kind = 5;
+    return cuda_fail(e);
+}
+
+int sldg_strang_step_sources(sldg_ctx *c, double dt)
+{
+    if (!c || c->src_ready != 3) return SLDG_EINVAL;
+    int rc;
+    if (launch_source_step(c, c->f[c->cur], 0.5 * dt) != cudaSuccess) return SLDG_ECUDA;
+    if ((rc = sldg_strang_step(c, dt))) return rc;
+    return cuda_fail(launch_source_step(c, c->f[c->cur], 0.5 * dt));
 }
 
 int sldg_set_third_buffer(sldg_ctx *c, double *f_c_dev)

@@ -83,6 +83,9 @@ struct sldg_ctx {
     long long launches;
     int sm_count;
     FieldWs fld;
+    double *src_dz, *src_dth;  // d_z phi, d_theta phi at the nodes [Nz][Ny][Nx] (source term of the delta-g formulation)
+    double *src_gv, *src_gr;   // d_v g_eq, d_r(g_eq/r) as [Nx][Pv] tables
+    int src_ready;             // bit 0: profiles set, bit 1: fields set
     double *f_c;            // optional third state buffer (Algorithm 2 keeps the state of time level n)
 };
 
@@ -105,3 +108,7 @@ size_t field_workspace_bytes(const sldg_params *p);
 void field_carve(sldg_ctx *c, char *base);
 cudaError_t launch_field_step(sldg_ctx *c, const double *fin, double tol, int max_iter);
 cudaError_t launch_diagnostics(sldg_ctx *c, const double *fin, double r_p, double *out_host);
+size_t source_workspace_bytes(const sldg_params *p);
+void source_carve(sldg_ctx *c, char *base);
+cudaError_t launch_source_profiles(sldg_ctx *c, const double *dv_geq, const double *dr_geq);
+cudaError_t launch_source_step(sldg_ctx *c, double *f, double tau);

@@ -42,16 +42,13 @@ __device__ __forceinline__ void trace_point(const double *__restrict__ a, const 
     if (order != 1) {
         double mx = xi - 0.5 * tx * ua, my = eta - 0.5 * ty * ub;
         int fi = (int)floor(mx), fj = (int)floor(my);
-        int ci, cj;
-        if (periodic) {
-            ci = wrap_idx(i + fi, nx);
-            cj = wrap_idx(j + fj, ny);
-        } else {
-            ci = min(max(i + fi, 0), nx - 1);
-            cj = min(max(j + fj, 0), ny - 1);
-            fi = ci - i;
-            fj = cj - j;
-        }
+        // per axis: modulo the box (bitwise-periodic field) or clamped; periodic 1: both axes, 0: none, 2: y only
+        // (polar plane: x = r bounded with zero radial velocity at both ends, y = theta)
+        const bool px = periodic == 1, py = periodic == 1 || periodic == 2;
+        const int ci = px ? wrap_idx(i + fi, nx) : min(max(i + fi, 0), nx - 1);
+        const int cj = py ? wrap_idx(j + fj, ny) : min(max(j + fj, 0), ny - 1);
+        if (!px) fi = ci - i;
+        if (!py) fj = cj - j;
         bilinear_vel(a, b, nx + 1, ci, cj, mx - fi, my - fj, ua, ub);
     }
     fx = xi - tx * ua;

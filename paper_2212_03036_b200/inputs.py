@@ -313,3 +313,113 @@ def cosine_bell(spec: GridSpec, centre=(0.2 * math.pi, 0.3 * math.pi), radius=0.
     r = np.sqrt((X - centre[0]) ** 2 + (Y - centre[1]) ** 2)
     bell = np.where(r < radius, np.cos(0.5 * math.pi * np.minimum(r, radius) / radius) ** 6, 0.0)
     return np.ascontiguousarray(np.broadcast_to(bell[None, None], (1, spec.N[3], spec.N[1], spec.N[0])))
+
+
+# --------------------------------------------------------------------------------------------------
+# Polar delta-g workload: the paper's own ITG set-up.  Axis 0 is r, axis 1 theta.
+# --------------------------------------------------------------------------------------------------
+
+POLAR_RMIN, POLAR_RMAX = 0.1, 14.5
+POLAR_LZ = 1506.759067
+POLAR_RP = 0.5 * (POLAR_RMAX + POLAR_RMIN)
+POLAR_DR = 8.0          # delta r = 4 delta r_n0 / delta r_Ti
+POLAR_M, POLAR_N = 5, 1
+
+
+def polar_grid(nr, nth, nz, nv, order=2, vmax=ITG_VMAX):
+    return GridSpec(n=(nr, nth, nz, nv), order=(order, order, order, order),
+                    lo=(POLAR_RMIN, 0.0, 0.0, -vmax), hi=(POLAR_RMAX, 2.0 * math.pi, POLAR_LZ, vmax))
+
+
+def _polar_profile(r, kappa, delta):
+    """exp(-kappa delta tanh((r - r_p)/delta)) and its logarithmic derivative -kappa sech^2((r - r_p)/delta)."""
+    t = np.tanh((r - POLAR_RP) / delta)
+    return np.exp(-kappa * delta * t), -kappa * (1.0 - t * t)
+
+
+def polar_profiles(r):
+    """n0, T_i (= T_e) and their logarithmic derivatives at radii r."""
+    rr = np.linspace(POLAR_RMIN, POLAR_RMAX, 20001)
+    shape, _ = _polar_profile(rr, 0.055, 2.9)
+    integral = float(np.sum(0.5 * (shape[1:] + shape[:-1]) * np.diff(rr)))
+    c_n0 = (POLAR_RMAX - POLAR_RMIN) / integral
+    n0, dln_n0 = _polar_profile(r, 0.055, 2.9)
+    T, dln_T = _polar_profile(r, 0.27586, 1.45)
+    return c_n0 * n0, dln_n0, T, dln_T
+
+
+def polar_equilibrium(spec: GridSpec):
+    """g_eq = r f_eq, d_v g_eq and d_r(g_eq / r) = d_r f_eq at the (v, r) nodes, each [Nv][Nr]."""
+    r = spec.node_coords(0)[None, :]
+    v = spec.node_coords(3)[:, None]
+    n0, dln_n0, T, dln_T = polar_profiles(r)
+    feq = n0 / np.sqrt(2.0 * np.pi * T) * np.exp(-v * v / (2.0 * T))
+    geq = r * feq
+    dv_geq = -(v / T) * geq
+    dr_feq = feq * (dln_n0 - 0.5 * dln_T + v * v / (2.0 * T) * dln_T)
+    return np.ascontiguousarray(geq), np.ascontiguousarray(dv_geq), np.ascontiguousarray(dr_feq)
+
+
+def polar_initial_dg(spec: GridSpec, eps=1e-6):
+    """delta g(t=0) = r f_eq eps exp(-(r - r_p)^2 / delta r) cos(2 pi n z / L + m theta), [Nz][Nv][Ntheta][Nr]."""
+    geq, _, _ = polar_equilibrium(spec)
+    r = spec.node_coords(0)
+    th = spec.node_coords(1)
+    z = spec.node_coords(2)
+    env = eps * np.exp(-((r - POLAR_RP) ** 2) / POLAR_DR)
+    phase = (2.0 * np.pi * POLAR_N * z / POLAR_LZ)[:, None, None] + POLAR_M * th[None, :, None]
+    return np.ascontiguousarray(geq[None, :, None, :] * (env[None, None, :] * np.cos(phase))[:, None, :, :])
+
+
+def polar_fields(spec: GridSpec, dt, cfl=0.8):
+    """Prescribed ITG-shaped potential phi = phi0 w(r) cos(m theta + 2 pi n z / L), w = exp(-(r - r_p)^2 / delta r)
+    sin^2(pi (r - r_min)/(r_max - r_min)) (decays to zero at both radial ends, as the paper's phi does).
+    Returns a dict: a = -d_theta phi / r, b = d_r phi / r at the vertices [Nz][ntheta+1][nr+1] by centred differences of the
+    vertex values (one-sided at the radial ends; a set to exactly zero there; the theta wrap row copied), Ez
+    = -d_z phi analytic at the nodes, dz_phi = -Ez, dth_phi = the centred theta difference at the vertices interpolated
+    bilinearly to the nodes (its Gauss sum over theta telescopes to zero, the property section 3.5 asks
+    for), phi0 such that max(|a| dt / h_r, |b| dt / h_theta) = cfl."""
+    nr, nth, nz, nv = spec.n
+    hr, hth = spec.h[0], spec.h[1]
+    rv = spec.vertex_coords(0)
+    thv = spec.vertex_coords(1)[:-1]
+    z = spec.node_coords(2)
+
+    def w(r):
+        return np.exp(-((r - POLAR_RP) ** 2) / POLAR_DR) * np.sin(np.pi * (r - POLAR_RMIN) / (POLAR_RMAX - POLAR_RMIN)) ** 2
+
+    kz = 2.0 * np.pi * POLAR_N / POLAR_LZ
+    phase = POLAR_M * thv[None, :, None] + (kz * z)[:, None, None]
+    phi = w(rv)[None, None, :] * np.cos(phase)                       # [Nz][nth][nr+1], unit amplitude
+    dth = (np.roll(phi, -1, axis=1) - np.roll(phi, 1, axis=1)) / (2.0 * hth)
+    dr = np.empty_like(phi)
+    dr[:, :, 1:-1] = (phi[:, :, 2:] - phi[:, :, :-2]) / (2.0 * hr)
+    dr[:, :, 0] = (phi[:, :, 1] - phi[:, :, 0]) / hr
+    dr[:, :, -1] = (phi[:, :, -1] - phi[:, :, -2]) / hr
+    a_p = -dth / rv[None, None, :]
+    a_p[:, :, 0] = 0.0
+    a_p[:, :, -1] = 0.0
+    b_p = dr / rv[None, None, :]
+    phi0 = cfl / max(np.abs(a_p).max() * dt / hr, np.abs(b_p).max() * dt / hth)
+    a = np.empty((phi.shape[0], nth + 1, nr + 1))
+    b = np.empty_like(a)
+    for dst, src in ((a, a_p), (b, b_p)):
+        dst[:, :nth, :] = phi0 * src
+        dst[:, nth, :] = dst[:, 0, :]
+    # node values
+    r = spec.node_coords(0)
+    th = spec.node_coords(1)
+    ph = POLAR_M * th[None, :, None] + (kz * z)[:, None, None]
+    Ez = phi0 * kz * w(r)[None, None, :] * np.sin(ph)
+    xi_r = spec.unit_nodes(0)
+    xi_t = spec.unit_nodes(1)
+    d0 = phi0 * dth                                                  # [Nz][nth][nr+1] at the vertices
+    d1 = np.roll(d0, -1, axis=1)                                     # vertex j+1
+    dth_nodes = np.empty((phi.shape[0], nth, len(xi_t), nr, len(xi_r)))
+    for q, eta in enumerate(xi_t):
+        for p, xi in enumerate(xi_r):
+            dth_nodes[:, :, q, :, p] = ((1 - xi) * (1 - eta) * d0[:, :, :-1] + xi * (1 - eta) * d0[:, :, 1:]
+                                        + (1 - xi) * eta * d1[:, :, :-1] + xi * eta * d1[:, :, 1:])
+    dth_nodes = dth_nodes.reshape(phi.shape[0], nth * len(xi_t), nr * len(xi_r))
+    return {"a": a, "b": b, "Ez": np.ascontiguousarray(Ez), "dz_phi": np.ascontiguousarray(-Ez),
+            "dth_phi": np.ascontiguousarray(dth_nodes), "phi0": phi0}
