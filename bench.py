@@ -436,6 +436,30 @@ def measure_itg(workload, K, Wm, layout, world, rank, local, barrier, with_e2e, 
     torch.cuda.synchronize()
     rho_ms = ev0.elapsed_time(ev1)
     fp64_peak = s.debug_fp64_peak(5)  # TFLOP/s, measured here and now (the roof of the ALU-bound kernels)
+    # NEXT rows, outside the Strang step: the source-term substep of the delta-g formulation (one in-place pass over f,
+    # PAPER.md:269-279; synthetic equilibrium tables and field derivatives of the right shapes) and the field step
+    # (conjugate gradients to 1e-10)
+    vv = spec.node_coords(3)
+    prof = np.ascontiguousarray(np.repeat((-vv * np.exp(-0.5 * vv * vv))[:, None], spec.N[0], axis=1))
+    s.set_equilibrium(torch.from_numpy(prof).cuda(), torch.from_numpy(np.ascontiguousarray(-prof)).cuda())
+    s.set_source_fields(Ez_d, Ez_d)
+    src_ms = []
+    for k in range(6):
+        s.source_step(1e-3 if k % 2 == 0 else -1e-3)
+        src_ms.append(s.last_timing_ms()[7])
+    src_ms = float(np.median(src_ms[1:]))
+    n0v, Tev = inputs.itg_vertex_profiles(spec)
+    s.set_profiles(torch.from_numpy(n0v).cuda(), torch.from_numpy(Tev).cuda(), 1.0)
+    s.field_step(1e-10, 2000)
+    torch.cuda.synchronize()
+    ev0.record()
+    s.field_step(1e-10, 2000)
+    ev1.record()
+    torch.cuda.synchronize()
+    field_ms = ev0.elapsed_time(ev1)
+    field_iters, field_relres = s.field_info()
+    s.set_Ez(Ez_d)          # the field step overwrote the prescribed fields: put them back for the legs below
+    s.set_vxy(a_d, b_d, 1)
 
     nbytes = spec.dofs * 8.0
     step_ms = total_ms / K
@@ -446,6 +470,9 @@ def measure_itg(workload, K, Wm, layout, world, rank, local, barrier, with_e2e, 
         "advect_xy_gbs": gbs(2 * nbytes, sm["xy"]),
         "ms_single_calls": sm,
         "charge_density_gbs": gbs(nbytes, rho_ms),
+        "source_step_ms": src_ms, "source_step_gbs": gbs(2 * nbytes, src_ms),
+        "source_step_frac_of_measured_copy": gbs(2 * nbytes, src_ms) / measured_peak()[0],
+        "field_step_ms": field_ms, "field_step_cg_iterations_max": field_iters, "field_step_relres_max": field_relres,
         "xy_apply_direct_path_blocks_total": s.debug_counter(0),
         "strang_step_fused_sweep_pairs": {"zv": fused_zv, "vz": fused_vz},
         "strang_step_ms": dict(({"zv_fused": float(med[0])} if fused_zv else {"z": float(med[0]), "v": float(med[1])}),

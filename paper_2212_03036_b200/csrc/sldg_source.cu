@@ -20,44 +20,48 @@ __global__ void __launch_bounds__(256) source_profile_kernel(const double *__res
     out[t] = v < Nv ? in[(long long)v * Nx + X] : 0.0;
 }
 
+// Block <-> rows (z, Y) of Nx lines; warp <-> U lines of the row at a time, lane <-> the v pairs lane + 32 k: no
+// divisions in the inner loops, all loads of the U lines issued before the first store.
 template <int U>
 __global__ void __launch_bounds__(256) source_step_kernel(double *__restrict__ f, const double *__restrict__ dz,
                                                           const double *__restrict__ dth, const double *__restrict__ gv,
                                                           const double *__restrict__ gr, GridDev g, double tau)
 {
-    const int P2 = g.Pv / 2;
-    const long long total = g.lines * P2;
-    const long long stride = (long long)gridDim.x * blockDim.x;
-    for (long long e0 = (long long)blockIdx.x * blockDim.x + threadIdx.x; e0 < total; e0 += U * stride) {
-        double2 u[U];
-        long long at[U];
+    constexpr int MAXP = 4;  // v pairs per lane held in registers (Pv <= 256); longer lines take more passes
+    const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
+    const int Nx = g.N[0], Ny = g.N[1], P2 = g.Pv / 2;
+    const int rows = g.N[2] * Ny;
+    for (int row = blockIdx.x; row < rows; row += gridDim.x) {
+        const int Z = row / Ny, Y = row - Z * Ny;
+        double *frow = f + Z * g.sZ + Y * g.sY;
+        const double *dzr = dz + (long long)row * Nx, *dtr = dth + (long long)row * Nx;
+        for (int X0 = warp * U; X0 < Nx; X0 += 8 * U) {
+            for (int v0 = lane; v0 < P2; v0 += 32 * MAXP) {
+                double2 u[U][MAXP];
 #pragma unroll
-        for (int k = 0; k < U; ++k) {  // all loads of the U elements first
-            const long long e = e0 + k * stride;
-            at[k] = -1;
-            if (e < total) {
-                const long long line = e / P2;
-                const int v2 = (int)(e - line * P2);
-                const int X = (int)(line % g.N[0]);
-                const long long t = line / g.N[0];
-                const int Y = (int)(t % g.N[1]), Z = (int)(t / g.N[1]);
-                at[k] = Z * g.sZ + Y * g.sY + X * g.sX + 2 * v2;
-                u[k] = __ldcs(reinterpret_cast<const double2 *>(f + at[k]));
+                for (int k = 0; k < U; ++k)
+#pragma unroll
+                    for (int p = 0; p < MAXP; ++p) {
+                        const int X = X0 + k, v2 = v0 + 32 * p;
+                        if (X < Nx && v2 < P2) u[k][p] = __ldcs(reinterpret_cast<const double2 *>(frow + X * g.sX + 2 * v2));
+                    }
+#pragma unroll
+                for (int k = 0; k < U; ++k) {
+                    const int X = X0 + k;
+                    if (X >= Nx) continue;
+                    const double a = tau * __ldg(dzr + X), b = tau * __ldg(dtr + X);
+#pragma unroll
+                    for (int p = 0; p < MAXP; ++p) {
+                        const int v2 = v0 + 32 * p;
+                        if (v2 >= P2) continue;
+                        const double2 pv = __ldg(reinterpret_cast<const double2 *>(gv + (long long)X * g.Pv + 2 * v2));
+                        const double2 pr = __ldg(reinterpret_cast<const double2 *>(gr + (long long)X * g.Pv + 2 * v2));
+                        u[k][p].x += a * pv.x + b * pr.x;
+                        u[k][p].y += a * pv.y + b * pr.y;
+                        __stcs(reinterpret_cast<double2 *>(frow + X * g.sX + 2 * v2), u[k][p]);
+                    }
+                }
             }
-        }
-#pragma unroll
-        for (int k = 0; k < U; ++k) {
-            const long long e = e0 + k * stride;
-            if (at[k] < 0) continue;
-            const long long line = e / P2;
-            const int v2 = (int)(e - line * P2);
-            const int X = (int)(line % g.N[0]);
-            const double a = tau * __ldg(dz + line), b = tau * __ldg(dth + line);
-            const double2 pv = __ldg(reinterpret_cast<const double2 *>(gv + (long long)X * g.Pv + 2 * v2));
-            const double2 pr = __ldg(reinterpret_cast<const double2 *>(gr + (long long)X * g.Pv + 2 * v2));
-            u[k].x += a * pv.x + b * pr.x;
-            u[k].y += a * pv.y + b * pr.y;
-            __stcs(reinterpret_cast<double2 *>(f + at[k]), u[k]);
         }
     }
 }
@@ -97,11 +101,9 @@ cudaError_t launch_source_profiles(sldg_ctx *c, const double *dv_geq, const doub
 cudaError_t launch_source_step(sldg_ctx *c, double *f, double tau)
 {
     const GridDev &g = c->g;
-    constexpr int U = 4;
-    const long long total = g.lines * (g.Pv / 2);
-    long long nblk = (total + 256LL * U - 1) / (256LL * U);
-    const long long cap = (long long)c->sm_count * 8 * 4;
-    source_step_kernel<U><<<(unsigned)(nblk < cap ? nblk : cap), 256, 0, c->stream>>>(f, c->src_dz, c->src_dth, c->src_gv,
+    const long long rows = (long long)g.N[2] * g.N[1];
+    const long long cap = (long long)c->sm_count * 8;
+    source_step_kernel<2><<<(unsigned)(rows < cap ? rows : cap), 256, 0, c->stream>>>(f, c->src_dz, c->src_dth, c->src_gv,
                                                                                    c->src_gr, g, tau);
     c->launches++;
     return cudaGetLastError();
