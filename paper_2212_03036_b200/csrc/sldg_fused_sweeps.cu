@@ -170,6 +170,7 @@ __global__ void __launch_bounds__(FUSED_BLOCK, 1) fused_sweep_kernel(const doubl
     // z,v pair, line-wise phase: byte offset inside the plane tile of row 0 of this lane's columns after the in-place z
     // sweep (column v ends up rotated by s_z(v) cells), for the lane's own source cell (left source of its target)
     // and for the next cell (right source); the columns of a cell rotate independently (s_z depends on the v NODE)
+    const int msw = (O == 2) ? ((lane >> 3) & 1) : 0;
     uint32_t off0[CPL][O], off1[CPL][O];
 #pragma unroll
     for (int k = 0; k < CPL; ++k)
@@ -178,8 +179,14 @@ __global__ void __launch_bounds__(FUSED_BLOCK, 1) fused_sweep_kernel(const doubl
             const int cell = lane + 32 * k;
             const int c0 = (ZFIRST && cell < nv) ? cell : 0;
             const int c1 = (c0 + 1 == nv) ? 0 : c0 + 1;
-            off0[k][m] = ZFIRST ? (uint32_t)(rotoff[c0 * O + m] + c0 * O + m) * 8u : 0u;
-            off1[k][m] = ZFIRST ? (uint32_t)(rotoff[c1 * O + m] + c1 * O + m) * 8u : 0u;
+            // o = 2: a lane's cell is two adjacent columns, so one 8-byte load per lane at a fixed DOF m strides by 16
+            // bytes and the 16 lanes of a half warp cover only half of the banks (2-way conflict: 36 % of the kernel's
+            // shared-memory wavefronts).  Lanes 8-15 and 24-31 therefore take the DOFs in the opposite order: slot m of
+            // such a lane holds DOF m ^ 1 until two selects put the pair back in order (the sums keep their order of
+            // operations: bit-identical to the separate sweeps), and a half warp reads 16 distinct columns modulo 16.
+            const int md = m ^ msw;
+            off0[k][m] = ZFIRST ? (uint32_t)(rotoff[c0 * O + md] + c0 * O + md) * 8u : 0u;
+            off1[k][m] = ZFIRST ? (uint32_t)(rotoff[c1 * O + md] + c1 * O + md) * 8u : 0u;
         }
     double ez_next = 0.0;
     int col = blockIdx.x, par = 0;
@@ -322,6 +329,10 @@ __global__ void __launch_bounds__(FUSED_BLOCK, 1) fused_sweep_kernel(const doubl
                             t1 = min(t1, t1 - plane_b);
                             u0[m] = lds_f64(tile_b + t0);
                             u1[m] = lds_f64(tile_b + t1);
+                        }
+                        if (O == 2 && msw) {
+                            double t = u0[0]; u0[0] = u0[O - 1]; u0[O - 1] = t;
+                            t = u1[0]; u1[0] = u1[O - 1]; u1[O - 1] = t;
                         }
                         int c = cell - s;  // the target whose left source cell this is
                         if (c < 0) c += nv;
