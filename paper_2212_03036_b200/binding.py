@@ -117,7 +117,10 @@ def make_params(spec, layout=0, max_stencil=3):
 class Sldg:
     """One SLDG context on the current CUDA device.  Tensors are torch CUDA tensors (fp64)."""
 
-    def __init__(self, spec, device="cuda", layout=0, stream=None):
+    def __init__(self, spec, device="cuda", layout=0, stream=None, guard_bytes=0):
+        """guard_bytes > 0 (a multiple of 256): every device buffer handed to the library is the middle of a larger
+        allocation whose margins are filled with a byte pattern; check_guards() verifies that no kernel wrote outside
+        its buffers (the pool's compute-sanitizer is closed: DESIGN.md section 12)."""
         import torch
 
         if not torch.cuda.is_available():
@@ -132,9 +135,18 @@ class Sldg:
         if sb == 0 or wb == 0:
             raise SldgError(SLDG_EINVAL, "sldg_state_bytes")
         self.state_bytes, self.workspace_bytes = sb, wb
-        self.f_a = torch.empty(sb // 8, dtype=torch.float64, device=self.device)
-        self.f_b = torch.empty(sb // 8, dtype=torch.float64, device=self.device)
-        self.workspace = torch.empty(wb, dtype=torch.uint8, device=self.device)
+        assert guard_bytes % 256 == 0
+        self.guard_bytes = guard_bytes
+        self._guarded = []
+
+        def alloc(nbytes):
+            raw = torch.full((nbytes + 2 * guard_bytes,), 0xA5, dtype=torch.uint8, device=self.device)
+            self._guarded.append(raw)
+            return raw[guard_bytes:guard_bytes + nbytes]
+
+        self.f_a = alloc(sb).view(torch.float64)
+        self.f_b = alloc(sb).view(torch.float64)
+        self.workspace = alloc(wb)
         self.stream = stream if stream is not None else torch.cuda.current_stream(self.device)
         h = C.c_void_p()
         with torch.cuda.device(self.device):
@@ -146,6 +158,12 @@ class Sldg:
     def _chk(self, rc, what):
         if rc != 0:
             raise SldgError(rc, what)
+
+    def check_guards(self):
+        """True if the margins around every buffer still hold their pattern (always True without guard_bytes)."""
+        self.torch.cuda.synchronize(self.device)
+        g = self.guard_bytes
+        return all(bool((raw[:g] == 0xA5).all()) and bool((raw[raw.numel() - g:] == 0xA5).all()) for raw in self._guarded) if g else True
 
     def close(self):
         if getattr(self, "h", None):
@@ -272,7 +290,10 @@ class Sldg:
 
     def step_algorithm2(self, dt, tol=1e-13, max_iter=2000):
         if getattr(self, "f_c", None) is None:  # the third copy of f
-            self.f_c = self.torch.empty(self.state_bytes // 8, dtype=self.torch.float64, device=self.device)
+            g = self.guard_bytes
+            raw = self.torch.full((self.state_bytes + 2 * g,), 0xA5, dtype=self.torch.uint8, device=self.device)
+            self._guarded.append(raw)
+            self.f_c = raw[g:g + self.state_bytes].view(self.torch.float64)
             self._chk(self.L.sldg_set_third_buffer(self.h, self.f_c.data_ptr()), "sldg_set_third_buffer")
         self._chk(self.L.sldg_step_algorithm2(self.h, float(dt), float(tol), int(max_iter)), "sldg_step_algorithm2")
 
