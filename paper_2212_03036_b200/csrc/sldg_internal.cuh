@@ -75,6 +75,7 @@ struct sldg_ctx {
     cudaStream_t cstream;   // copy stream: sldg_strang_step_host uploads a, b under the first sweeps
     cudaEvent_t cev[2];     // fork / join of that upload
     int ab_pending;         // an upload of a, b is in flight on cstream: the next 2d step waits for it
+    int tile;               // z-tiled pair kernel: 1 when the whole plane does not fit, 2 first (SLDG_FORCE_TILE), 0 never (SLDG_NO_TILE)
     int fuse, last_fused;   // fuse: sldg_strang_step runs each pair of adjacent sweeps in one pass
     size_t n_partials;
     int trace_order, vel_periodic;
@@ -104,6 +105,7 @@ cudaError_t launch_xy_apply(sldg_ctx *c, const double *fin, double *fout);
 cudaError_t count_weight_blocks(sldg_ctx *c, long long *total_host);
 cudaError_t launch_fused_sweeps(sldg_ctx *c, const double *fin, double *fout, double tau_z, double tau_v, bool z_first,
                                 bool z_only = false);
+cudaError_t launch_tiled_sweeps(sldg_ctx *c, const double *fin, double *fout, double tau_z, double tau_v, bool z_first);
 size_t field_workspace_bytes(const sldg_params *p);
 void field_carve(sldg_ctx *c, char *base);
 cudaError_t launch_field_step(sldg_ctx *c, const double *fin, double tol, int max_iter);

@@ -125,7 +125,7 @@ def test_c4_strang_step_fused_equals_separate_calls_and_conserves_mass(torch, ca
     s.strang_step(DT)
     s.check()
     # o=2: both pairs run fused; o=3 (144 x 144 planes): only v,z does
-    assert (int(s.last_timing_ms()[6]) & 6) == (6 if o == 2 else 4), "the fused sweep pairs did not run at bench size"
+    assert (int(s.last_timing_ms()[6]) & 6) == (6 if o == 2 else 4), "the fused sweep pairs did not run at bench size"  # o = 3: the z,v pair stays two kernels (sldg_fused_sweeps.cu, sldg_tiled_sweeps.cu say why)
     m1 = float(s.mass().cpu()[0])
     assert abs(m1 - m0) <= 1e-13 * abs(m0)
     # the same step as five separate calls in a second context

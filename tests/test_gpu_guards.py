@@ -24,11 +24,13 @@ CASES = [(2, (16, 16, 8, 16)), (3, (9, 7, 3, 8)), (1, (12, 10, 5, 16)), (2, (5, 
 
 
 @pytest.mark.parametrize("o,cells", CASES)
-@pytest.mark.parametrize("fuse", [True, False])
+@pytest.mark.parametrize("fuse", ["plane", "tiled", "separate"])
 def test_no_kernel_writes_outside_its_buffers(torch, monkeypatch, o, cells, fuse):
     from paper_2212_03036_b200.binding import Sldg, SldgError
-    if not fuse:
+    if fuse == "separate":
         monkeypatch.setenv("SLDG_NO_FUSE", "1")
+    if fuse == "tiled":
+        monkeypatch.setenv("SLDG_FORCE_TILE", "1")
     spec = inputs.itg_grid(*cells, o)
     f = inputs.itg_initial_f(spec, eps=0.05)
     cu = lambda x: torch.from_numpy(np.ascontiguousarray(x)).cuda()
