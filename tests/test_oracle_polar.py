@@ -93,3 +93,84 @@ def test_polar_step_conserves_mass_and_nothing_crosses_the_radial_ends():
     g2 = polar.strang_step_sources(spec, inputs.polar_initial_dg(spec, 0.1), fl, dv, dr, dt)
     md = oracle.mass(spec, np.ascontiguousarray(g2)) - oracle.mass(spec, inputs.polar_initial_dg(spec, 0.1))
     assert abs(md) < 1e-13 * oracle.mass(spec, np.abs(g2))
+
+
+def _polar_manufactured(nr, nth=16, nz=2):
+    spec = inputs.GridSpec(n=(nr, nth, nz, 2), order=(2, 2, 2, 2), lo=(0.5, 0.0, 0.0, -1.0), hi=(2.5, 2 * math.pi, 3.0, 1.0))
+    rv = spec.vertex_coords(0)
+    th = spec.vertex_coords(1)[:-1]
+    zeq = (np.arange(spec.N[2]) + 0.5) * spec.h[2] / 2
+    R, TH, Z = rv[None, None, :], th[None, :, None], zeq[:, None, None]
+    q = math.pi / (2 * 2.0)                      # u(r) = cos(q (r - r_min)): u'(r_min) = 0, u(r_max) = 0
+    u, ur, urr = np.cos(q * (R - 0.5)), -q * np.sin(q * (R - 0.5)), -q * q * np.cos(q * (R - 0.5))
+    kz = 2 * math.pi / 3.0
+    ang = np.cos(3 * TH)
+    g = 1.0 + 0.5 * np.cos(kz * Z)               # z profile with mean 1: <phi> = u ang
+    dln = 0.3 * np.sin(R)                        # n0'/n0
+    Te = 1.0 + 0.2 * R
+    rhs = (-(urr + (1.0 / R + dln) * ur) * ang + 9.0 * u * ang / R ** 2) * g + u * ang * (g - 1.0) / Te
+    return spec, rhs, dln[0, 0], Te[0, 0], u * ang * g
+
+
+def test_polar_quasi_neutrality_manufactured_solution_second_order():
+    # eq. (2) with Neumann at r_min and Dirichlet at r_max: a dropped 1/r or n0'/n0 term, a wrong
+    # theta symbol or a wrong <phi> fails the convergence
+    errs = []
+    for nr in (16, 32):
+        spec, rhs, dln, Te, exact = _polar_manufactured(nr)
+        phi = polar.polar_solve_phi(spec, rhs, dln, Te)
+        errs.append(np.abs(phi - exact).max())
+        assert np.abs(phi[:, :, -1]).max() == 0.0
+    assert errs[0] < 5e-3 and 3.5 < errs[0] / errs[1] < 4.5, errs
+
+
+def test_polar_solver_single_mode_against_a_dense_solve():
+    # one (kz, m) mode: the solution stays in that mode and equals the dense solve of the difference equations written
+    # out here with numpy.linalg (independent of the banded routine and of the FFT bookkeeping)
+    spec = inputs.GridSpec(n=(12, 8, 3, 2), order=(2, 2, 2, 2), lo=(0.3, 0.0, 0.0, -1.0), hi=(2.1, 2 * math.pi, 5.0, 1.0))
+    rv = spec.vertex_coords(0)
+    th = spec.vertex_coords(1)[:-1]
+    zeq = (np.arange(spec.N[2]) + 0.5) * spec.h[2] / 2
+    prof = np.sin(1.7 * rv) + 0.3
+    m, kzi = 2, 1
+    rhs = prof[None, None, :] * np.cos(m * th[None, :, None] + 2 * math.pi * kzi * zeq[:, None, None] / 5.0)
+    dln, Te = 0.2 * rv, 0.7 + 0.1 * rv
+    phi = polar.polar_solve_phi(spec, rhs, dln, Te)
+    nr, h = 12, spec.h[0]
+    M = np.zeros((nr, nr))
+    for i in range(nr):
+        adv = (1.0 / rv[i] + dln[i]) / (2 * h)
+        M[i, i] = 2 / h ** 2 + m * m / rv[i] ** 2 + 1.0 / Te[i]
+        if i + 1 < nr:
+            M[i, i + 1] = -1 / h ** 2 - adv
+        if i > 0:
+            M[i, i - 1] = -1 / h ** 2 + adv
+        else:
+            M[0, 1] += -1 / h ** 2 + adv
+    amp = np.concatenate([np.linalg.solve(M, prof[:nr]), [0.0]])
+    want = amp[None, None, :] * np.cos(m * th[None, :, None] + 2 * math.pi * kzi * zeq[:, None, None] / 5.0)
+    assert np.abs(phi - want).max() < 1e-12 * np.abs(want).max()
+
+
+def test_polar_resampling_and_derived_fields():
+    spec = inputs.polar_grid(6, 8, 3, 4, 2)
+    r, th, z = spec.node_coords(0), spec.node_coords(1), spec.node_coords(2)
+    rho = (1.0 + 0.01 * z)[:, None, None] * (2.0 + 0.1 * r)[None, None, :] * np.ones_like(th)[None, :, None]
+    out = polar.polar_resample(spec, rho)
+    rv = spec.vertex_coords(0)
+    zeq = (np.arange(spec.N[2]) + 0.5) * spec.h[2] / 2
+    want = (1.0 + 0.01 * zeq)[:, None, None] * (2.0 + 0.1 * rv)[None, None, :] * np.ones(8)[None, :, None]
+    assert np.abs(out - want).max() < 1e-12      # linear in r: exact at every vertex, the radial ends included
+    # derived fields of one Fourier mode: centred differences multiply by sin(k h)/h; radial ends of a are zero
+    thv = spec.vertex_coords(1)[:-1]
+    phi = (np.sin(rv)[None, None, :] * np.cos(3 * thv[None, :, None] + 2 * math.pi * zeq[:, None, None] / spec.hi[2]))
+    a, b, e, dth = polar.polar_derive(spec, phi)
+    hth, hz = spec.h[1], spec.h[2] / 2
+    ph = 3 * thv[None, :, None] + 2 * math.pi * zeq[:, None, None] / spec.hi[2]
+    assert np.abs(dth - (-np.sin(3 * hth) / hth * np.sin(rv)[None, None, :] * np.sin(ph))).max() < 1e-12
+    assert np.abs(a[:, :, 1:-1] - (-dth / rv[None, None, :])[:, :, 1:-1]).max() < 1e-15
+    assert np.all(a[:, :, 0] == 0.0) and np.all(a[:, :, -1] == 0.0) and np.all(b[:, :, 0] == 0.0)
+    kz = 2 * math.pi / spec.hi[2]
+    assert np.abs(e - (np.sin(kz * hz) / hz * np.sin(rv)[None, None, :] * np.sin(ph))).max() < 1e-12
+    h = spec.h[0]
+    assert np.abs(b[:, :, 3] - (phi[:, :, 4] - phi[:, :, 2]) / (2 * h) / rv[3]).max() < 1e-15
