@@ -205,6 +205,20 @@ int sldg_source_step(sldg_ctx *ctx, double tau);
 /* Algorithm 1 steps 2-4, 6-9 with the fields currently set: source(dt/2), z(dt/2), v(dt/2), 2d(dt),
  * v(dt/2), z(dt/2), source(dt/2). */
 int sldg_strang_step_sources(sldg_ctx *ctx, double dt);
+/* The paper's quasi-neutrality solver in polar coordinates (eq. 2; Neumann at r_min, Dirichlet at r_max,
+ * PAPER.md:43; Fourier transform in theta and z, second-order differences and a tridiagonal solve in r):
+ * sldg_set_polar_profiles: r n0(r), n0'/n0 (r), T_e(r) at the nr + 1 radial vertices (device doubles, copied).
+ * sldg_polar_field_step: charge density of the current delta-g -> rhs = rho~/(r n0) on the field grid (nr + 1 radial
+ * vertices x ntheta x Nz equidistant z points) -> phi -> drift (-d_theta phi/r, d_r phi/r) at the vertices with zero
+ * radial ends, E_z, d_z phi and d_theta phi at the nodes, written where sldg_set_vxy(.., 2), sldg_set_Ez and
+ * sldg_set_source_fields put them.  <phi> = z average (R21). */
+int sldg_set_polar_profiles(sldg_ctx *ctx, const double *r_n0_dev, const double *dln_n0_dev, const double *Te_dev);
+int sldg_polar_field_step(sldg_ctx *ctx);
+int sldg_get_polar_phi(sldg_ctx *ctx, double *phi_dev);                 /* [Nz][ntheta][nr+1] */
+int sldg_get_source_fields(sldg_ctx *ctx, double *dz_phi_dev, double *dtheta_phi_dev); /* [Nz][Ntheta][Nr], either may be NULL */
+/* Algorithm 1 with all nine steps in the delta-g formulation: field, source(dt/2), z(dt/2), v(dt/2),
+ * field, 2d(dt), v(dt/2), z(dt/2), source(dt/2).  Needs sldg_set_polar_profiles and sldg_set_equilibrium. */
+int sldg_step_algorithm1_polar(sldg_ctx *ctx, double dt);
 const char *sldg_strerror(int code);
 
 #ifdef __cplusplus

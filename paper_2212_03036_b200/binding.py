@@ -25,6 +25,8 @@ EXPORTS = [
     "sldg_set_profiles", "sldg_field_step", "sldg_field_info", "sldg_get_phi", "sldg_get_fields", "sldg_diagnostics",
     "sldg_step_algorithm1", "sldg_set_third_buffer", "sldg_step_algorithm2",
     "sldg_set_equilibrium", "sldg_set_source_fields", "sldg_source_step", "sldg_strang_step_sources",
+    "sldg_set_polar_profiles", "sldg_polar_field_step", "sldg_get_polar_phi", "sldg_get_source_fields",
+    "sldg_step_algorithm1_polar",
 ]
 
 
@@ -98,6 +100,11 @@ def load_library():
     L.sldg_set_source_fields.argtypes = [vp, dp, dp]
     L.sldg_source_step.argtypes = [vp, C.c_double]
     L.sldg_strang_step_sources.argtypes = [vp, C.c_double]
+    L.sldg_set_polar_profiles.argtypes = [vp, dp, dp, dp]
+    L.sldg_polar_field_step.argtypes = [vp]
+    L.sldg_get_polar_phi.argtypes = [vp, dp]
+    L.sldg_get_source_fields.argtypes = [vp, dp, dp]
+    L.sldg_step_algorithm1_polar.argtypes = [vp, C.c_double]
     _lib = L
     return L
 
@@ -313,6 +320,30 @@ class Sldg:
 
     def strang_step_sources(self, dt):
         self._chk(self.L.sldg_strang_step_sources(self.h, float(dt)), "sldg_strang_step_sources")
+
+    def set_polar_profiles(self, r_n0, dln_n0, Te):
+        for u in (r_n0, dln_n0, Te):
+            assert u.is_cuda and u.dtype == self.torch.float64 and u.is_contiguous() and u.numel() == self.spec.n[0] + 1
+        self._chk(self.L.sldg_set_polar_profiles(self.h, r_n0.data_ptr(), dln_n0.data_ptr(), Te.data_ptr()), "sldg_set_polar_profiles")
+
+    def polar_field_step(self):
+        self._chk(self.L.sldg_polar_field_step(self.h), "sldg_polar_field_step")
+
+    def get_polar_phi(self):
+        out = self.torch.empty((self.spec.N[2], self.spec.n[1], self.spec.n[0] + 1), dtype=self.torch.float64, device=self.device)
+        self._chk(self.L.sldg_get_polar_phi(self.h, out.data_ptr()), "sldg_get_polar_phi")
+        return out
+
+    def get_source_fields(self):
+        t = self.torch
+        Nx, Ny, Nz, _ = self.spec.N
+        dz = t.empty((Nz, Ny, Nx), dtype=t.float64, device=self.device)
+        dth = t.empty_like(dz)
+        self._chk(self.L.sldg_get_source_fields(self.h, dz.data_ptr(), dth.data_ptr()), "sldg_get_source_fields")
+        return dz, dth
+
+    def step_algorithm1_polar(self, dt):
+        self._chk(self.L.sldg_step_algorithm1_polar(self.h, float(dt)), "sldg_step_algorithm1_polar")
 
     # ---- diagnostics ---------------------------------------------------------------------------
     def check(self):

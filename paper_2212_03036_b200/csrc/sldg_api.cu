@@ -51,7 +51,7 @@ void fill_grid(const sldg_params *p, GridDev *g)
 }
 
 struct WorkspaceMap {
-    size_t Ez, va, vb, hdr, W, partials, rho, scalar, err, stage_ok, field, source, total;
+    size_t Ez, va, vb, hdr, W, partials, rho, scalar, err, stage_ok, field, source, polar, total;
     size_t n_partials;
 };
 
@@ -77,6 +77,7 @@ WorkspaceMap map_workspace(const sldg_params *p)
     m.stage_ok = take(xy_apply_stage_flags(p) * 4);
     m.field = take(field_workspace_bytes(p));
     m.source = take(source_workspace_bytes(p));
+    m.polar = take(polar_workspace_bytes(p));
     m.total = off;
     return m;
 }
@@ -273,6 +274,7 @@ int sldg_create(const sldg_params *p, double *f_a_dev, double *f_b_dev, void *wo
     c->stage_ok = (int32_t *)(ws + m.stage_ok);
     field_carve(c, ws + m.field);
     source_carve(c, ws + m.source);
+    polar_carve(c, ws + m.polar);
     c->fuse = getenv("SLDG_NO_FUSE") ? 0 : 1;
     c->tile = getenv("SLDG_NO_TILE") ? 0 : (getenv("SLDG_FORCE_TILE") ? 2 : 1);
     c->trace_order = 2;
@@ -715,6 +717,49 @@ int sldg_strang_step_sources(sldg_ctx *c, double dt)
     if (launch_source_step(c, c->f[c->cur], 0.5 * dt) != cudaSuccess) return SLDG_ECUDA;
     if ((rc = sldg_strang_step(c, dt))) return rc;
     return cuda_fail(launch_source_step(c, c->f[c->cur], 0.5 * dt));
+}
+
+int sldg_set_polar_profiles(sldg_ctx *c, const double *r_n0_dev, const double *dln_n0_dev, const double *Te_dev)
+{
+    if (!c || !r_n0_dev || !dln_n0_dev || !Te_dev || c->g.n[0] < 3) return SLDG_EINVAL;
+    return cuda_fail(launch_polar_profiles(c, r_n0_dev, dln_n0_dev, Te_dev));
+}
+
+int sldg_polar_field_step(sldg_ctx *c)
+{
+    if (!c || !c->pol.ready) return SLDG_EINVAL;
+    return cuda_fail(launch_polar_field_step(c, c->f[c->cur]));
+}
+
+int sldg_get_polar_phi(sldg_ctx *c, double *phi_dev)
+{
+    if (!c || !phi_dev || !c->pol.have_phi) return SLDG_EINVAL;
+    const size_t bytes = (size_t)c->g.N[2] * c->g.n[1] * (c->g.n[0] + 1) * 8;
+    return cuda_fail(cudaMemcpyAsync(phi_dev, c->pol.phi, bytes, cudaMemcpyDeviceToDevice, c->stream));
+}
+
+int sldg_get_source_fields(sldg_ctx *c, double *dz_phi_dev, double *dtheta_phi_dev)
+{
+    if (!c || !(c->src_ready & 2)) return SLDG_EINVAL;
+    const size_t bytes = (size_t)c->g.lines * 8;
+    if (dz_phi_dev && cudaMemcpyAsync(dz_phi_dev, c->src_dz, bytes, cudaMemcpyDeviceToDevice, c->stream) != cudaSuccess) return SLDG_ECUDA;
+    if (dtheta_phi_dev && cudaMemcpyAsync(dtheta_phi_dev, c->src_dth, bytes, cudaMemcpyDeviceToDevice, c->stream) != cudaSuccess) return SLDG_ECUDA;
+    return SLDG_OK;
+}
+
+int sldg_step_algorithm1_polar(sldg_ctx *c, double dt)
+{
+    if (!c || !c->pol.ready || !(c->src_ready & 1)) return SLDG_EINVAL;
+    int rc, fused;
+    if ((rc = sldg_polar_field_step(c))) return rc;                                          // 1
+    if (launch_source_step(c, c->f[c->cur], 0.5 * dt) != cudaSuccess) return SLDG_ECUDA;     // 2
+    if ((rc = do_pair(c, 0.5 * dt, true, c->ev[1], &fused))) return rc;                       // 3, 4
+    if ((rc = sldg_polar_field_step(c))) return rc;                                          // 5
+    if ((rc = do_xy(c, dt, 2))) return rc;                                                    // 6
+    if ((rc = do_pair(c, 0.5 * dt, false, c->ev[4], &fused))) return rc;                      // 7, 8
+    if (launch_source_step(c, c->f[c->cur], 0.5 * dt) != cudaSuccess) return SLDG_ECUDA;     // 9
+    c->ev_kind = 0;
+    return SLDG_OK;
 }
 
 int sldg_set_third_buffer(sldg_ctx *c, double *f_c_dev)

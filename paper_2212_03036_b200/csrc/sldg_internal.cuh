@@ -54,6 +54,14 @@ struct FieldWs {
     int have_profiles, have_phi;
 };
 
+// Workspace of the polar quasi-neutrality solver (sldg_polar_field.cu): profiles at the r vertices, two complex arrays on
+// the field grid [Nz][nth][nr+1], the potential, the Thomas scratch, the twiddle tables.
+struct PolarWs {
+    double *rn0, *dln, *Te, *phi, *cp;
+    double2 *ca, *cb, *tw_th, *tw_z;
+    int ready, have_phi;
+};
+
 struct sldg_ctx {
     sldg_params p;
     GridDev g;
@@ -84,6 +92,7 @@ struct sldg_ctx {
     long long launches;
     int sm_count;
     FieldWs fld;
+    PolarWs pol;
     double *src_dz, *src_dth;  // d_z phi, d_theta phi at the nodes [Nz][Ny][Nx] (source term of the delta-g formulation)
     double *src_gv, *src_gr;   // d_v g_eq, d_r(g_eq/r) as [Nx][Pv] tables
     int src_ready;             // bit 0: profiles set, bit 1: fields set
@@ -114,3 +123,7 @@ size_t source_workspace_bytes(const sldg_params *p);
 void source_carve(sldg_ctx *c, char *base);
 cudaError_t launch_source_profiles(sldg_ctx *c, const double *dv_geq, const double *dr_geq);
 cudaError_t launch_source_step(sldg_ctx *c, double *f, double tau);
+size_t polar_workspace_bytes(const sldg_params *p);
+void polar_carve(sldg_ctx *c, char *base);
+cudaError_t launch_polar_profiles(sldg_ctx *c, const double *rn0, const double *dln, const double *Te);
+cudaError_t launch_polar_field_step(sldg_ctx *c, const double *fin);

@@ -94,3 +94,59 @@ def test_data_at_the_radial_ends_stays_there(torch):
     inner0[:, :, :, half:] = 0.0
     assert abs(oracle.mass(spec, inner) - oracle.mass(spec, inner0)) <= 1e-12 * oracle.mass(spec, f)
     s.close()
+
+
+def _polar_ctx(torch, spec, dg):
+    from paper_2212_03036_b200.binding import Sldg
+    cu = lambda x: torch.from_numpy(np.ascontiguousarray(x)).cuda()
+    rv = spec.vertex_coords(0)
+    n0, dln_n0, T, _ = inputs.polar_profiles(rv)
+    _, dv, dr = inputs.polar_equilibrium(spec)
+    s = Sldg(spec)
+    s.import_state(cu(dg))
+    s.set_polar_profiles(cu(rv * n0), cu(dln_n0), cu(T))
+    s.set_equilibrium(cu(dv), cu(dr))
+    return s, n0, dln_n0, T, dv, dr
+
+
+@pytest.mark.parametrize("o,cells", [(2, (16, 24, 4, 16)), (3, (8, 12, 2, 8)), (1, (9, 12, 5, 12)), (2, (20, 15, 3, 8))])
+def test_polar_quasi_neutrality_solve_matches_the_oracle(torch, o, cells):
+    # eq. (2) as printed: Fourier sums in theta and z, tridiagonal solves in r (Neumann / Dirichlet), drift with zero
+    # radial ends -- a direct solver on both sides, so the potential agrees to round-off
+    spec = inputs.polar_grid(*cells, o)
+    dg = inputs.polar_initial_dg(spec, eps=0.1)
+    s, n0, dln_n0, T, dv, dr = _polar_ctx(torch, spec, dg)
+    s.polar_field_step()
+    want = polar.polar_field_step(spec, dg, n0, dln_n0, T)
+    phi = s.get_polar_phi().cpu().numpy()
+    scale = np.abs(want["phi"]).max()
+    assert np.abs(phi - want["phi"]).max() <= 1e-11 * scale
+    Ez, a, b = (x.cpu().numpy() for x in s.get_fields())
+    dz, dth = (x.cpu().numpy() for x in s.get_source_fields())
+    assert np.abs(a - want["a"]).max() <= 1e-10 * np.abs(want["a"]).max()
+    assert np.abs(b - want["b"]).max() <= 1e-10 * np.abs(want["b"]).max()
+    assert np.abs(Ez - want["Ez"]).max() <= 1e-10 * np.abs(want["Ez"]).max()
+    assert np.abs(dz - want["dz_phi"]).max() <= 1e-10 * np.abs(want["Ez"]).max()
+    assert np.abs(dth - want["dth_phi"]).max() <= 1e-10 * np.abs(want["dth_phi"]).max()
+    assert np.all(a[:, :, 0] == 0.0) and np.all(a[:, :, -1] == 0.0)
+    assert np.array_equal(a[:, -1], a[:, 0]) and np.array_equal(b[:, -1], b[:, 0])
+    s.close()
+
+
+@pytest.mark.parametrize("o,cells,eps", [(2, (16, 24, 4, 16), 1e-6), (2, (16, 24, 4, 16), 0.05), (3, (8, 12, 2, 8), 0.02)])
+def test_polar_algorithm1_self_consistent_steps(torch, o, cells, eps):
+    # the paper's own set-up on a small mesh: Algorithm 1 with all nine steps, potential from eq. (2)
+    spec = inputs.polar_grid(*cells, o)
+    dg = inputs.polar_initial_dg(spec, eps=eps)
+    s, n0, dln_n0, T, dv, dr = _polar_ctx(torch, spec, dg)
+    ref = dg.copy()
+    dt = 4.0
+    for n in range(4):
+        s.step_algorithm1_polar(dt)
+        ref, fs = polar.polar_algorithm1_step(spec, ref, n0, dln_n0, T, dv, dr, dt)
+    s.check()
+    got = s.export_state().cpu().numpy()
+    assert np.abs(got - ref).max() <= TOL * np.abs(ref).max()
+    scale = oracle.mass(spec, np.abs(ref))
+    assert abs(float(s.mass().cpu()[0]) - oracle.mass(spec, dg)) <= 1e-13 * scale
+    s.close()
