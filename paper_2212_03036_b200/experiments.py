@@ -76,7 +76,79 @@ def format_table(rows):
     return "\n".join(out)
 
 
-if __name__ == "__main__":
+def _main_swirl():
     for o in (2, 3):
         print(f"o = {o} (k = {o - 1}); the paper's Table 1 is k = 1: L2 orders 2.39, 2.42, 2.29")
         print(format_table(swirl_convergence(order=o)))
+
+
+def polar_itg(cells=(64, 64, 32, 64), order=2, dt=4.0, steps=1500, eps=1e-6, every=25):
+    """The paper's ion-temperature-gradient run through the library: delta-g formulation in polar
+    coordinates, Algorithm 1 with all nine steps, potential from eq. (2).  Returns rows (t, electric energy
+    sqrt(int phi^2(r_p, theta, z) dtheta dz), change of the mass of delta-g relative to the total mass int g_eq) every
+    `every` steps.  The paper observes an exponential growth of the electric energy until nonlinear saturation."""
+    import torch
+
+    from .binding import Sldg
+
+    spec = inputs.polar_grid(*cells, order)
+    dg = inputs.polar_initial_dg(spec, eps=eps)
+    rv = spec.vertex_coords(0)
+    n0, dln_n0, T, _ = inputs.polar_profiles(rv)
+    _, dv, dr = inputs.polar_equilibrium(spec)
+    cu = lambda x: torch.from_numpy(np.ascontiguousarray(x)).cuda()
+    s = Sldg(spec)
+    s.import_state_host(dg)
+    s.set_polar_profiles(cu(rv * n0), cu(dln_n0), cu(T))
+    s.set_equilibrium(cu(dv), cu(dr))
+    ip = int(round((inputs.POLAR_RP - spec.lo[0]) / spec.h[0]))      # the r vertex at r_p
+    w = spec.h[1] * spec.h[2] / spec.order[2]
+    geq, _, _ = inputs.polar_equilibrium(spec)
+    _, wq = np.polynomial.legendre.leggauss(order)
+    wr = np.tile(0.5 * wq, spec.n[0]) * spec.h[0]
+    wv = np.tile(0.5 * wq, spec.n[3]) * spec.h[3]
+    scale = float((geq * wv[:, None] * wr[None, :]).sum() * (spec.hi[1] - spec.lo[1]) * (spec.hi[2] - spec.lo[2]))  # int g_eq
+    m0 = float(s.mass().cpu()[0])
+    rows = []
+    from .binding import SldgError
+    for n in range(steps + 1):
+        if n % every == 0:
+            try:  # the run ends where an upstream cell leaves the 3x3 stencil (PAPER.md:293): the nonlinear phase
+                s.check()
+            except SldgError as err:
+                rows.append({"t": n * dt, "electric": float("nan"), "mass_change": float("nan"), "stopped": str(err)})
+                break
+            s.polar_field_step()
+            phi = s.get_polar_phi()
+            e = float(torch.sqrt((phi[:, :, ip] ** 2).sum() * w))
+            rows.append({"t": n * dt, "electric": e, "mass_change": abs(float(s.mass().cpu()[0]) - m0) / scale})
+        if n < steps:
+            s.step_algorithm1_polar(dt)
+    s.close()
+    return rows
+
+
+def growth_rate(rows, t0, t1):
+    """Least-squares slope of log(electric energy) over t in [t0, t1]."""
+    sel = [(r["t"], math.log(r["electric"])) for r in rows if t0 <= r["t"] <= t1 and r["electric"] > 0]
+    t = np.array([a for a, _ in sel])
+    y = np.array([b for _, b in sel])
+    return float(np.polyfit(t, y, 1)[0])
+
+
+if __name__ == "__main__":
+    import sys
+
+    if len(sys.argv) > 1 and sys.argv[1] == "itg":
+        steps = int(sys.argv[2]) if len(sys.argv) > 2 else 1500
+        rows = polar_itg(steps=steps)
+        print("| t | electric energy | change of the total mass (relative to int g_eq) |")
+        print("|---|---|---|")
+        for r in rows:
+            print(f"| {r['t']:.0f} | {r['electric']:.4e} | {r['mass_change']:.1e} |" + (f" {r['stopped']}" if "stopped" in r else ""))
+        rows = [r for r in rows if "stopped" not in r]
+        T = rows[-1]["t"]
+        for a, b in ((0.2 * T, 0.5 * T), (0.4 * T, 0.7 * T), (0.5 * T, 0.9 * T)):
+            print(f"growth rate of the electric energy over t in [{a:.0f}, {b:.0f}]: {growth_rate(rows, a, b):.5f}")
+    else:
+        _main_swirl()
