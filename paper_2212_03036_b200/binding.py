@@ -147,6 +147,8 @@ class Sldg:
         self._guarded = []
 
         def alloc(nbytes):
+            if guard_bytes == 0:
+                return torch.empty(nbytes, dtype=torch.uint8, device=self.device)
             raw = torch.full((nbytes + 2 * guard_bytes,), 0xA5, dtype=torch.uint8, device=self.device)
             self._guarded.append(raw)
             return raw[guard_bytes:guard_bytes + nbytes]
@@ -298,9 +300,12 @@ class Sldg:
     def step_algorithm2(self, dt, tol=1e-13, max_iter=2000):
         if getattr(self, "f_c", None) is None:  # the third copy of f
             g = self.guard_bytes
-            raw = self.torch.full((self.state_bytes + 2 * g,), 0xA5, dtype=self.torch.uint8, device=self.device)
-            self._guarded.append(raw)
-            self.f_c = raw[g:g + self.state_bytes].view(self.torch.float64)
+            if g == 0:
+                self.f_c = self.torch.empty(self.state_bytes // 8, dtype=self.torch.float64, device=self.device)
+            else:
+                raw = self.torch.full((self.state_bytes + 2 * g,), 0xA5, dtype=self.torch.uint8, device=self.device)
+                self._guarded.append(raw)
+                self.f_c = raw[g:g + self.state_bytes].view(self.torch.float64)
             self._chk(self.L.sldg_set_third_buffer(self.h, self.f_c.data_ptr()), "sldg_set_third_buffer")
         self._chk(self.L.sldg_step_algorithm2(self.h, float(dt), float(tol), int(max_iter)), "sldg_step_algorithm2")
 
