@@ -219,6 +219,8 @@ int sldg_get_source_fields(sldg_ctx *ctx, double *dz_phi_dev, double *dtheta_phi
 /* Algorithm 1 with all nine steps in the delta-g formulation: field, source(dt/2), z(dt/2), v(dt/2),
  * field, 2d(dt), v(dt/2), z(dt/2), source(dt/2).  Needs sldg_set_polar_profiles and sldg_set_equilibrium. */
 int sldg_step_algorithm1_polar(sldg_ctx *ctx, double dt);
+/* Algorithm 2 with all thirteen steps in the delta-g formulation; needs sldg_set_third_buffer too. */
+int sldg_step_algorithm2_polar(sldg_ctx *ctx, double dt);
 const char *sldg_strerror(int code);
 
 #ifdef __cplusplus

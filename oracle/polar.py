@@ -188,3 +188,26 @@ def polar_algorithm1_step(spec, dg, n0, dln_n0, Te, dv_geq, dr_geq, dt):
     dg = oracle.advect_z(spec, dg, 0.5 * dt)
     dg = source_step(dg, fs["dz_phi"], fs["dth_phi"], dv_geq, dr_geq, 0.5 * dt)
     return dg, fs
+
+
+def polar_algorithm2_step(spec, dg, n0, dln_n0, Te, dv_geq, dr_geq, dt):
+    """Algorithm 2, all thirteen steps: 1 field phi^n; predictor from dg^n: 2 source(dt/2), 3 z(dt/2),
+    4 v(dt/2), 5 2d(dt/2) with first-order tracing (eq. 14) -> dg^{n+1/2}; 6 field phi^{n+1/2}; corrector from dg^n:
+    7 source(dt/2), 8 z(dt/2), 9 v(dt/2), 10 2d(dt) with second-order tracing (eq. 15), 11 v(dt/2), 12 z(dt/2),
+    13 source(dt/2)."""
+    import oracle
+
+    fs = polar_field_step(spec, dg, n0, dln_n0, Te)                                              # 1
+    g = source_step(dg, fs["dz_phi"], fs["dth_phi"], dv_geq, dr_geq, 0.5 * dt)                   # 2
+    g = oracle.advect_z(spec, np.ascontiguousarray(g), 0.5 * dt)                                 # 3
+    g = oracle.advect_v(spec, g, fs["Ez"], 0.5 * dt)                                             # 4
+    g = oracle.advect_xy(spec, g, fs["a"], fs["b"], 0.5 * dt, 1, 2)                              # 5
+    fs = polar_field_step(spec, g, n0, dln_n0, Te)                                               # 6
+    dg = source_step(dg, fs["dz_phi"], fs["dth_phi"], dv_geq, dr_geq, 0.5 * dt)                  # 7
+    dg = oracle.advect_z(spec, np.ascontiguousarray(dg), 0.5 * dt)                               # 8
+    dg = oracle.advect_v(spec, dg, fs["Ez"], 0.5 * dt)                                           # 9
+    dg = oracle.advect_xy(spec, dg, fs["a"], fs["b"], dt, 2, 2)                                  # 10
+    dg = oracle.advect_v(spec, dg, fs["Ez"], 0.5 * dt)                                           # 11
+    dg = oracle.advect_z(spec, dg, 0.5 * dt)                                                     # 12
+    dg = source_step(dg, fs["dz_phi"], fs["dth_phi"], dv_geq, dr_geq, 0.5 * dt)                  # 13
+    return dg, fs

@@ -26,7 +26,7 @@ EXPORTS = [
     "sldg_step_algorithm1", "sldg_set_third_buffer", "sldg_step_algorithm2",
     "sldg_set_equilibrium", "sldg_set_source_fields", "sldg_source_step", "sldg_strang_step_sources",
     "sldg_set_polar_profiles", "sldg_polar_field_step", "sldg_get_polar_phi", "sldg_get_source_fields",
-    "sldg_step_algorithm1_polar",
+    "sldg_step_algorithm1_polar", "sldg_step_algorithm2_polar",
 ]
 
 
@@ -105,6 +105,7 @@ def load_library():
     L.sldg_get_polar_phi.argtypes = [vp, dp]
     L.sldg_get_source_fields.argtypes = [vp, dp, dp]
     L.sldg_step_algorithm1_polar.argtypes = [vp, C.c_double]
+    L.sldg_step_algorithm2_polar.argtypes = [vp, C.c_double]
     _lib = L
     return L
 
@@ -297,7 +298,15 @@ class Sldg:
     def step_algorithm1(self, dt, tol=1e-13, max_iter=2000):
         self._chk(self.L.sldg_step_algorithm1(self.h, float(dt), float(tol), int(max_iter)), "sldg_step_algorithm1")
 
+    def step_algorithm2_polar(self, dt):
+        self._third_buffer()
+        self._chk(self.L.sldg_step_algorithm2_polar(self.h, float(dt)), "sldg_step_algorithm2_polar")
+
     def step_algorithm2(self, dt, tol=1e-13, max_iter=2000):
+        self._third_buffer()
+        self._chk(self.L.sldg_step_algorithm2(self.h, float(dt), float(tol), int(max_iter)), "sldg_step_algorithm2")
+
+    def _third_buffer(self):
         if getattr(self, "f_c", None) is None:  # the third copy of f
             g = self.guard_bytes
             if g == 0:
@@ -307,7 +316,6 @@ class Sldg:
                 self._guarded.append(raw)
                 self.f_c = raw[g:g + self.state_bytes].view(self.torch.float64)
             self._chk(self.L.sldg_set_third_buffer(self.h, self.f_c.data_ptr()), "sldg_set_third_buffer")
-        self._chk(self.L.sldg_step_algorithm2(self.h, float(dt), float(tol), int(max_iter)), "sldg_step_algorithm2")
 
     # ---- delta-g formulation: source term (polar coordinates, axis 0 = r, axis 1 = theta) ------------
     def set_equilibrium(self, dv_geq, dr_geq):

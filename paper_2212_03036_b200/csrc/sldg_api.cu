@@ -823,6 +823,36 @@ int sldg_step_algorithm2(sldg_ctx *c, double dt, double tol, int max_iter)
     return SLDG_OK;
 }
 
+int sldg_step_algorithm2_polar(sldg_ctx *c, double dt)
+{
+    if (!c || !c->f_c || !c->pol.ready || !(c->src_ready & 1)) return SLDG_EINVAL;
+    int rc;
+    double *fn = c->f[c->cur];  // delta g of time level n
+    if ((rc = sldg_polar_field_step(c))) return rc;                                                    // 1  phi^n
+    // predictor: the source step writes into another buffer, level n stays untouched
+    aim_away_from(c, fn);
+    if (launch_source_step(c, c->f[c->cur ^ 1], 0.5 * dt, fn) != cudaSuccess) return SLDG_ECUDA;       // 2
+    swap_state(c);
+    if ((rc = pair_keeping(c, 0.5 * dt, true, fn))) return rc;                                         // 3, 4
+    aim_away_from(c, fn);
+    if ((rc = do_xy(c, 0.5 * dt, 1))) return rc;                                                       // 5  eq. (14)
+    if ((rc = sldg_polar_field_step(c))) return rc;                                                    // 6  phi^{n+1/2}
+    // corrector from level n
+    if (c->f[0] == fn) c->cur = 0;
+    else if (c->f[1] == fn) c->cur = 1;
+    else {
+        c->f_c = c->f[c->cur];
+        c->f[c->cur] = fn;
+    }
+    if (launch_source_step(c, c->f[c->cur], 0.5 * dt) != cudaSuccess) return SLDG_ECUDA;               // 7
+    if ((rc = pair_keeping(c, 0.5 * dt, true, nullptr))) return rc;                                    // 8, 9
+    if ((rc = do_xy(c, dt, 2))) return rc;                                                             // 10 eq. (15)
+    if ((rc = pair_keeping(c, 0.5 * dt, false, nullptr))) return rc;                                   // 11, 12
+    if (launch_source_step(c, c->f[c->cur], 0.5 * dt) != cudaSuccess) return SLDG_ECUDA;               // 13
+    c->ev_kind = 0;
+    return SLDG_OK;
+}
+
 int sldg_debug_geometry(sldg_ctx *c, int z, int32_t *anchor_dev, int32_t *mask_dev, double *W_dev)
 {
     if (!c || z < 0 || z >= c->g.N[2]) return SLDG_EINVAL;

@@ -122,7 +122,7 @@ cudaError_t launch_diagnostics(sldg_ctx *c, const double *fin, double r_p, doubl
 size_t source_workspace_bytes(const sldg_params *p);
 void source_carve(sldg_ctx *c, char *base);
 cudaError_t launch_source_profiles(sldg_ctx *c, const double *dv_geq, const double *dr_geq);
-cudaError_t launch_source_step(sldg_ctx *c, double *f, double tau);
+cudaError_t launch_source_step(sldg_ctx *c, double *f, double tau, const double *fin = nullptr);  // fin: out of place
 size_t polar_workspace_bytes(const sldg_params *p);
 void polar_carve(sldg_ctx *c, char *base);
 cudaError_t launch_polar_profiles(sldg_ctx *c, const double *rn0, const double *dln, const double *Te);

@@ -23,7 +23,7 @@ __global__ void __launch_bounds__(256) source_profile_kernel(const double *__res
 // Block <-> rows (z, Y) of Nx lines; warp <-> U lines of the row at a time, lane <-> the v pairs lane + 32 k: no
 // divisions in the inner loops, all loads of the U lines issued before the first store.
 template <int U>
-__global__ void __launch_bounds__(256) source_step_kernel(double *__restrict__ f, const double *__restrict__ dz,
+__global__ void __launch_bounds__(256) source_step_kernel(const double *fin, double *f, const double *__restrict__ dz,
                                                           const double *__restrict__ dth, const double *__restrict__ gv,
                                                           const double *__restrict__ gr, GridDev g, double tau)
 {
@@ -34,6 +34,7 @@ __global__ void __launch_bounds__(256) source_step_kernel(double *__restrict__ f
     for (int row = blockIdx.x; row < rows; row += gridDim.x) {
         const int Z = row / Ny, Y = row - Z * Ny;
         double *frow = f + Z * g.sZ + Y * g.sY;
+        const double *irow = fin + Z * g.sZ + Y * g.sY;  // fin == f: in place
         const double *dzr = dz + (long long)row * Nx, *dtr = dth + (long long)row * Nx;
         for (int X0 = warp * U; X0 < Nx; X0 += 8 * U) {
             for (int v0 = lane; v0 < P2; v0 += 32 * MAXP) {
@@ -43,7 +44,7 @@ __global__ void __launch_bounds__(256) source_step_kernel(double *__restrict__ f
 #pragma unroll
                     for (int p = 0; p < MAXP; ++p) {
                         const int X = X0 + k, v2 = v0 + 32 * p;
-                        if (X < Nx && v2 < P2) u[k][p] = __ldcs(reinterpret_cast<const double2 *>(frow + X * g.sX + 2 * v2));
+                        if (X < Nx && v2 < P2) u[k][p] = __ldcs(reinterpret_cast<const double2 *>(irow + X * g.sX + 2 * v2));
                     }
 #pragma unroll
                 for (int k = 0; k < U; ++k) {
@@ -98,12 +99,13 @@ cudaError_t launch_source_profiles(sldg_ctx *c, const double *dv_geq, const doub
     return cudaGetLastError();
 }
 
-cudaError_t launch_source_step(sldg_ctx *c, double *f, double tau)
+cudaError_t launch_source_step(sldg_ctx *c, double *f, double tau, const double *fin)
 {
+    if (!fin) fin = f;
     const GridDev &g = c->g;
     const long long rows = (long long)g.N[2] * g.N[1];
     const long long cap = (long long)c->sm_count * 8;
-    source_step_kernel<2><<<(unsigned)(rows < cap ? rows : cap), 256, 0, c->stream>>>(f, c->src_dz, c->src_dth, c->src_gv,
+    source_step_kernel<2><<<(unsigned)(rows < cap ? rows : cap), 256, 0, c->stream>>>(fin, f, c->src_dz, c->src_dth, c->src_gv,
                                                                                    c->src_gr, g, tau);
     c->launches++;
     return cudaGetLastError();

@@ -150,3 +150,25 @@ def test_polar_algorithm1_self_consistent_steps(torch, o, cells, eps):
     scale = oracle.mass(spec, np.abs(ref))
     assert abs(float(s.mass().cpu()[0]) - oracle.mass(spec, dg)) <= 1e-13 * scale
     s.close()
+
+
+@pytest.mark.parametrize("fuse", [True, False])
+@pytest.mark.parametrize("o,cells,eps", [(2, (16, 24, 4, 16), 0.05), (3, (8, 12, 2, 8), 0.02)])
+def test_polar_algorithm2_predictor_corrector(torch, monkeypatch, fuse, o, cells, eps):
+    # Algorithm 2 with all thirteen steps: the predictor's source step is out of place, the three buffers rotate
+    if not fuse:
+        monkeypatch.setenv("SLDG_NO_FUSE", "1")
+    spec = inputs.polar_grid(*cells, o)
+    dg = inputs.polar_initial_dg(spec, eps=eps)
+    s, n0, dln_n0, T, dv, dr = _polar_ctx(torch, spec, dg)
+    ref = dg.copy()
+    dt = 4.0
+    for n in range(3):
+        s.step_algorithm2_polar(dt)
+        ref, fs = polar.polar_algorithm2_step(spec, ref, n0, dln_n0, T, dv, dr, dt)
+        got = s.export_state().cpu().numpy()
+        assert np.abs(got - ref).max() <= TOL * np.abs(ref).max(), n
+    s.check()
+    scale = oracle.mass(spec, np.abs(ref))
+    assert abs(float(s.mass().cpu()[0]) - oracle.mass(spec, dg)) <= 1e-13 * scale
+    s.close()

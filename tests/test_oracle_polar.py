@@ -174,3 +174,22 @@ def test_polar_resampling_and_derived_fields():
     assert np.abs(e - (np.sin(kz * hz) / hz * np.sin(rv)[None, None, :] * np.sin(ph))).max() < 1e-12
     h = spec.h[0]
     assert np.abs(b[:, :, 3] - (phi[:, :, 4] - phi[:, :, 2]) / (2 * h) / rv[3]).max() < 1e-15
+
+
+def test_polar_algorithms_differ_by_a_local_second_order_term():
+    # as in the Cartesian case: one step of Algorithm 1 and one of Algorithm 2 from the same state differ
+    # by O(dt^2) -- the field of Algorithm 1's second half is a first-order approximation of phi^{n+1/2}
+    spec = inputs.polar_grid(12, 16, 4, 12, 2)
+    rv = spec.vertex_coords(0)
+    n0, dln_n0, T, _ = inputs.polar_profiles(rv)
+    _, dv, dr = inputs.polar_equilibrium(spec)
+    dg0 = inputs.polar_initial_dg(spec, eps=0.05)
+    m0 = oracle.mass(spec, dg0)
+    d = []
+    for dt in (4.0, 2.0, 1.0):
+        g1, _ = polar.polar_algorithm1_step(spec, dg0.copy(), n0, dln_n0, T, dv, dr, dt)
+        g2, _ = polar.polar_algorithm2_step(spec, dg0.copy(), n0, dln_n0, T, dv, dr, dt)
+        d.append(np.abs(g1 - g2).max())
+        scale = oracle.mass(spec, np.abs(g2))
+        assert abs(oracle.mass(spec, np.ascontiguousarray(g2)) - m0) < 1e-13 * scale
+    assert 1.8 < math.log2(d[0] / d[1]) < 2.2 and 1.8 < math.log2(d[1] / d[2]) < 2.2, d
