@@ -543,12 +543,22 @@ int sldg_strang_step_host(sldg_ctx *c, double dt, const double *Ez_host, const d
     }
     int rc = sldg_strang_step(c, dt);
     if (rc) return rc;
-    if (rho_host || mass_host) {
-        if (launch_charge_density(c, c->f[c->cur], rho_dev) != cudaSuccess) return SLDG_ECUDA;
-    }
     if (rho_host) {
-        if (cudaMemcpyAsync(rho_host, rho_dev, (size_t)g.lines * 8, cudaMemcpyDeviceToHost, c->stream) != cudaSuccess)
-            return SLDG_ECUDA;
+        // rho in slabs of z: the download of a slab (copy stream) runs under the reduction of the next one
+        const int nslab = g.N[2] < 8 ? g.N[2] : 8;
+        const long long per_z = (long long)g.N[1] * g.N[0];
+        for (int k = 0; k < nslab; ++k) {
+            const long long l0 = (long long)g.N[2] * k / nslab * per_z, l1 = (long long)g.N[2] * (k + 1) / nslab * per_z;
+            if (launch_charge_density(c, c->f[c->cur], rho_dev, l0, l1) != cudaSuccess) return SLDG_ECUDA;
+            cudaEventRecord(c->cev[0], c->stream);
+            cudaStreamWaitEvent(c->cstream, c->cev[0], 0);
+            if (cudaMemcpyAsync(rho_host + l0, rho_dev + l0, (size_t)(l1 - l0) * 8, cudaMemcpyDeviceToHost, c->cstream) != cudaSuccess)
+                return SLDG_ECUDA;
+        }
+        cudaEventRecord(c->cev[0], c->cstream);
+        cudaStreamWaitEvent(c->stream, c->cev[0], 0);  // the caller's stream sees the downloads complete
+    } else if (mass_host) {
+        if (launch_charge_density(c, c->f[c->cur], rho_dev) != cudaSuccess) return SLDG_ECUDA;
     }
     if (mass_host) {
         if (launch_mass_from_rho(c, rho_dev, mass_dev) != cudaSuccess) return SLDG_ECUDA;

@@ -104,7 +104,7 @@ cudaError_t launch_pack(sldg_ctx *c, const double *canon, double *internal);
 cudaError_t launch_unpack(sldg_ctx *c, const double *internal, double *canon);
 cudaError_t launch_advect_z(sldg_ctx *c, const double *fin, double *fout, double tau);
 cudaError_t launch_advect_v(sldg_ctx *c, const double *fin, double *fout, double tau);
-cudaError_t launch_charge_density(sldg_ctx *c, const double *fin, double *rho);
+cudaError_t launch_charge_density(sldg_ctx *c, const double *fin, double *rho, long long line0 = 0, long long line1 = -1);  // lines [line0, line1)
 cudaError_t launch_mass(sldg_ctx *c, const double *fin, double *mass_out);
 cudaError_t launch_mass_from_rho(sldg_ctx *c, const double *rho, double *mass_out);
 cudaError_t launch_xy_geometry(sldg_ctx *c, double tau, int trace_order);

@@ -294,12 +294,12 @@ cudaError_t launch_advect_z(sldg_ctx *c, const double *fin, double *fout, double
 // --------------------------------------------------------------------------------------------------
 __global__ void __launch_bounds__(256) charge_density_kernel(const double *__restrict__ fin,
                                                              double *__restrict__ rho, GridDev g,
-                                                             Basis bs)
+                                                             Basis bs, unsigned line0, unsigned line1)
 {
     const int lane = threadIdx.x & 31;
-    const unsigned warp = (blockIdx.x * blockDim.x + threadIdx.x) >> 5;
+    const unsigned warp = line0 + ((blockIdx.x * blockDim.x + threadIdx.x) >> 5);
     const unsigned nwarp = (gridDim.x * blockDim.x) >> 5;
-    const unsigned lines = (unsigned)g.lines;
+    const unsigned lines = line1;  // this launch does the lines [line0, line1)
     const int Nv = g.N[3], ov = g.o[3];
     for (unsigned line = warp; line < lines; line += nwarp) {
         const double *u = fin + line_base_fast(g, line);
@@ -318,14 +318,16 @@ __global__ void __launch_bounds__(256) charge_density_kernel(const double *__res
     }
 }
 
-cudaError_t launch_charge_density(sldg_ctx *c, const double *fin, double *rho)
+cudaError_t launch_charge_density(sldg_ctx *c, const double *fin, double *rho, long long line0, long long line1)
 {
     const GridDev &g = c->g;
     if (g.lines >= (1ll << 31)) return cudaErrorInvalidValue;
-    long long nblk = (g.lines + 7) / 8;
+    if (line1 < 0) line1 = g.lines;
+    long long nblk = (line1 - line0 + 7) / 8;
     long long cap = (long long)c->sm_count * 8 * 16;
     int grid = (int)(nblk < cap ? nblk : cap);
-    charge_density_kernel<<<grid, 256, 0, c->stream>>>(fin, rho, g, c->basis);
+    if (grid < 1) return cudaSuccess;
+    charge_density_kernel<<<grid, 256, 0, c->stream>>>(fin, rho, g, c->basis, (unsigned)line0, (unsigned)line1);
     c->launches++;
     return cudaGetLastError();
 }
