@@ -8,7 +8,8 @@ SURVEY.md 8(a)).  Metric (BASELINE.json / PAPER.md:380): 2*|f|*8 bytes per subst
 Strang step, divided by device time -- ALGORITHMIC (unfused-equivalent) bytes: the fused step physically makes three
 passes over f, so `value` can exceed the copy rate; `hbm_gbs_actual` beside it is bytes really moved / time.
 One JSON line on stdout (rank 0).  The default workload is BASELINE.json configs[4]; its o = 3 half
-(96x96x48x48 cells) is timed in the same run and reported as the sub-record "o3".
+(96x96x48x48 cells) is timed in the same run and reported as the sub-record "o3", the paper's own grid (64x64x64x128 cells,
+o = 2) as the sub-record "paper_grid".
 
 N > 1 (torchrun): the path does not shard (north_star: one GPU, no collectives) -> N independent
 replicas, one per GPU; value = sum over replicas / max-over-ranks time.  "scaling": "weak".
@@ -400,25 +401,20 @@ def measure_itg(workload, K, Wm, layout, world, rank, local, barrier, with_e2e, 
     if log:
         log.close()
     total_ms = ev0.elapsed_time(ev1)
+    hist_timed = s.timing_history(min(K, 64))
     launches = s.launch_count() - launches0
     clk = sampler.stop(t_wall0, t_wall1) if (rank == 0 and clocks) else None
     s.check()
     total_ms = max_over_ranks(total_ms, world)
     mass1 = float(s.mass().cpu()[0])
 
-    # breakdown of the Strang step: a few extra steps, device events inside the library (same stream)
-    per = []
-    for _ in range(max(3, min(K, 10))):
-        s.strang_step(dt)
-        per.append(s.last_timing_ms())
-    med = np.median(np.array(per), axis=0)
-    fused_zv, fused_vz = bool(int(med[6]) & 2), bool(int(med[6]) & 4)
-    blocks = s.debug_counter(1)  # non-empty (target, source) weight blocks of the last 2d step
-    # the substeps one by one (the calls of the boundary): z(dt/2), v(dt/2), xy(dt), each 2*|f|*8 bytes
+    # the substeps one by one (the calls of the boundary): z(dt/2), v(dt/2), xy(dt), each 2*|f|*8 bytes -- right after the
+    # timed steps, in the same power / clock regime (under the 1 kW cap the SM clock sinks over seconds of sustained load:
+    # the ALU-bound 2d geometry measured 0.75 ms fresh and 0.91 ms ten seconds later in the same process)
     single = {"z": [], "v": [], "xy": [], "xy_geometry": []}
-    nrep = max(5, min(K, 10))
+    nrep = 5
     for name, call in (("z", lambda: s.advect_z(0.5 * dt)), ("v", lambda: s.advect_v(0.5 * dt)), ("xy", lambda: s.advect_xy(dt, 2))):
-        for _ in range(3):
+        for _ in range(2):
             call()  # warm-up of this kernel sequence; then nrep consecutive calls, each timed by the library's own events
         for _ in range(nrep):
             call()
@@ -427,6 +423,12 @@ def measure_itg(workload, K, Wm, layout, world, rank, local, barrier, with_e2e, 
             if name == "xy":
                 single["xy_geometry"].append(t[2])
     s.check()
+    # breakdown of the Strang step: the per-kernel CUDA-event times of the K TIMED steps themselves, from the library's
+    # event history (recorded on the library's stream during the timed region, read here: no synchronisation in the loop)
+    per = hist_timed
+    med = np.median(np.array(per), axis=0)
+    fused_zv, fused_vz = bool(int(med[6]) & 2), bool(int(med[6]) & 4)
+    blocks = s.debug_counter(1)  # non-empty (target, source) weight blocks of the last 2d step
     sm = {k: float(np.median(v)) for k, v in single.items()}
     sm_min = {k: float(np.min(v)) for k, v in single.items()}
     rho = s.charge_density()
@@ -595,6 +597,10 @@ def run_ours(args):
     if args.workload == "c4" and not args.no_o3:
         # the other half of BASELINE.json configs[4]: "also run at o=3 on 96x96x48x48 cells", same K and W
         o3 = measure_itg("c4o3", K, Wm, args.layout, world, rank, local, barrier, False, None, clocks=False)
+    paper = None
+    if args.workload == "c4" and not args.no_paper:
+        # the paper's own grid (64x64x64x128 cells, 256 KB planes: the z-tiled pair kernel), like for like with its A100 numbers
+        paper = measure_itg("paper", K, Wm, args.layout, world, rank, local, barrier, False, None, clocks=False)
     if rank == 0:
         cpu = cpu_oracle_baseline() if (world == 1 and not args.no_cpu_baseline) else None
         line = {
@@ -607,6 +613,9 @@ def run_ours(args):
         if o3 is not None:
             o3["metric"], o3["unit"], o3["steps"], o3["warmup"] = line["metric"], "GB/s", K, Wm
             line["o3"] = o3
+        if paper is not None:
+            paper["metric"], paper["unit"], paper["steps"], paper["warmup"] = line["metric"], "GB/s", K, Wm
+            line["paper_grid"] = paper
         line["paper_context"] = "A100: z 956, v 760, xy 209 GB/s per substep, ~590 GB/s whole step (PAPER.md:408-429)"
         print(json.dumps(line), flush=True)
     if world > 1:
@@ -627,6 +636,7 @@ def main():
     ap.add_argument("--layout", type=int, default=0)
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--no-o3", action="store_true", help="skip the o=3 half of configs[4] (sub-record \"o3\")")
+    ap.add_argument("--no-paper", action="store_true", help="skip the paper's own grid (sub-record \"paper_grid\")")
     ap.add_argument("--probe", default=None, choices=["fp64"], help="only measure and print the fp64 FMA roof")
     args = ap.parse_args()
     args.warmup = max(args.warmup, 3) if args.impl == "ours" else args.warmup

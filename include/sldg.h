@@ -134,6 +134,9 @@ int sldg_check(sldg_ctx *ctx);
  * ms[4] holds the time of the pair and ms[5] = 0.
  * After a single sldg_advect_* call only that entry (and ms[7]) is set.  Synchronises. */
 int sldg_last_timing_ms(sldg_ctx *ctx, float ms[8]);
+/* The same eight numbers for each of the last n sldg_strang_step calls (n <= 64, oldest first; ms: n x 8 floats): the
+ * library keeps the events of the last 64 steps, so a timed loop needs no synchronisation inside it.  Synchronises. */
+int sldg_timing_history(sldg_ctx *ctx, int n, float *ms);
 /* Number of kernels the library launched on behalf of this context since creation. */
 long long sldg_launch_count(sldg_ctx *ctx);
 /* Debug / test access to the geometry of the last sldg_advect_xy: for z node `z` copies, per target

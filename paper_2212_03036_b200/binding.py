@@ -26,7 +26,7 @@ EXPORTS = [
     "sldg_step_algorithm1", "sldg_set_third_buffer", "sldg_step_algorithm2",
     "sldg_set_equilibrium", "sldg_set_source_fields", "sldg_source_step", "sldg_strang_step_sources",
     "sldg_set_polar_profiles", "sldg_polar_field_step", "sldg_get_polar_phi", "sldg_get_source_fields",
-    "sldg_step_algorithm1_polar", "sldg_step_algorithm2_polar",
+    "sldg_step_algorithm1_polar", "sldg_step_algorithm2_polar", "sldg_timing_history",
 ]
 
 
@@ -81,6 +81,7 @@ def load_library():
     L.sldg_check.argtypes = [vp]
     L.sldg_last_timing_ms.argtypes = [vp, C.POINTER(C.c_float * 8)]
     L.sldg_launch_count.argtypes = [vp]
+    L.sldg_timing_history.argtypes = [vp, C.c_int, C.POINTER(C.c_float)]
     L.sldg_launch_count.restype = C.c_longlong
     L.sldg_debug_geometry.argtypes = [vp, C.c_int, ip, ip, dp]
     L.sldg_debug_counter.argtypes = [vp, C.c_int, C.POINTER(C.c_longlong)]
@@ -367,6 +368,12 @@ class Sldg:
         ms = (C.c_float * 8)()
         self._chk(self.L.sldg_last_timing_ms(self.h, C.byref(ms)), "sldg_last_timing_ms")
         return list(ms)
+
+    def timing_history(self, n):
+        """Per-kernel device times of the last n Strang steps, n x 8 (see sldg_last_timing_ms), oldest first."""
+        buf = (C.c_float * (8 * n))()
+        self._chk(self.L.sldg_timing_history(self.h, int(n), buf), "sldg_timing_history")
+        return [list(buf[8 * i:8 * i + 8]) for i in range(n)]
 
     def launch_count(self):
         return int(self.L.sldg_launch_count(self.h))

@@ -217,6 +217,16 @@ void fill_shift_poly(int o, ShiftPoly *sp)
 
 int cuda_fail(cudaError_t e) { return e == cudaSuccess ? SLDG_OK : SLDG_ECUDA; }
 
+// the events a call records are those of one slot of the history ring (ev[0..5]: the substeps, ev[6..7] = gev: the
+// geometry kernel); a Strang step moves on to the next slot when it is done, so that the per-kernel times of the last
+// SLDG_HIST steps can be read after a timed loop without a synchronisation inside it (sldg_timing_history)
+void use_history_slot(sldg_ctx *c, int h)
+{
+    for (int k = 0; k < 8; ++k) c->ev[k] = c->hev[h][k];
+    c->gev[0] = c->hev[h][6];
+    c->gev[1] = c->hev[h][7];
+}
+
 void swap_state(sldg_ctx *c) { c->cur ^= 1; }
 
 }  // namespace
@@ -283,13 +293,15 @@ int sldg_create(const sldg_params *p, double *f_a_dev, double *f_b_dev, void *wo
         delete c;
         return SLDG_ECUDA;
     }
-    for (int k = 0; k < 8; ++k)
-        if (cudaEventCreate(&c->ev[k]) != cudaSuccess) {
-            sldg_destroy(c);
-            return SLDG_ECUDA;
-        }
+    for (int h = 0; h < SLDG_HIST; ++h)
+        for (int k = 0; k < 8; ++k)
+            if (cudaEventCreate(&c->hev[h][k]) != cudaSuccess) {
+                sldg_destroy(c);
+                return SLDG_ECUDA;
+            }
+    use_history_slot(c, 0);
     for (int k = 0; k < 2; ++k)
-        if (cudaEventCreate(&c->gev[k]) != cudaSuccess || cudaEventCreate(&c->cev[k]) != cudaSuccess) {
+        if (cudaEventCreate(&c->cev[k]) != cudaSuccess) {
             sldg_destroy(c);
             return SLDG_ECUDA;
         }
@@ -311,14 +323,14 @@ int sldg_create(const sldg_params *p, double *f_a_dev, double *f_b_dev, void *wo
 int sldg_destroy(sldg_ctx *c)
 {
     if (!c) return SLDG_EINVAL;
-    for (int k = 0; k < 8; ++k)
-        if (c->ev[k]) cudaEventDestroy(c->ev[k]);
+    for (int h = 0; h < SLDG_HIST; ++h)
+        for (int k = 0; k < 8; ++k)
+            if (c->hev[h][k]) cudaEventDestroy(c->hev[h][k]);
     if (c->cstream) {
         cudaStreamSynchronize(c->cstream);
         cudaStreamDestroy(c->cstream);
     }
     for (int k = 0; k < 2; ++k) {
-        if (c->gev[k]) cudaEventDestroy(c->gev[k]);
         if (c->cev[k]) cudaEventDestroy(c->cev[k]);
     }
     delete c;
@@ -507,6 +519,7 @@ int sldg_strang_step(sldg_ctx *c, double dt)
     if (!c) return SLDG_EINVAL;
     int rc;
     int fused0 = 0, fused1 = 0;
+    use_history_slot(c, c->hpos);
     cudaEventRecord(c->ev[0], c->stream);
     if ((rc = do_pair(c, 0.5 * dt, true, c->ev[1], &fused0))) return rc;
     cudaEventRecord(c->ev[2], c->stream);
@@ -516,6 +529,11 @@ int sldg_strang_step(sldg_ctx *c, double dt)
     cudaEventRecord(c->ev[5], c->stream);
     c->last_fused = (fused0 ? 2 : 0) + (fused1 ? 4 : 0);
     c->ev_kind = 1;
+    c->hist_fused[c->hpos] = c->last_fused;
+    c->hpos = (c->hpos + 1) % SLDG_HIST;
+    c->hcount++;
+    c->last_slot = (c->hpos + SLDG_HIST - 1) % SLDG_HIST;
+    use_history_slot(c, c->hpos);  // single substep calls that follow record into the next slot, not over this step's
     return SLDG_OK;
 }
 
@@ -584,17 +602,13 @@ int sldg_last_timing_ms(sldg_ctx *c, float ms[8])
     for (int k = 0; k < 8; ++k) ms[k] = 0.0f;
     if (c->ev_kind == 0) return SLDG_OK;
     if (cudaStreamSynchronize(c->stream) != cudaSuccess) return SLDG_ECUDA;
+    cudaEvent_t *E = c->ev_kind == 1 ? c->hev[c->last_slot] : c->ev;  // a Strang step's events sit in its history slot
     auto el = [&](int a, int b) {
         float t = 0.0f;
-        cudaEventElapsedTime(&t, c->ev[a], c->ev[b]);
+        cudaEventElapsedTime(&t, E[a], E[b]);
         return t;
     };
-    auto geom = [&]() {
-        float t = 0.0f;
-        cudaEventSynchronize(c->gev[1]);
-        cudaEventElapsedTime(&t, c->gev[0], c->gev[1]);
-        return t;
-    };
+    auto geom = [&]() { return el(6, 7); };
     if (c->ev_kind == 1) {
         ms[0] = el(0, 1); ms[1] = el(1, 2); ms[3] = el(2, 3); ms[4] = el(3, 4); ms[5] = el(4, 5);
         ms[2] = geom();
@@ -609,6 +623,25 @@ int sldg_last_timing_ms(sldg_ctx *c, float ms[8])
         ms[3] = ms[7] = el(0, 1);
     } else if (c->ev_kind == 5) {
         ms[7] = el(0, 1);
+    }
+    return SLDG_OK;
+}
+
+int sldg_timing_history(sldg_ctx *c, int n, float *ms)
+{
+    if (!c || !ms || n < 1 || n > SLDG_HIST || n > c->hcount) return SLDG_EINVAL;
+    if (cudaStreamSynchronize(c->stream) != cudaSuccess) return SLDG_ECUDA;
+    for (int i = 0; i < n; ++i) {
+        const int h = (c->hpos + SLDG_HIST - n + i) % SLDG_HIST;  // oldest first
+        cudaEvent_t *e = c->hev[h];
+        float *o = ms + 8 * i, t = 0.0f;
+        auto el = [&](int a, int b) {
+            cudaEventElapsedTime(&t, e[a], e[b]);
+            return t;
+        };
+        o[0] = el(0, 1); o[1] = el(1, 2); o[2] = el(6, 7); o[3] = el(2, 3); o[4] = el(3, 4); o[5] = el(4, 5);
+        o[6] = (float)c->hist_fused[h];
+        o[7] = el(0, 5);
     }
     return SLDG_OK;
 }

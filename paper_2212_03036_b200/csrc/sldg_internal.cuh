@@ -9,6 +9,7 @@
 #define SLDG_MAXO 3
 #define SLDG_MAXO2 9
 #define SLDG_MAXQ 5       // quadrature points per edge for the Green's-theorem line integrals (2o-1)
+#define SLDG_HIST 64      // Strang steps whose per-kernel event times are kept (sldg_timing_history)
 #define SLDG_PV_ALIGN 16  // internal v-line pitch is a multiple of 16 doubles (128 B)
 
 // Doubles between two weight blocks of the 2d geometry in memory: o^4, at o = 3 padded to an even number (bulk
@@ -87,7 +88,12 @@ struct sldg_ctx {
     int fuse, last_fused;   // fuse: sldg_strang_step runs each pair of adjacent sweeps in one pass
     size_t n_partials;
     int trace_order, vel_periodic;
-    cudaEvent_t ev[8];
+    cudaEvent_t ev[8];      // events of the call in progress: handles of the history slot in use (owned by hev)
+    cudaEvent_t hev[SLDG_HIST][8];  // per Strang step: ev[0..5] and the two geometry events; ring of the last SLDG_HIST steps
+    int hist_fused[SLDG_HIST];
+    int hpos;               // slot the next Strang step records into
+    long long hcount;       // Strang steps recorded since creation
+    int last_slot;
     int ev_kind;            // 0 none, 1 strang, 2 z, 3 v, 4 xy
     long long launches;
     int sm_count;

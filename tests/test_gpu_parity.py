@@ -577,3 +577,26 @@ def test_z_tiled_sweep_pairs_are_bit_identical_to_separate_sweeps(torch, monkeyp
         outs.append(s.export_state().cpu().numpy())
         s.close()
     assert np.array_equal(outs[0], outs[1])
+
+
+def test_timing_history_matches_last_timing(torch):
+    """sldg_timing_history returns, for each of the last n Strang steps, what sldg_last_timing_ms returned right after
+    that step; single substep calls in between do not disturb the recorded steps."""
+    spec = inputs.itg_grid(12, 10, 6, 16, 2)
+    f = inputs.itg_initial_f(spec)
+    a, b, Ez, _ = inputs.itg_fields(spec, 2.0, 0.8)
+    s = _sldg(spec)
+    s.import_state(_dev(torch, f))
+    s.set_Ez(_dev(torch, Ez))
+    s.set_vxy(_dev(torch, a), _dev(torch, b), 1)
+    want = []
+    for n in range(5):
+        s.strang_step(2.0)
+        want.append(s.last_timing_ms())
+        if n == 2:
+            s.advect_z(0.1)
+            s.advect_xy(0.1, 2)
+    got = s.timing_history(5)
+    assert np.allclose(np.array(got), np.array(want), rtol=0, atol=0)
+    assert all(g[7] > 0 and abs(g[7] - (g[0] + g[1] + g[3] + g[4] + g[5])) < 0.05 for g in got)
+    s.close()
