@@ -15,6 +15,7 @@
 //       z to the Gauss-Legendre z nodes, bilinear interpolation in (x,y) to the nodes for E_z; written
 //       where sldg_set_vxy / sldg_set_Ez would put them.
 #include <math.h>
+#include <stdlib.h>
 
 #include "sldg_internal.cuh"
 
@@ -139,7 +140,7 @@ __global__ void __launch_bounds__(T) field_cg_kernel(double *__restrict__ x_all,
                                                      double *__restrict__ q_all, const double *__restrict__ n0,
                                                      const double *__restrict__ Te, int nx, int ny, double ihx2,
                                                      double ihy2, double shift, double tol, int max_iter, int zero_mean,
-                                                     int *__restrict__ iters, double *__restrict__ relres)
+                                                     int warm, int *__restrict__ iters, double *__restrict__ relres)
 {
     __shared__ double red[2 * T / 32];
     const int N = nx * ny;
@@ -161,32 +162,49 @@ __global__ void __launch_bounds__(T) field_cg_kernel(double *__restrict__ x_all,
         return (nE + nW) * ihx2 + (nN + nS) * ihy2 + shift * n0[k] / Te[k];
     };
 
-    double rz = 0.0, bb = 0.0;
+    // stencil of the symmetrised operator n0 (A + shift / Te) at vertex k
+    auto apply = [&](const double *u, int k) {
+        const int i = k % nx, j = k / nx;
+        double nE, nW, nN, nS;
+        faces(k, nE, nW, nN, nS);
+        const double uc = u[k];
+        return -(nE * (u[j * nx + wrapf(i + 1, nx)] - uc) - nW * (uc - u[j * nx + wrapf(i - 1, nx)])) * ihx2 -
+               (nN * (u[wrapf(j + 1, ny) * nx + i] - uc) - nS * (uc - u[wrapf(j - 1, ny) * nx + i])) * ihy2 +
+               shift * n0[k] / Te[k] * uc;
+    };
+    // start: x0 = 0, or (warm) the solution of the previous field step left in x -- in a time-stepping run the potential
+    // changes little from one solve to the next and most of the iterations go away
+    double rz = 0.0, bb = 0.0, r0 = 0.0;
     for (int k = threadIdx.x; k < N; k += T) {
-        const double rk = n0[k] * b[k];
+        const double bk = n0[k] * b[k];
+        double rk = bk;
+        if (warm) rk -= apply(x, k);
+        else x[k] = 0.0;
         const double zk = rk / diag(k);
-        x[k] = 0.0;
         r[k] = rk;
         p[k] = zk;
         rz = fma(rk, zk, rz);
-        bb = fma(rk, rk, bb);
+        bb = fma(bk, bk, bb);
+        r0 = fma(rk, rk, r0);
+    }
+    {
+        double dummy = 0.0;
+        block_sum2<T>(r0, dummy, red);
     }
     block_sum2<T>(rz, bb, red);
-    double rr = bb;
+    double rr = r0;
     int it = 0;
+    if (!(bb > 0.0)) {
+        for (int k = threadIdx.x; k < N; k += T) x[k] = 0.0;  // zero source: zero potential, whatever the initial guess
+        rr = 0.0;
+    }
     if (bb > 0.0) {
         for (; it < max_iter && rr > tol * tol * bb; ++it) {
             double pq = 0.0, dummy = 0.0;
             for (int k = threadIdx.x; k < N; k += T) {
-                const int i = k % nx, j = k / nx;
-                double nE, nW, nN, nS;
-                faces(k, nE, nW, nN, nS);
-                const double pc = p[k];
-                const double qk = -(nE * (p[j * nx + wrapf(i + 1, nx)] - pc) - nW * (pc - p[j * nx + wrapf(i - 1, nx)])) * ihx2 -
-                                  (nN * (p[wrapf(j + 1, ny) * nx + i] - pc) - nS * (pc - p[wrapf(j - 1, ny) * nx + i])) * ihy2 +
-                                  shift * n0[k] / Te[k] * pc;
+                const double qk = apply(p, k);
                 q[k] = qk;
-                pq = fma(pc, qk, pq);
+                pq = fma(p[k], qk, pq);
             }
             block_sum2<T>(pq, dummy, red);
             const double alpha = rz / pq;
@@ -440,6 +458,7 @@ cudaError_t launch_field_step(sldg_ctx *c, const double *fin, double tol, int ma
     const long long total = (long long)Nz * ncell;
     constexpr int T = 1024;
     cudaStream_t st = c->stream;
+    const int warm = f.have_phi && !getenv("SLDG_FIELD_COLD") ? 1 : 0;  // previous potential as the initial guess
     cudaError_t e = launch_charge_density(c, fin, c->rho_ws);
     if (e != cudaSuccess) return e;
     field_resample_kernel<<<field_grid_blocks(c, total), 256, 0, st>>>(c->rho_ws, f.n0, f.rhs, g, c->basis);
@@ -448,10 +467,10 @@ cudaError_t launch_field_step(sldg_ctx *c, const double *fin, double tol, int ma
     field_defect_kernel<T><<<1, T, 0, st>>>(f.n0, f.bar[1], ncell, f.scal);
     const double ihx2 = 1.0 / (g.h[0] * g.h[0]), ihy2 = 1.0 / (g.h[1] * g.h[1]);
     field_cg_kernel<T><<<1, T, 0, st>>>(f.bar[0], f.bar[1], f.bar[2], f.bar[3], f.bar[4], f.n0, f.Te, nx, ny, ihx2, ihy2, 0.0,
-                                        tol, max_iter, 1, f.iters + Nz, f.relres + Nz);
+                                        tol, max_iter, 1, warm, f.iters + Nz, f.relres + Nz);
     field_rhs_shift_kernel<<<field_grid_blocks(c, total), 256, 0, st>>>(f.rhs, f.bar[0], f.Te, f.scal, ncell, total);
     field_cg_kernel<T><<<Nz, T, 0, st>>>(f.phi, f.rhs, f.r, f.p, f.q, f.n0, f.Te, nx, ny, ihx2, ihy2, 1.0, tol, max_iter, 0,
-                                         f.iters, f.relres);
+                                         warm, f.iters, f.relres);
     field_drift_kernel<<<field_grid_blocks(c, (long long)Nz * (ny + 1) * (nx + 1)), 256, 0, st>>>(f.phi, c->va, c->vb, g,
                                                                                                  c->basis, f.invB);
     field_nodes_kernel<<<field_grid_blocks(c, g.lines), 256, 0, st>>>(f.phi, c->Ez, f.phin, g, c->basis);
