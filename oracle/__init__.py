@@ -6,7 +6,9 @@ import this package.  It imports nothing from paper_2212_03036_b200 except, in c
 input generators (paper_2212_03036_b200.inputs holds no arithmetic of the method).
 
 Parity pins: every function is pinned in tests/test_oracle_1d.py and tests/test_oracle_2d.py (list in
-DESIGN.md, "Oracle pins").
+DESIGN.md, "Oracle pins").  The rows beyond the hot path have their own modules, same rules: oracle/field.py (Cartesian
+field step, invariants, Algorithms 1 and 2; pins in tests/test_oracle_field.py) and oracle/polar.py (source term, the
+paper's polar quasi-neutrality solver, the delta-g algorithms; pins in tests/test_oracle_polar.py).
 """
 from __future__ import annotations
 
