@@ -143,3 +143,44 @@ def test_c4_strang_step_fused_equals_separate_calls_and_conserves_mass(torch, ca
     same = bool(torch.equal(_view(s)[..., :Nv], _view(t)[..., :Nv]))
     t.close()
     assert same
+
+
+def test_c4_source_step_and_field_step_at_bench_size(torch, case):
+    """The rows beyond the hot path in the launch configurations bench.py times: the source term on sampled lines (exact
+    formula) and the field step against the oracle's direct solve (the whole potential: 129 sparse systems
+    of 128^2 unknowns take the oracle a few seconds).  Runs last: it changes the state and the fields of the fixture."""
+    from oracle import field
+    spec, f0, a, b, Ez, s = case
+    Nz, Nv, Ny, Nx = spec.shape
+    rng = np.random.default_rng(17)
+    # ---- source term ------------------------------------------------------------------------------------------------
+    s.import_state_host(f0)
+    vv = spec.node_coords(3)
+    gv = np.ascontiguousarray(np.repeat((-vv * np.exp(-0.5 * vv * vv))[:, None], Nx, axis=1) * (1.0 + 0.1 * np.arange(Nx))[None, :])
+    gr = np.ascontiguousarray(np.repeat(np.exp(-0.5 * vv * vv)[:, None], Nx, axis=1) * np.cos(0.05 * np.arange(Nx))[None, :])
+    dz = np.ascontiguousarray(Ez * 1.7)
+    dth = np.ascontiguousarray(np.roll(Ez, 3, axis=1) * 0.4)
+    s.set_equilibrium(torch.from_numpy(gv).cuda(), torch.from_numpy(gr).cuda())
+    s.set_source_fields(torch.from_numpy(dz).cuda(), torch.from_numpy(dth).cuda())
+    s.source_step(0.37)
+    view = _view(s)
+    for _ in range(48):
+        z, y, x = int(rng.integers(Nz)), int(rng.integers(Ny)), int(rng.integers(Nx))
+        got = view[z, y, x, :Nv].cpu().numpy()
+        want = f0[z, :, y, x] + 0.37 * (dz[z, y, x] * gv[:, x] + dth[z, y, x] * gr[:, x])
+        assert np.abs(got - want).max() <= 1e-15 * np.abs(want).max() + 1e-300
+    # ---- field step -------------------------------------------------------------------------------------------------
+    s.import_state_host(f0)
+    n0, Te = inputs.itg_vertex_profiles(spec)
+    s.set_profiles(torch.from_numpy(n0).cuda(), torch.from_numpy(Te).cuda(), 1.0)
+    s.field_step(1e-14, 20000)
+    iters, relres = s.field_info()
+    assert relres <= 1e-13, (iters, relres)
+    want = field.field_step(spec, oracle.charge_density(spec, f0), n0, Te, 1.0)
+    phi = s.get_phi().cpu().numpy()
+    scale = np.abs(want["phi"]).max()
+    assert np.abs(phi - want["phi"]).max() <= 1e-8 * scale
+    Ezg, ag, bg = (t.cpu().numpy() for t in s.get_fields())
+    assert np.abs(ag - want["a"]).max() <= 1e-8 * scale / spec.h[1]
+    assert np.abs(bg - want["b"]).max() <= 1e-8 * scale / spec.h[0]
+    assert np.abs(Ezg - want["Ez"]).max() <= 1e-8 * scale / (spec.h[2] / spec.order[2])
