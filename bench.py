@@ -116,6 +116,12 @@ class ClockSampler:
         for line in self.proc.stdout:
             self.rows.append((time.time(), line.strip()))
 
+    def wait_first(self, timeout=3.0):
+        """nvidia-smi needs a few tenths of a second to print its first line: the timed region (0.1 s) starts after it."""
+        t_end = time.time() + timeout
+        while self.proc is not None and not self.rows and time.time() < t_end:
+            time.sleep(0.01)
+
     def stop(self, t0, t1):
         if self.proc is None:
             return {"sm_mhz": None, "sm_max_mhz": None, "reasons": ["nvidia-smi unavailable"]}
@@ -123,7 +129,10 @@ class ClockSampler:
         self.proc.terminate()
         sm, smax, reasons = [], None, set()
         names = ["hw_slowdown", "hw_thermal_slowdown", "sw_thermal_slowdown", "sw_power_cap"]
-        rows = [r for (t, r) in self.rows if t0 - 0.05 <= t <= t1 + 0.15] or [r for (_, r) in self.rows]
+        # samples inside the timed region; nvidia-smi samples every 100 ms, so a 0.1 s region may hold one or none: then
+        # the samples right around it (0.3 s) stand in
+        rows = ([r for (t, r) in self.rows if t0 - 0.05 <= t <= t1 + 0.15] or
+                [r for (t, r) in self.rows if t0 - 0.3 <= t <= t1 + 0.3] or [r for (_, r) in self.rows])
         for r in rows:
             p = [x.strip() for x in r.split(",")]
             try:
@@ -375,12 +384,14 @@ def measure_itg(workload, K, Wm, layout, world, rank, local, barrier, with_e2e, 
     mass0 = float(s.mass().cpu()[0])
 
     # ---------------- device-resident leg -----------------------------------------------------------
-    for _ in range(Wm):
-        s.strang_step(dt)
-    s.check()
     sampler = ClockSampler(local)
     if rank == 0 and clocks:
         sampler.start()
+    for _ in range(Wm):
+        s.strang_step(dt)
+    s.check()
+    if rank == 0 and clocks:
+        sampler.wait_first()
     launches0 = s.launch_count()
     ev0, ev1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
     barrier()
