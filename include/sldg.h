@@ -55,8 +55,9 @@ enum {
     SLDG_EINVAL = -1,   /* bad parameter, null pointer, misaligned or too small buffer               */
     SLDG_ECUDA = -2,    /* CUDA runtime / launch error, or no device                                  */
     SLDG_ESTENCIL = -3, /* an upstream cell's bounding box exceeds max_stencil   */
-    SLDG_EGEOM = -4     /* upstream cell not convex / not positively oriented (crossed characteristics,
+    SLDG_EGEOM = -4,    /* upstream cell not convex / not positively oriented (crossed characteristics,
                            PAPER.md:190) or a singular Vandermonde system              */
+    SLDG_ELIMIT = -5    /* the problem exceeds the fixed scratch of sldg_mass_static                  */
 };
 
 /* Sizes (bytes) of each ping-pong state buffer and of the workspace for these parameters; 0 on
@@ -225,6 +226,25 @@ int sldg_step_algorithm1_polar(sldg_ctx *ctx, double dt);
 /* Algorithm 2 with all thirteen steps in the delta-g formulation; needs sldg_set_third_buffer too. */
 int sldg_step_algorithm2_polar(sldg_ctx *ctx, double dt);
 const char *sldg_strerror(int code);
+
+/* ---- allocation-free entry point (sldg_static.cu) -------------------------------------------------------------
+ * Total mass (the v integral is the charge density of PAPER.md:57) of a distribution given in the
+ * canonical layout [Nz][Nv][Ny][Nx], WITHOUT a context, a workspace or any allocation: for callers that may not call
+ * cudaMalloc (CUDA graph capture, serving loops).  The intermediate charge density and partial sums live in a file-scope
+ * static __device__ array of SLDG_STATIC_MAX_NODES + 1024 doubles (8 MiB + 8 KiB per GPU that loads the library).
+ *   p               only n, order, lo, hi are read (order[d] in 1..3)
+ *   f_canonical_dev DEVICE, borrowed, read only, 8-byte aligned
+ *   mass_dev        DEVICE, one double, written
+ *   cuda_stream     a cudaStream_t of the CURRENT device (NULL = legacy default stream); asynchronous
+ * Returns SLDG_ELIMIT when Nx*Ny*Nz > SLDG_STATIC_MAX_NODES (nothing is launched), SLDG_EINVAL on bad arguments,
+ * SLDG_ECUDA on a launch error or without a device.  Every call on a device shares the one array: calls ordered on a
+ * stream are safe, calls that overlap on the GPU race.  Nothing in the array needs clearing between calls.
+ * sldg_mass_static_setup looks up the array's device address for the current device (cudaGetSymbolAddress, once per
+ * device; the first sldg_mass_static does it otherwise -- call it beforehand when the first call is under capture). */
+#define SLDG_STATIC_MAX_NODES (1 << 20)
+long long sldg_mass_static_max_nodes(void);
+int sldg_mass_static_setup(void);
+int sldg_mass_static(const sldg_params *p, const double *f_canonical_dev, double *mass_dev, void *cuda_stream);
 
 #ifdef __cplusplus
 }

@@ -14,6 +14,7 @@ _HERE = os.path.dirname(os.path.abspath(__file__))
 _lib = None
 
 SLDG_OK, SLDG_EINVAL, SLDG_ECUDA, SLDG_ESTENCIL, SLDG_EGEOM = 0, -1, -2, -3, -4
+SLDG_ELIMIT = -5
 
 EXPORTS = [
     "sldg_state_bytes", "sldg_workspace_bytes", "sldg_create", "sldg_destroy", "sldg_import_state",
@@ -27,6 +28,7 @@ EXPORTS = [
     "sldg_set_equilibrium", "sldg_set_source_fields", "sldg_source_step", "sldg_strang_step_sources",
     "sldg_set_polar_profiles", "sldg_polar_field_step", "sldg_get_polar_phi", "sldg_get_source_fields",
     "sldg_step_algorithm1_polar", "sldg_step_algorithm2_polar", "sldg_timing_history",
+    "sldg_mass_static", "sldg_mass_static_setup", "sldg_mass_static_max_nodes",
 ]
 
 
@@ -107,6 +109,10 @@ def load_library():
     L.sldg_get_source_fields.argtypes = [vp, dp, dp]
     L.sldg_step_algorithm1_polar.argtypes = [vp, C.c_double]
     L.sldg_step_algorithm2_polar.argtypes = [vp, C.c_double]
+    L.sldg_mass_static.argtypes = [PP, dp, dp, vp]
+    L.sldg_mass_static_setup.argtypes = []
+    L.sldg_mass_static_max_nodes.argtypes = []
+    L.sldg_mass_static_max_nodes.restype = C.c_longlong
     _lib = L
     return L
 
@@ -121,6 +127,31 @@ def make_params(spec, layout=0, max_stencil=3):
     p.max_stencil = max_stencil
     p.layout = layout
     return p
+
+
+def mass_static(spec, f_canonical, out, stream=None):
+    """sldg_mass_static: total mass of a canonical-layout distribution into the one-element CUDA tensor `out`, with no
+    context, no workspace and no allocation (the scratch is a static device array inside libsldg.so).  Calls on one
+    stream are ordered; calls that overlap on the GPU race on the shared scratch."""
+    import torch
+
+    if not torch.cuda.is_available():
+        raise RuntimeError("libsldg needs a CUDA device (sm_100a); there is no CPU fallback")
+    L = load_library()
+    assert f_canonical.is_cuda and f_canonical.dtype == torch.float64 and f_canonical.is_contiguous()
+    assert tuple(f_canonical.shape) == tuple(spec.shape)
+    assert out.is_cuda and out.dtype == torch.float64 and out.numel() == 1 and out.device == f_canonical.device
+    p = make_params(spec)
+    with torch.cuda.device(f_canonical.device):
+        st = stream if stream is not None else torch.cuda.current_stream()
+        rc = L.sldg_mass_static(C.byref(p), f_canonical.data_ptr(), out.data_ptr(), st.cuda_stream)
+    if rc == SLDG_ELIMIT:
+        N = [int(spec.n[d]) * int(spec.order[d]) for d in range(3)]
+        raise ValueError(f"sldg_mass_static: Nx*Ny*Nz = {N[0] * N[1] * N[2]} nodes exceed the static scratch of "
+                         f"{L.sldg_mass_static_max_nodes()} nodes; use Sldg.mass() (caller-allocated workspace)")
+    if rc != 0:
+        raise SldgError(rc, "sldg_mass_static")
+    return out
 
 
 class Sldg:
