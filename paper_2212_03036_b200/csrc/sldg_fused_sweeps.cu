@@ -35,7 +35,9 @@ constexpr int FUSED_MAXCPL = 4;  // v cells per lane in the line-wise phases (nv
 // [Pv] ints, z shift [Pv] ints | barriers | z,v pair: line order per plane parity [2][Nz] shorts, marks [2][Nz] bytes
 __host__ __device__ inline size_t fused_table_bytes(int Nz, int Pv, int O)
 {
-    return (size_t)Nz * 2 * O * O * 8 + (size_t)Pv * 2 * O * O * 8 + (size_t)Nz * 4 + (size_t)Pv * 8 + 64 +
+    // o <= 2: A, B of the column's z shift stay in the registers of the column's threads (every KB of tables is a line
+    // less fetched ahead: 0.02 ms per KB and z,v pair at 128 x 128)
+    return (size_t)Nz * 2 * O * O * 8 + (O <= 2 ? 0 : (size_t)Pv * 2 * O * O * 8) + (size_t)Nz * 4 + (size_t)Pv * 8 + 64 +
            (size_t)Nz * 6 + 16;  // + line order of the z,v pair's line-wise phase [2][Nz] shorts, marks [2][Nz] bytes
 }
 
@@ -54,7 +56,8 @@ __global__ void __launch_bounds__(FUSED_BLOCK, 1) fused_sweep_kernel(const doubl
     double *buf = reinterpret_cast<double *>(fused_smem);  // [L_a | H | L_b]
     double *vAB = buf + (size_t)(2 * NL + NH) * Pv;        // [Nz][2][O][O]: A then B of the line's v shift
     double *zAB = vAB + (size_t)Nz * 2 * O * O;            // [2 O O][Pv]: A then B of the column's z shift
-    int *vs = reinterpret_cast<int *>(zAB + (size_t)Pv * 2 * O * O);  // [Nz]: the line's integer v shift, wrapped
+    constexpr bool ZREG = O <= 2;                          // zAB in registers instead (fused_table_bytes)
+    int *vs = reinterpret_cast<int *>(zAB + (ZREG ? 0 : (size_t)Pv * 2 * O * O));  // [Nz]: the line's integer v shift, wrapped
     int *rotoff = vs + Nz;                                 // [Pv]: s_z(v) * O * Pv, the column's rotation in doubles
     int *zs = rotoff + Pv;                                 // [Pv]: s_z(v), wrapped
     const int NzPv = Nz * Pv;
@@ -66,10 +69,12 @@ __global__ void __launch_bounds__(FUSED_BLOCK, 1) fused_sweep_kernel(const doubl
     const int nq = min(FUSED_THREADS / Pv, nz);  // slices of z
     const int v = tid % Pv, qd = tid / Pv;
     const bool zact = qd < nq && v < Nv;
-    if (tid < Pv) {
-        // (s, A, B) of the z shift depend on the v node only: once per block, into shared memory
+    double Azr[ZREG ? O : 1][ZREG ? O : 1], Bzr[ZREG ? O : 1][ZREG ? O : 1];  // ZREG: A, B of this thread's column
+    if (tid < Pv || ZREG) {
+        // (s, A, B) of the z shift depend on the v node only: once per block, into shared memory (o = 3) or into the
+        // registers of every thread of the column
         const int ov = g.o[3];
-        const int vv = tid < Nv ? tid : 0;
+        const int vv = v < Nv ? v : 0;
         const int l = vv / ov, q = vv - l * ov;
         const double vq = __dadd_rn(g.lo[3], __dmul_rn(__dadd_rn((double)l, bs.xi[ov][q]), g.h[3]));
         int s0;
@@ -77,14 +82,21 @@ __global__ void __launch_bounds__(FUSED_BLOCK, 1) fused_sweep_kernel(const doubl
         shift_of(vq, tau_z, g.h[2], s0, alpha);
         eval_shift<O>(spz, alpha, A0, B0);
         s0 = wrapi(s0, nz);
-        zs[tid] = s0;
-        rotoff[tid] = tid < Nv ? s0 * O * Pv : 0;
+        if (tid < Pv) {
+            zs[tid] = s0;
+            rotoff[tid] = tid < Nv ? s0 * O * Pv : 0;
+        }
 #pragma unroll
         for (int j = 0; j < O; ++j)
 #pragma unroll
             for (int m = 0; m < O; ++m) {
-                zAB[(j * O + m) * Pv + tid] = A0[j][m];
-                zAB[(O * O + j * O + m) * Pv + tid] = B0[j][m];
+                if (ZREG) {
+                    Azr[ZREG ? j : 0][ZREG ? m : 0] = A0[j][m];
+                    Bzr[ZREG ? j : 0][ZREG ? m : 0] = B0[j][m];
+                } else if (tid < Pv) {
+                    zAB[(j * O + m) * Pv + tid] = A0[j][m];
+                    zAB[(O * O + j * O + m) * Pv + tid] = B0[j][m];
+                }
             }
     }
     const int zi0 = (int)((long long)qd * nz / nq), zi1 = (int)((long long)(qd + 1) * nz / nq);
@@ -234,8 +246,8 @@ __global__ void __launch_bounds__(FUSED_BLOCK, 1) fused_sweep_kernel(const doubl
                 for (int j = 0; j < O; ++j)
 #pragma unroll
                     for (int m = 0; m < O; ++m) {
-                        Az[j][m] = zAB[(j * O + m) * Pv + v];
-                        Bz[j][m] = zAB[(O * O + j * O + m) * Pv + v];
+                        Az[j][m] = ZREG ? Azr[ZREG ? j : 0][ZREG ? m : 0] : zAB[(j * O + m) * Pv + v];
+                        Bz[j][m] = ZREG ? Bzr[ZREG ? j : 0][ZREG ? m : 0] : zAB[(O * O + j * O + m) * Pv + v];
                     }
                 c = zi0 + sz;
                 if (c >= nz) c -= nz;
@@ -440,8 +452,8 @@ __global__ void __launch_bounds__(FUSED_BLOCK, 1) fused_sweep_kernel(const doubl
                 for (int j = 0; j < O; ++j)
 #pragma unroll
                     for (int m = 0; m < O; ++m) {
-                        Az[j][m] = zAB[(j * O + m) * Pv + v];
-                        Bz[j][m] = zAB[(O * O + j * O + m) * Pv + v];
+                        Az[j][m] = ZREG ? Azr[ZREG ? j : 0][ZREG ? m : 0] : zAB[(j * O + m) * Pv + v];
+                        Bz[j][m] = ZREG ? Bzr[ZREG ? j : 0][ZREG ? m : 0] : zAB[(O * O + j * O + m) * Pv + v];
                     }
                 int c = zi0 + zs[v];
                 if (c >= nz) c -= nz;
@@ -496,7 +508,8 @@ cudaError_t launch_fused_sweeps(sldg_ctx *c, const double *fin, double *fout, do
     // the per-line tables of the v shift (vs, vAB, the E_z prefetch) are filled by thread <-> line
     if (!z_only && Nz > FUSED_THREADS) return cudaErrorNotSupported;
     const size_t tables = fused_table_bytes(Nz, g.Pv, O), row = (size_t)g.Pv * 8;
-    const size_t budget = 227 * 1024 - 1024;
+    static const int budget_kb = getenv("SLDG_FUSED_KB") ? atoi(getenv("SLDG_FUSED_KB")) : 227;  // KB of dynamic shared memory the kernel may take (sm_100: 227 per block)
+    const size_t budget = (size_t)budget_kb * 1024;
     if (tables + row * Nz > budget) return cudaErrorNotSupported;
     long long NLl = (long long)((budget - tables) / row) - Nz;  // spare lines = lines fetched one plane ahead
     const int NL = (int)(NLl > Nz ? Nz : (NLl < 0 ? 0 : NLl));

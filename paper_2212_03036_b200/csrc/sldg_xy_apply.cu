@@ -458,9 +458,19 @@ __global__ void __launch_bounds__(256, 2) xy_apply_direct_kernel(const double *_
         for (int m = 0; m < O2; ++m)
 #pragma unroll
             for (int e = 0; e < NV; ++e) acc[m][e] = 0.0;
+        // the non-empty source cells in ascending slot order (with CPW > 1 the cells of a warp have different masks: the
+        // warp runs as many rounds as its fullest cell has blocks, not one per slot that any of them uses)
+        int rem = msk;
 #pragma unroll 1
-        for (int slot = 0; slot < 9; ++slot) {
-            if (!((msk >> slot) & 1)) continue;
+        for (int it = 0; it < 9; ++it) {
+            int slot = it;
+            if (CPW == 1) {
+                if (!((msk >> slot) & 1)) continue;
+            } else {
+                if (!rem) break;
+                slot = __ffs(rem) - 1;
+                rem &= rem - 1;
+            }
             const int r = wrap_idx(ax + slot % 3, nx), s = wrap_idx(ay + slot / 3, ny);  // nx, ny may be < 3
             const double *Wp = W + ((size_t)cellid * 9 + nb++) * sldg_w_block_doubles(O);
 #pragma unroll
@@ -472,11 +482,30 @@ __global__ void __launch_bounds__(256, 2) xy_apply_direct_kernel(const double *_
 #pragma unroll
                     for (int e = 0; e < NV; ++e) in[e] = e < nve ? __ldg(src + LPC * e) : 0.0;
                     const int k = kp + O * kq;
+                    if (O == 1 || (O == 3 && CPW == 1)) {
+                        // one cell per warp at o = 3: one weight at a time (NV >= 4 has no registers for more)
 #pragma unroll
-                    for (int m = 0; m < O2; ++m) {
-                        const double w = __ldg(Wp + k * O2 + m);
+                        for (int m = 0; m < O2; ++m) {
+                            const double w = __ldg(Wp + k * O2 + m);
 #pragma unroll
-                        for (int e = 0; e < NV; ++e) acc[m][e] = fma(w, in[e], acc[m][e]);
+                            for (int e = 0; e < NV; ++e) acc[m][e] = fma(w, in[e], acc[m][e]);
+                        }
+                    } else {
+                        // the o^2 weights W[k][.] as 16-byte loads: blocks start 16-byte aligned (o = 3: 82 doubles per
+                        // block, so the pair after the last weight exists); with CPW cells per warp a weight load touches
+                        // CPW cache lines, and the L1 wavefronts of the weights bound the short-chunk kernel
+                        constexpr int NPAIR = (O2 + 2) / 2;       // pairs that cover o^2 weights from either parity
+                        const int b = (k * O2) & ~1, odd = (k * O2) & 1;
+                        double2 t[NPAIR];
+#pragma unroll
+                        for (int q = 0; q < NPAIR; ++q)
+                            if (2 * q < O2 + odd) t[q] = __ldg(reinterpret_cast<const double2 *>(Wp + b) + q);
+#pragma unroll
+                        for (int m = 0; m < O2; ++m) {
+                            const double w = ((m + odd) & 1) ? t[(m + odd) >> 1].y : t[(m + odd) >> 1].x;
+#pragma unroll
+                            for (int e = 0; e < NV; ++e) acc[m][e] = fma(w, in[e], acc[m][e]);
+                        }
                     }
                 }
         }
