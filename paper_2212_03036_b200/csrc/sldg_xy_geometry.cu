@@ -31,8 +31,11 @@ using namespace sldg_geom;
 
 namespace {
 
+#ifndef SLDG_GEOM_MINB2
+#define SLDG_GEOM_MINB2 5  // resident blocks per SM the o = 2 kernel is compiled for (102 registers)
+#endif
 template <int O>
-__global__ void __launch_bounds__(GeomShared<O>::CELLS) xy_geometry_kernel(const double *__restrict__ va,
+__global__ void __launch_bounds__(GeomShared<O>::CELLS, (O == 2 ? SLDG_GEOM_MINB2 : 1)) xy_geometry_kernel(const double *__restrict__ va,
                                                                            const double *__restrict__ vb,
                                                                            int4 *__restrict__ hdr, double *__restrict__ W,
                                                                            int32_t *err,

@@ -18,41 +18,15 @@ __device__ __forceinline__ int wrap_idx(int i, int n)
 __device__ __forceinline__ double dmin(double a, double b) { return a < b ? a : b; }
 __device__ __forceinline__ double dmax(double a, double b) { return a > b ? a : b; }
 
-// piecewise-bilinear velocity of cell (ci,cj) at local (xi,eta)
-__device__ __forceinline__ void bilinear_vel(const double *__restrict__ a, const double *__restrict__ b,
-                                             int pitch, int ci, int cj, double xi, double eta,
+// piecewise-bilinear velocity at local (xi,eta) of a cell, from the cell's four vertex values (lower-left,
+// lower-right, upper-left, upper-right)
+__device__ __forceinline__ void bilinear_val(const double (&va)[4], const double (&vb)[4], double xi, double eta,
                                              double &ua, double &ub)
 {
-    const double *a0 = a + (long long)cj * pitch + ci;
-    const double *b0 = b + (long long)cj * pitch + ci;
     const double w00 = (1.0 - xi) * (1.0 - eta), w10 = xi * (1.0 - eta), w01 = (1.0 - xi) * eta,
                  w11 = xi * eta;
-    ua = w00 * __ldg(a0) + w10 * __ldg(a0 + 1) + w01 * __ldg(a0 + pitch) + w11 * __ldg(a0 + pitch + 1);
-    ub = w00 * __ldg(b0) + w10 * __ldg(b0 + 1) + w01 * __ldg(b0 + pitch) + w11 * __ldg(b0 + pitch + 1);
-}
-
-// foot of the characteristic through local (xi,eta) of cell (i,j), relative to that cell, cell units
-__device__ __forceinline__ void trace_point(const double *__restrict__ a, const double *__restrict__ b,
-                                            int nx, int ny, double tx, double ty, int i, int j,
-                                            double xi, double eta, int order, int periodic, double &fx,
-                                            double &fy)
-{
-    double ua, ub;
-    bilinear_vel(a, b, nx + 1, i, j, xi, eta, ua, ub);
-    if (order != 1) {
-        double mx = xi - 0.5 * tx * ua, my = eta - 0.5 * ty * ub;
-        int fi = (int)floor(mx), fj = (int)floor(my);
-        // per axis: modulo the box (bitwise-periodic field) or clamped; periodic 1: both axes, 0: none, 2: y only
-        // (polar plane: x = r bounded with zero radial velocity at both ends, y = theta)
-        const bool px = periodic == 1, py = periodic == 1 || periodic == 2;
-        const int ci = px ? wrap_idx(i + fi, nx) : min(max(i + fi, 0), nx - 1);
-        const int cj = py ? wrap_idx(j + fj, ny) : min(max(j + fj, 0), ny - 1);
-        if (!px) fi = ci - i;
-        if (!py) fj = cj - j;
-        bilinear_vel(a, b, nx + 1, ci, cj, mx - fi, my - fj, ua, ub);
-    }
-    fx = xi - tx * ua;
-    fy = eta - ty * ub;
+    ua = w00 * va[0] + w10 * va[1] + w01 * va[2] + w11 * va[3];
+    ub = w00 * vb[0] + w10 * vb[1] + w01 * vb[2] + w11 * vb[3];
 }
 
 // Gauss-Jordan with partial pivoting on [V | X], fully unrolled so that everything stays in registers (o <= 2).
@@ -298,24 +272,66 @@ __device__ __forceinline__ int geometry_setup(const double *__restrict__ va, con
     const double *a = va + z * vplane, *b = vb + z * vplane;
     const double tx = tau / g.h[0], ty = tau / g.h[1];
 
-    // steps 1 and 4, tracing: the four corners (counter-clockwise from lower-left) and the O2 Gauss-Legendre nodes.
-    // One rolled loop over the 4 + O2 points -- unrolled, eight copies of the two bilinear look-ups were a quarter of the
-    // kernel's code --, feet parked in this cell's column of sh.Vi (x at [pt], y at [4 + O2 + pt]).
+    // steps 1 and 4, tracing: the four corners (counter-clockwise from lower-left) and the O2 Gauss-Legendre nodes, feet
+    // parked in this cell's column of sh.Vi (x at [pt], y at [4 + O2 + pt]).  Every point starts in the target cell, so
+    // the first velocity look-up of eq. (15) uses the same four vertex values for all of them: loaded once.  The points
+    // are traced in groups of TG, the second look-ups of a group (one cell each, wherever the half-step points fell)
+    // requested together: a thread waits for global memory 1 + NPT / TG times instead of 2 NPT times (these waits were
+    // 14 % of the kernel's stall samples).  The group loop stays rolled (code size).
     constexpr int NPT = 4 + O2;
+    constexpr int TG = O == 3 ? 2 : 2;
+    const int pitch = nx + 1;
+    double av[4], bv[4];
+    {
+        const double *a0 = a + (long long)j * pitch + i, *b0 = b + (long long)j * pitch + i;
+        av[0] = __ldg(a0); av[1] = __ldg(a0 + 1); av[2] = __ldg(a0 + pitch); av[3] = __ldg(a0 + pitch + 1);
+        bv[0] = __ldg(b0); bv[1] = __ldg(b0 + 1); bv[2] = __ldg(b0 + pitch); bv[3] = __ldg(b0 + pitch + 1);
+    }
+    // foot of the characteristic through local (xi,eta) of cell (i,j), relative to that cell, cell units: eq. (14), or
+    // eq. (15) as an explicit midpoint step whose half-step point is looked up, per axis, modulo the box (bitwise-periodic
+    // field) or clamped; periodic 1: both axes, 0: none, 2: y only (polar plane: x = r bounded with zero radial velocity
+    // at both ends, y = theta)
+    const bool perx = periodic == 1, pery = periodic == 1 || periodic == 2;
 #pragma unroll 1
-    for (int pt = 0; pt < NPT; ++pt) {
-        double xi, eta;
-        if (pt < 4) {
-            xi = (pt == 1 || pt == 2) ? 1.0 : 0.0;
-            eta = pt >= 2 ? 1.0 : 0.0;
-        } else {
-            xi = bs.xi[O][(pt - 4) % O];
-            eta = bs.xi[O][(pt - 4) / O];
+    for (int p0 = 0; p0 < NPT; p0 += TG) {
+        double xi[TG], eta[TG], ua[TG], ub[TG];
+#pragma unroll
+        for (int q = 0; q < TG; ++q) {
+            const int pt = p0 + q < NPT ? p0 + q : NPT - 1;  // a last group may repeat the last point
+            if (pt < 4) {
+                xi[q] = (pt == 1 || pt == 2) ? 1.0 : 0.0;
+                eta[q] = pt >= 2 ? 1.0 : 0.0;
+            } else {
+                xi[q] = bs.xi[O][(pt - 4) % O];
+                eta[q] = bs.xi[O][(pt - 4) / O];
+            }
+            bilinear_val(av, bv, xi[q], eta[q], ua[q], ub[q]);
         }
-        double px, py;
-        trace_point(a, b, nx, ny, tx, ty, i, j, xi, eta, order, periodic, px, py);
-        sh.Vi[pt][c] = px;
-        sh.Vi[NPT + pt][c] = py;
+        if (order != 1) {
+            double lx[TG], ly[TG], wa[TG][4], wb[TG][4];
+#pragma unroll
+            for (int q = 0; q < TG; ++q) {
+                const double mx = xi[q] - 0.5 * tx * ua[q], my = eta[q] - 0.5 * ty * ub[q];
+                int fi = (int)floor(mx), fj = (int)floor(my);
+                const int ci = perx ? wrap_idx(i + fi, nx) : min(max(i + fi, 0), nx - 1);
+                const int cj = pery ? wrap_idx(j + fj, ny) : min(max(j + fj, 0), ny - 1);
+                if (!perx) fi = ci - i;
+                if (!pery) fj = cj - j;
+                lx[q] = mx - fi;
+                ly[q] = my - fj;
+                const double *a0 = a + (long long)cj * pitch + ci, *b0 = b + (long long)cj * pitch + ci;
+                wa[q][0] = __ldg(a0); wa[q][1] = __ldg(a0 + 1); wa[q][2] = __ldg(a0 + pitch); wa[q][3] = __ldg(a0 + pitch + 1);
+                wb[q][0] = __ldg(b0); wb[q][1] = __ldg(b0 + 1); wb[q][2] = __ldg(b0 + pitch); wb[q][3] = __ldg(b0 + pitch + 1);
+            }
+#pragma unroll
+            for (int q = 0; q < TG; ++q) bilinear_val(wa[q], wb[q], lx[q], ly[q], ua[q], ub[q]);
+        }
+#pragma unroll
+        for (int q = 0; q < TG; ++q) {
+            const int pt = p0 + q < NPT ? p0 + q : NPT - 1;
+            sh.Vi[pt][c] = xi[q] - tx * ua[q];
+            sh.Vi[NPT + pt][c] = eta[q] - ty * ub[q];
+        }
     }
     // step 1: upstream quadrilateral
     double cx[4], cy[4];
