@@ -309,6 +309,11 @@ int sldg_create(const sldg_params *p, double *f_a_dev, double *f_b_dev, void *wo
         sldg_destroy(c);
         return SLDG_ECUDA;
     }
+    for (int k = 0; k < SLDG_EZ_CHUNKS; ++k)
+        if (cudaEventCreateWithFlags(&c->ezev[k], cudaEventDisableTiming) != cudaSuccess) {
+            sldg_destroy(c);
+            return SLDG_ECUDA;
+        }
     // fields default to zero, error word cleared
     cudaError_t e = cudaMemsetAsync(ws + m.Ez, 0, m.hdr - m.Ez, c->stream);
     if (e == cudaSuccess) e = cudaMemsetAsync(c->err, 0, 256, c->stream);
@@ -333,6 +338,8 @@ int sldg_destroy(sldg_ctx *c)
     for (int k = 0; k < 2; ++k) {
         if (c->cev[k]) cudaEventDestroy(c->cev[k]);
     }
+    for (int k = 0; k < SLDG_EZ_CHUNKS; ++k)
+        if (c->ezev[k]) cudaEventDestroy(c->ezev[k]);
     delete c;
     return SLDG_OK;
 }
@@ -421,6 +428,19 @@ static cudaError_t launch_pair(sldg_ctx *c, double tau, bool z_first)
     const double *fin = c->f[c->cur];
     double *fout = c->f[c->cur ^ 1];
     cudaError_t e = cudaErrorNotSupported;
+    if (c->ez_chunks > 0 && z_first) {
+        // sldg_strang_step_host: E_z is arriving on the copy stream in chunks of y rows; the planes of a chunk are
+        // swept as soon as its rows are there (the caller checked that the whole-plane kernel takes this pair)
+        const int nch = c->ez_chunks, Ny = c->g.N[1], Nx = c->g.N[0];
+        c->ez_chunks = 0;
+        for (int k = 0; k < nch; ++k) {
+            const int y0 = (int)((long long)Ny * k / nch), y1 = (int)((long long)Ny * (k + 1) / nch);
+            cudaStreamWaitEvent(c->stream, c->ezev[k], 0);
+            e = launch_fused_sweeps(c, fin, fout, tau, tau, true, false, y0 * Nx, y1 * Nx);
+            if (e != cudaSuccess) return e;
+        }
+        return e;
+    }
     if (c->tile == 2) e = launch_tiled_sweeps(c, fin, fout, tau, tau, z_first);
     if (e == cudaErrorNotSupported) {
         cudaGetLastError();
@@ -545,15 +565,33 @@ int sldg_strang_step_host(sldg_ctx *c, double dt, const double *Ez_host, const d
     const GridDev &g = c->g;
     double *rho_dev = c->rho_ws;
     double *mass_dev = c->scalar_ws;
-    if (Ez_host &&
+    // E_z is first needed by the v sweep of the z,v pair.  Where that pair runs as the whole-plane kernel (one pass over the
+    // (z,v) planes in the order of (y,x)), E_z goes up on the copy stream in chunks of y rows -- strided copies, E_z is
+    // [Nz][Ny][Nx] -- and the planes of a chunk are swept as soon as its rows have arrived (launch_pair): only the first
+    // chunk's upload is exposed.  Otherwise one copy on the caller's stream ahead of the step.
+    const bool ez_chunked = Ez_host && c->fuse && c->tile != 2 && g.N[1] >= SLDG_EZ_CHUNKS && fused_sweeps_supported(c, true);
+    if (Ez_host && !ez_chunked &&
         cudaMemcpyAsync(c->Ez, Ez_host, (size_t)g.lines * 8, cudaMemcpyHostToDevice, c->stream) != cudaSuccess)
         return SLDG_ECUDA;
+    if (ez_chunked || a_host) {
+        cudaEventRecord(c->cev[0], c->stream);
+        cudaStreamWaitEvent(c->cstream, c->cev[0], 0);
+    }
+    if (ez_chunked) {
+        const size_t pitch = (size_t)g.N[1] * g.N[0] * 8;
+        for (int k = 0; k < SLDG_EZ_CHUNKS; ++k) {
+            const long long y0 = (long long)g.N[1] * k / SLDG_EZ_CHUNKS, y1 = (long long)g.N[1] * (k + 1) / SLDG_EZ_CHUNKS;
+            if (cudaMemcpy2DAsync(c->Ez + y0 * g.N[0], pitch, Ez_host + y0 * g.N[0], pitch, (size_t)(y1 - y0) * g.N[0] * 8,
+                                  (size_t)g.N[2], cudaMemcpyHostToDevice, c->cstream) != cudaSuccess)
+                return SLDG_ECUDA;
+            cudaEventRecord(c->ezev[k], c->cstream);
+        }
+        c->ez_chunks = SLDG_EZ_CHUNKS;
+    }
     if (a_host) {
         size_t bytes = (size_t)g.N[2] * (g.n[0] + 1) * (g.n[1] + 1) * 8;
         c->vel_periodic = periodic == 2 ? 2 : (periodic ? 1 : 0);
         // a, b are first needed by the 2d step: their upload runs on the copy stream under the z and v sweeps
-        cudaEventRecord(c->cev[0], c->stream);
-        cudaStreamWaitEvent(c->cstream, c->cev[0], 0);
         if (cudaMemcpyAsync(c->va, a_host, bytes, cudaMemcpyHostToDevice, c->cstream) != cudaSuccess) return SLDG_ECUDA;
         if (cudaMemcpyAsync(c->vb, b_host, bytes, cudaMemcpyHostToDevice, c->cstream) != cudaSuccess) return SLDG_ECUDA;
         cudaEventRecord(c->cev[1], c->cstream);

@@ -48,7 +48,8 @@ __global__ void __launch_bounds__(FUSED_BLOCK, 1) fused_sweep_kernel(const doubl
                                                                        double *__restrict__ fout,
                                                                        const double *__restrict__ Ez, GridDev g,
                                                                        ShiftPoly spz, ShiftPoly spv, Basis bs,
-                                                                       double tau_z, double tau_v, int NL)
+                                                                       double tau_z, double tau_v, int NL, int col0,
+                                                                       int col1)
 {
     extern __shared__ __align__(16) unsigned char fused_smem[];
     const int Nz = g.N[2], nz = g.n[2], Nv = g.N[3], nv = g.n[3], Pv = g.Pv;
@@ -62,7 +63,7 @@ __global__ void __launch_bounds__(FUSED_BLOCK, 1) fused_sweep_kernel(const doubl
     int *zs = rotoff + Pv;                                 // [Pv]: s_z(v), wrapped
     const int NzPv = Nz * Pv;
     const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
-    const int ncol = g.N[1] * g.N[0];
+    const int ncol = col1;  // this launch does the planes (Y,X) with index Y * Nx + X in [col0, col1)
     const long long plane_nodes = (long long)g.N[1] * g.N[0];
 
     // z sweep: thread <-> (v, slice qd of the target z cells); (s, A, B) depend on the v node only
@@ -155,7 +156,7 @@ __global__ void __launch_bounds__(FUSED_BLOCK, 1) fused_sweep_kernel(const doubl
     if (warp == FUSED_THREADS / 32) {
         // ---------------- producer warp ------------------------------------------------------------------------
         uint32_t phD = 0, phF = 0;
-        int col = blockIdx.x, par = 0;
+        int col = col0 + blockIdx.x, par = 0;
         if (col < ncol) issue_lines(col, buf, 0, NL, &bars[0]);  // L lines of the first (even) plane
         if (ZFIRST && col < ncol) issue_lines(col, buf, NL, NH, &bars[2]);  // z,v: and its H lines
         for (bool first = true; col < ncol; col += gridDim.x, par ^= 1, first = false) {
@@ -201,7 +202,7 @@ __global__ void __launch_bounds__(FUSED_BLOCK, 1) fused_sweep_kernel(const doubl
             off1[k][m] = ZFIRST ? (uint32_t)(rotoff[c1 * O + md] + c1 * O + md) * 8u : 0u;
         }
     double ez_next = 0.0;
-    int col = blockIdx.x, par = 0;
+    int col = col0 + blockIdx.x, par = 0;
     uint32_t phL[2] = {0, 0}, phH = 0;
     if (!ZONLY && col < ncol && tid < Nz) ez_next = __ldg(Ez + tid * plane_nodes + col);
     for (; col < ncol; col += gridDim.x, par ^= 1) {
@@ -494,33 +495,56 @@ __global__ void __launch_bounds__(FUSED_BLOCK, 1) fused_sweep_kernel(const doubl
 
 }  // namespace
 
-// The pair (z then v, or v then z) in one pass; returns cudaErrorNotSupported when the (z,v) plane does not fit
-// (the caller then runs the two separate kernels).
-cudaError_t launch_fused_sweeps(sldg_ctx *c, const double *fin, double *fout, double tau_z, double tau_v, bool z_first,
-                                bool z_only)
+// Whether the pair can run in this kernel (see launch_fused_sweeps); *NL_out = lines fetched one plane ahead.
+static bool fused_pair_fits(const sldg_ctx *c, bool z_first, bool z_only, int *NL_out, size_t *smem_out)
 {
     if (z_only) z_first = false;
     const GridDev &g = c->g;
     const int O = g.o[2];
-    if (!z_only && g.o[3] != O) return cudaErrorNotSupported;
-    if (g.Pv > FUSED_THREADS || (!z_only && g.n[3] > 32 * FUSED_MAXCPL)) return cudaErrorNotSupported;
+    if (!z_only && g.o[3] != O) return false;
+    if (g.Pv > FUSED_THREADS || (!z_only && g.n[3] > 32 * FUSED_MAXCPL)) return false;
     const int Nz = g.N[2];
     // the per-line tables of the v shift (vs, vAB, the E_z prefetch) are filled by thread <-> line
-    if (!z_only && Nz > FUSED_THREADS) return cudaErrorNotSupported;
+    if (!z_only && Nz > FUSED_THREADS) return false;
     const size_t tables = fused_table_bytes(Nz, g.Pv, O), row = (size_t)g.Pv * 8;
     static const int budget_kb = getenv("SLDG_FUSED_KB") ? atoi(getenv("SLDG_FUSED_KB")) : 227;  // KB of dynamic shared memory the kernel may take (sm_100: 227 per block)
     const size_t budget = (size_t)budget_kb * 1024;
-    if (tables + row * Nz > budget) return cudaErrorNotSupported;
+    if (tables + row * Nz > budget) return false;
     long long NLl = (long long)((budget - tables) / row) - Nz;  // spare lines = lines fetched one plane ahead
     const int NL = (int)(NLl > Nz ? Nz : (NLl < 0 ? 0 : NLl));
     // z first: the z sweep cannot start before the whole plane is there, so the lines that do not fit beside the
     // current plane (NH = Nz - NL, fetched only when it is done) are fully exposed; measured at 144 x 144 (o = 3,
     // NL = 0.28 Nz) the pair is then slower than the two separate kernels.  v first hides them under its L lines.
-    if ((z_first || z_only) && 2 * NL < Nz) return cudaErrorNotSupported;
-    const size_t smem = tables + row * (size_t)(2 * NL + (Nz - NL));
+    if ((z_first || z_only) && 2 * NL < Nz) return false;
+    *NL_out = NL;
+    *smem_out = tables + row * (size_t)(2 * NL + (Nz - NL));
+    return true;
+}
+
+bool fused_sweeps_supported(const sldg_ctx *c, bool z_first)
+{
+    int NL;
+    size_t smem;
+    return fused_pair_fits(c, z_first, false, &NL, &smem);
+}
+
+// The pair (z then v, or v then z) in one pass over the planes (Y,X) with index Y * Nx + X in [col0, col1) (col1 < 0:
+// all from col0 on); returns cudaErrorNotSupported when the (z,v) plane does not fit (the caller then runs the two
+// separate kernels).
+cudaError_t launch_fused_sweeps(sldg_ctx *c, const double *fin, double *fout, double tau_z, double tau_v, bool z_first,
+                                bool z_only, int col0, int col1)
+{
+    if (z_only) z_first = false;
+    const GridDev &g = c->g;
+    const int O = g.o[2];
+    int NL;
+    size_t smem;
+    if (!fused_pair_fits(c, z_first, z_only, &NL, &smem)) return cudaErrorNotSupported;
     const bool cpl2 = g.n[3] <= 64;
     const bool fullv = g.n[3] == (cpl2 ? 64 : 128);  // every lane of the line-wise phase has all its cells
-    const int ncol = g.N[0] * g.N[1];
+    if (col1 < 0) col1 = g.N[0] * g.N[1];
+    const int ncol = col1 - col0;
+    if (ncol <= 0) return cudaSuccess;
     const int grid = ncol < c->sm_count ? ncol : c->sm_count;
 #define LAUNCH_F(OO)                                                                                              \
     do {                                                                                                          \
@@ -533,7 +557,7 @@ cudaError_t launch_fused_sweeps(sldg_ctx *c, const double *fin, double *fout, do
                                     : fused_sweep_kernel<OO, 4, false, false, false>);                            \
         cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);                       \
         kern<<<grid, FUSED_BLOCK, smem, c->stream>>>(fin, fout, c->Ez, g, c->sp_z, c->sp_v, c->basis, tau_z,    \
-                                                       tau_v, NL);                                                \
+                                                       tau_v, NL, col0, col1);                                    \
     } while (0)
     if (O == 1) LAUNCH_F(1); else if (O == 2) LAUNCH_F(2); else LAUNCH_F(3);
 #undef LAUNCH_F

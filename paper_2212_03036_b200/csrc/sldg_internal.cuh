@@ -10,6 +10,7 @@
 #define SLDG_MAXO2 9
 #define SLDG_MAXQ 5       // quadrature points per edge for the Green's-theorem line integrals (2o-1)
 #define SLDG_HIST 64      // Strang steps whose per-kernel event times are kept (sldg_timing_history)
+#define SLDG_EZ_CHUNKS 4   // y chunks of the E_z upload of sldg_strang_step_host
 #define SLDG_PV_ALIGN 16  // internal v-line pitch is a multiple of 16 doubles (128 B)
 
 // Doubles between two weight blocks of the 2d geometry in memory: o^4, at o = 3 padded to an even number (bulk
@@ -84,6 +85,10 @@ struct sldg_ctx {
     cudaStream_t cstream;   // copy stream: sldg_strang_step_host uploads a, b under the first sweeps
     cudaEvent_t cev[2];     // fork / join of that upload
     int ab_pending;         // an upload of a, b is in flight on cstream: the next 2d step waits for it
+    // sldg_strang_step_host: E_z uploaded on cstream in ez_chunks chunks of y rows, chunk k complete at ezev[k]; the fused
+    // z,v pair that follows is launched per chunk behind its event (0: no such upload in flight)
+    int ez_chunks;
+    cudaEvent_t ezev[SLDG_EZ_CHUNKS];
     int tile;               // z-tiled pair kernel: 1 when the whole plane does not fit, 2 first (SLDG_FORCE_TILE), 0 never (SLDG_NO_TILE)
     int fuse, last_fused;   // fuse: sldg_strang_step runs each pair of adjacent sweeps in one pass
     size_t n_partials;
@@ -118,8 +123,10 @@ size_t xy_apply_stage_flags(const sldg_params *p);  // number of stage_ok entrie
 cudaError_t launch_geometry_expand(sldg_ctx *c, int z, int32_t *anchor, int32_t *mask, double *Wd);
 cudaError_t launch_xy_apply(sldg_ctx *c, const double *fin, double *fout);
 cudaError_t count_weight_blocks(sldg_ctx *c, long long *total_host);
+// planes (Y,X) with index Y * Nx + X in [col0, col1); col1 < 0: all from col0 on
 cudaError_t launch_fused_sweeps(sldg_ctx *c, const double *fin, double *fout, double tau_z, double tau_v, bool z_first,
-                                bool z_only = false);
+                                bool z_only = false, int col0 = 0, int col1 = -1);
+bool fused_sweeps_supported(const sldg_ctx *c, bool z_first);  // launch_fused_sweeps would not return cudaErrorNotSupported
 cudaError_t launch_tiled_sweeps(sldg_ctx *c, const double *fin, double *fout, double tau_z, double tau_v, bool z_first);
 size_t field_workspace_bytes(const sldg_params *p);
 void field_carve(sldg_ctx *c, char *base);

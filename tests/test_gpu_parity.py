@@ -600,3 +600,36 @@ def test_timing_history_matches_last_timing(torch):
     assert np.allclose(np.array(got), np.array(want), rtol=0, atol=0)
     assert all(g[7] > 0 and abs(g[7] - (g[0] + g[1] + g[3] + g[4] + g[5])) < 0.05 for g in got)
     s.close()
+
+
+@pytest.mark.parametrize("no_fuse", [False, True])
+def test_strang_step_host_chunked_field_upload_is_bit_identical(torch, monkeypatch, no_fuse):
+    """sldg_strang_step_host uploads E_z in chunks of y rows under the fused z,v pair, which is then launched chunk by
+    chunk: same bits as the device-resident step with the fields set beforehand -- two steps with different fields, a
+    number of y rows that the chunks do not divide, and with the fused pairs switched off (one plain upload)."""
+    if no_fuse:
+        monkeypatch.setenv("SLDG_NO_FUSE", "1")
+    spec = inputs.itg_grid(6, 7, 5, 12, 2)
+    f = inputs.itg_initial_f(spec, eps=0.05)
+    dt = 2.0
+    fields = [inputs.itg_fields(spec, dt, 0.8)[:3], inputs.itg_fields(spec, dt, 0.5)[:3]]
+    fields[1] = tuple(np.ascontiguousarray(-x) for x in fields[1])
+    outs = []
+    for host in (False, True):
+        s = _sldg(spec)
+        s.import_state(_dev(torch, f))
+        rho = np.empty((spec.shape[0], spec.shape[2], spec.shape[3]))
+        mass = np.empty(1)
+        for a, b, Ez in fields:
+            if host:
+                s.strang_step_host(dt, Ez, a, b, 1, rho, mass)
+            else:
+                s.set_Ez(_dev(torch, Ez))
+                s.set_vxy(_dev(torch, a), _dev(torch, b), 1)
+                s.strang_step(dt)
+        s.check()
+        outs.append(s.export_state().cpu().numpy())
+        if host:
+            assert np.array_equal(rho, s.charge_density().cpu().numpy())
+        s.close()
+    assert np.array_equal(outs[0], outs[1])
