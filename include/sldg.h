@@ -120,7 +120,11 @@ int sldg_set_trace_order(sldg_ctx *ctx, int trace_order); /* used by sldg_strang
 /* The same step driven from HOST buffers (what a host-side field solver sees): copies Ez, a, b from
  * host to device, runs sldg_strang_step, then the charge density and the mass, copies rho and mass back
  * to the host, and synchronises the stream.  Pinned host buffers make the copies asynchronous.
- * Any of Ez_host / a_host+b_host / rho_host / mass_host may be NULL to skip that transfer. */
+ * Any of Ez_host / a_host+b_host / rho_host / mass_host may be NULL to skip that transfer.
+ * The transfers overlap the kernels where the data dependences allow: E_z goes up in chunks of y rows, each chunk's
+ * (z,v) planes swept as soon as it has arrived (when the z,v pair runs fused); a, b go up under the first sweeps; rho
+ * comes down in slabs of z under the reduction of the next slab.  The host buffers must stay valid until the call
+ * returns (it synchronises). */
 int sldg_strang_step_host(sldg_ctx *ctx, double dt, const double *Ez_host, const double *a_host,
                           const double *b_host, int periodic, double *rho_host, double *mass_host);
 

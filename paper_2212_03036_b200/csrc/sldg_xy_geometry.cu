@@ -31,6 +31,9 @@ using namespace sldg_geom;
 
 namespace {
 
+#ifndef SLDG_GEOM_WARPS
+#define SLDG_GEOM_WARPS 1  // 1: the warps of a block work independently (32 cells each); 0: block-wide phases
+#endif
 #ifndef SLDG_GEOM_MINB2
 #define SLDG_GEOM_MINB2 5  // resident blocks per SM the o = 2 kernel is compiled for (102 registers)
 #endif
@@ -44,11 +47,21 @@ __global__ void __launch_bounds__(GeomShared<O>::CELLS, (O == 2 ? SLDG_GEOM_MINB
 {
     constexpr int CELLS = GeomShared<O>::CELLS;
     extern __shared__ __align__(16) unsigned char geom_smem[];
-    GeomShared<O> &sh = *reinterpret_cast<GeomShared<O> *>(geom_smem);
     const int ncell = g.n[0] * g.n[1];
     const int t0 = blockIdx.x * CELLS, z = blockIdx.y;
+#if SLDG_GEOM_WARPS
+    // every warp does its own 32 cells -- set-up, enumeration of their pieces, the pieces -- on its own slice of shared
+    // memory and synchronises with __syncwarp only: no block-wide barrier (their stalls were 9 % of the kernel's samples;
+    // the warps of a block drift apart and hide each other's latencies)
+    GeomShared<O, 32> &sh = reinterpret_cast<GeomShared<O, 32> *>(geom_smem)[threadIdx.x >> 5];
+    const int w0 = t0 + (threadIdx.x & ~31);
+    geometry_block<O, 32, true>(sh, threadIdx.x & 31, 32, [&](int c) { return w0 + c < ncell ? w0 + c : -1; }, z, va, vb,
+                                hdr, W, err, g, bs, tau, order, periodic);
+#else
+    GeomShared<O> &sh = *reinterpret_cast<GeomShared<O> *>(geom_smem);
     geometry_block<O, CELLS>(sh, threadIdx.x, CELLS, [&](int c) { return t0 + c < ncell ? t0 + c : -1; }, z, va, vb,
                              hdr, W, err, g, bs, tau, order, periodic);
+#endif
 }
 
 // debug/test helper: expand the packed weight blocks of one z plane to the dense [cell][slot] form
@@ -94,8 +107,10 @@ cudaError_t launch_xy_geometry(sldg_ctx *c, double tau, int trace_order)
 #define LAUNCH_G(OO)                                                                                              \
     do {                                                                                                          \
         auto kern = xy_geometry_kernel<OO>;                                                                       \
-        cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)sizeof(GeomShared<OO>));     \
-        kern<<<grid, GeomShared<OO>::CELLS, sizeof(GeomShared<OO>), stream>>>(                                    \
+        const size_t smem = SLDG_GEOM_WARPS ? (GeomShared<OO>::CELLS / 32) * sizeof(GeomShared<OO, 32>)            \
+                                            : sizeof(GeomShared<OO>);                                             \
+        cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);                       \
+        kern<<<grid, GeomShared<OO>::CELLS, smem, stream>>>(                                                      \
             c->va, c->vb, c->hdr, c->W, c->err, g, c->basis, tau, trace_order, c->vel_periodic);        \
     } while (0)
     if (O == 1) LAUNCH_G(1); else if (O == 2) LAUNCH_G(2); else LAUNCH_G(3);

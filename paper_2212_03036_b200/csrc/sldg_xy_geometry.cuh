@@ -256,7 +256,7 @@ struct GeomShared {
     double Vi[NVI][CELLS];
     double xc[CELLS], yc[CELLS];           // centre of the node feet
     int r0[CELLS], s0[CELLS], nr[CELLS], ns[CELLS], mask[CELLS];
-    unsigned short item[CELLS * 11];       // work item -> cell | candidate index << 8, 0xffff = padding
+    unsigned short item[CELLS * 11];       // work item -> cell | candidate index << 7 | dr << 11 | ds << 13, 0xffff = padding
     int warp_tot[CELLS / 32];
 };
 
@@ -578,14 +578,24 @@ __device__ __forceinline__ void geometry_block(GeomShared<O, CELLS> &sh, int tid
     // (padded to the next multiple of 32 where they would straddle), each warp's list rounded up to 32.
     int first = 0, pos = 0;
     if (tid < CELLS) {
-#pragma unroll 1
-        for (int l = 0; l < 32; ++l) {
-            const int nl = __shfl_sync(0xffffffffu, n, l);
-            if ((pos & 31) + nl > 32) pos = (pos + 31) & ~31;
-            if (lane == l) first = pos;
-            pos += nl;
+        // exclusive prefix of the counts over the warp; then, boundary by boundary, the first cell whose items would
+        // straddle a multiple of 32 moves up to it, and every later cell with it (at most 9 boundaries; a loop over
+        // the 32 lanes in turn was 3 % of the kernel's instructions)
+        int S = n;
+#pragma unroll
+        for (int d = 1; d < 32; d <<= 1) {
+            const int u = __shfl_up_sync(0xffffffffu, S, d);
+            if (lane >= d) S += u;
         }
-        pos = (pos + 31) & ~31;
+        first = S - n;
+        for (;;) {
+            const unsigned strad = __ballot_sync(0xffffffffu, (first & 31) + n > 32);
+            if (!strad) break;
+            const int l0 = __ffs(strad) - 1;
+            const int s0 = __shfl_sync(0xffffffffu, first, l0);
+            if (lane >= l0) first += 32 - (s0 & 31);
+        }
+        pos = (__shfl_sync(0xffffffffu, first + n, 31) + 31) & ~31;
         if (lane == 0) sh.warp_tot[warp] = pos;
     }
     sync();
@@ -596,16 +606,26 @@ __device__ __forceinline__ void geometry_block(GeomShared<O, CELLS> &sh, int tid
     }
     for (int it = tid; it < total; it += nthreads) sh.item[it] = 0xffff;
     sync();
-    for (int k = 0; k < n; ++k) sh.item[base + first + k] = (unsigned short)(tid | (k << 8));
+    {
+        // item code: cell | candidate index k << 7 | dr << 11 | ds << 13 (k = dr + ds (nr + 1)): 15 bits, never 0xffff
+        const int w = n > 0 ? sh.nr[tid < CELLS ? tid : 0] + 1 : 1;
+        int dr = 0, ds = 0;
+        for (int k = 0; k < n; ++k) {
+            sh.item[base + first + k] = (unsigned short)(tid | (k << 7) | (dr << 11) | (ds << 13));
+            if (++dr == w) {
+                dr = 0;
+                ++ds;
+            }
+        }
+    }
     sync();
 
     // phase 2: one piece per thread and pass (whole warps: total is a multiple of 32)
     for (int it = tid; it < total; it += nthreads) {
         const int code = sh.item[it];
         const bool valid = code != 0xffff;
-        const int cc = valid ? (code & 0xff) : 0, k = valid ? (code >> 8) : 0;
-        const int w = sh.nr[cc] + 1;
-        const int ds = k / w, dr = k - ds * w;
+        const int cc = valid ? (code & 0x7f) : 0, k = valid ? ((code >> 7) & 15) : 0;
+        const int dr = valid ? ((code >> 11) & 3) : 0, ds = valid ? ((code >> 13) & 3) : 0;
         const long long cellid = (long long)z * ncell + cell_of(cc);
         geometry_piece<O>(sh, valid, cc, k, dr, ds, bs, W + (size_t)cellid * 9 * sldg_w_block_doubles(O), &sh.mask[cc]);
     }
