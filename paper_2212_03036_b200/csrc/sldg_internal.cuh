@@ -10,7 +10,9 @@
 #define SLDG_MAXO2 9
 #define SLDG_MAXQ 5       // quadrature points per edge for the Green's-theorem line integrals (2o-1)
 #define SLDG_HIST 64      // Strang steps whose per-kernel event times are kept (sldg_timing_history)
-#define SLDG_EZ_CHUNKS 4   // y chunks of the E_z upload of sldg_strang_step_host
+#ifndef SLDG_EZ_CHUNKS
+#define SLDG_EZ_CHUNKS 8   // y chunks of the E_z upload of sldg_strang_step_host
+#endif
 #define SLDG_PV_ALIGN 16  // internal v-line pitch is a multiple of 16 doubles (128 B)
 
 // Doubles between two weight blocks of the 2d geometry in memory: o^4, at o = 3 padded to an even number (bulk
