@@ -122,9 +122,13 @@ int sldg_set_trace_order(sldg_ctx *ctx, int trace_order); /* used by sldg_strang
  * to the host, and synchronises the stream.  Pinned host buffers make the copies asynchronous.
  * Any of Ez_host / a_host+b_host / rho_host / mass_host may be NULL to skip that transfer.
  * The transfers overlap the kernels where the data dependences allow: E_z goes up in chunks of y rows, each chunk's
- * (z,v) planes swept as soon as it has arrived (when the z,v pair runs fused); a, b go up under the first sweeps; rho
- * comes down in slabs of z under the reduction of the next slab.  The host buffers must stay valid until the call
- * returns (it synchronises). */
+ * (z,v) planes swept as soon as it has arrived (when the z,v pair runs fused); a, b go up under the first sweeps.  rho:
+ * where the v,z pair runs fused at o = 2 with unpadded v lines of whole warps (Nv a multiple of 32), that kernel forms the
+ * charge density from its own results -- no further pass over f -- and is launched in chunks of y rows, the rows of a
+ * chunk coming down under the next chunk; otherwise a reduction over f in slabs of z, each slab coming down under the
+ * reduction of the next.  The two sum over v in a different order: rho_host agrees with sldg_charge_density to
+ * round-off (1e-14 relative), not bit for bit; the state is the same bit for bit.  The host buffers must stay valid
+ * until the call returns (it synchronises). */
 int sldg_strang_step_host(sldg_ctx *ctx, double dt, const double *Ez_host, const double *a_host,
                           const double *b_host, int periodic, double *rho_host, double *mass_host);
 

@@ -310,7 +310,8 @@ int sldg_create(const sldg_params *p, double *f_a_dev, double *f_b_dev, void *wo
         return SLDG_ECUDA;
     }
     for (int k = 0; k < SLDG_EZ_CHUNKS; ++k)
-        if (cudaEventCreateWithFlags(&c->ezev[k], cudaEventDisableTiming) != cudaSuccess) {
+        if (cudaEventCreateWithFlags(&c->ezev[k], cudaEventDisableTiming) != cudaSuccess ||
+            cudaEventCreateWithFlags(&c->rhoev[k], cudaEventDisableTiming) != cudaSuccess) {
             sldg_destroy(c);
             return SLDG_ECUDA;
         }
@@ -338,8 +339,10 @@ int sldg_destroy(sldg_ctx *c)
     for (int k = 0; k < 2; ++k) {
         if (c->cev[k]) cudaEventDestroy(c->cev[k]);
     }
-    for (int k = 0; k < SLDG_EZ_CHUNKS; ++k)
+    for (int k = 0; k < SLDG_EZ_CHUNKS; ++k) {
         if (c->ezev[k]) cudaEventDestroy(c->ezev[k]);
+        if (c->rhoev[k]) cudaEventDestroy(c->rhoev[k]);
+    }
     delete c;
     return SLDG_OK;
 }
@@ -437,6 +440,25 @@ static cudaError_t launch_pair(sldg_ctx *c, double tau, bool z_first)
             const int y0 = (int)((long long)Ny * k / nch), y1 = (int)((long long)Ny * (k + 1) / nch);
             cudaStreamWaitEvent(c->stream, c->ezev[k], 0);
             e = launch_fused_sweeps(c, fin, fout, tau, tau, true, false, y0 * Nx, y1 * Nx);
+            if (e != cudaSuccess) return e;
+        }
+        return e;
+    }
+    if (c->rho_chunks > 0 && !z_first) {
+        // sldg_strang_step_host: the v,z pair in chunks of y rows; each launch also writes the charge density of its planes
+        // (the caller checked that the kernel takes this pair), whose rows go down to the host on the copy stream -- strided
+        // copies, rho is [Nz][Ny][Nx] -- under the next chunk's sweep
+        const int nch = c->rho_chunks, Ny = c->g.N[1], Nx = c->g.N[0];
+        const size_t pitch = (size_t)Ny * Nx * 8;
+        c->rho_chunks = 0;
+        for (int k = 0; k < nch; ++k) {
+            const long long y0 = (long long)Ny * k / nch, y1 = (long long)Ny * (k + 1) / nch;
+            e = launch_fused_sweeps(c, fin, fout, tau, tau, false, false, (int)(y0 * Nx), (int)(y1 * Nx), c->rho_ws);
+            if (e != cudaSuccess) return e;
+            cudaEventRecord(c->rhoev[k], c->stream);
+            cudaStreamWaitEvent(c->cstream, c->rhoev[k], 0);
+            e = cudaMemcpy2DAsync(c->rho_host + y0 * Nx, pitch, c->rho_ws + y0 * Nx, pitch, (size_t)(y1 - y0) * Nx * 8,
+                                  (size_t)c->g.N[2], cudaMemcpyDeviceToHost, c->cstream);
             if (e != cudaSuccess) return e;
         }
         return e;
@@ -597,9 +619,22 @@ int sldg_strang_step_host(sldg_ctx *c, double dt, const double *Ez_host, const d
         cudaEventRecord(c->cev[1], c->cstream);
         c->ab_pending = 1;
     }
+    // rho: where the v,z pair runs as the whole-plane kernel at o = 2, that kernel forms the charge density from its own
+    // results (no further pass over f) and is launched in chunks of y rows, the download of a chunk's rows under the next
+    // chunk (launch_pair); otherwise a reduction over f in slabs of z after the step, downloads under the next slab.  The
+    // two differ in the order of the v sum (last bits).
+    const bool rho_fused = rho_host && c->fuse && c->tile != 2 && g.N[1] >= SLDG_EZ_CHUNKS && fused_sweeps_supported(c, false, true);
+    if (rho_fused) {
+        c->rho_chunks = SLDG_EZ_CHUNKS;
+        c->rho_host = rho_host;
+    }
     int rc = sldg_strang_step(c, dt);
+    c->rho_chunks = 0;
     if (rc) return rc;
-    if (rho_host) {
+    if (rho_fused) {
+        cudaEventRecord(c->cev[0], c->cstream);
+        cudaStreamWaitEvent(c->stream, c->cev[0], 0);  // the caller's stream sees the downloads complete
+    } else if (rho_host) {
         // rho in slabs of z: the download of a slab (copy stream) runs under the reduction of the next one
         const int nslab = g.N[2] < 8 ? g.N[2] : 8;
         const long long per_z = (long long)g.N[1] * g.N[0];

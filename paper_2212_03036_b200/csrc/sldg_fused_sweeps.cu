@@ -33,23 +33,27 @@ constexpr int FUSED_MAXCPL = 4;  // v cells per lane in the line-wise phases (nv
 // dynamic shared memory: planes [2 NL + NH][Pv] doubles | per line: A, B of its v shift [Nz][2 O^2] doubles |
 // per column: A, B of its z shift [2 O^2][Pv] doubles | per line: s [Nz] ints | per column: rotation offset
 // [Pv] ints, z shift [Pv] ints | barriers | z,v pair: line order per plane parity [2][Nz] shorts, marks [2][Nz] bytes
-__host__ __device__ inline size_t fused_table_bytes(int Nz, int Pv, int O)
+__host__ __device__ inline size_t fused_table_bytes(int Nz, int Pv, int O, bool rho = false)
 {
     // o <= 2: A, B of the column's z shift stay in the registers of the column's threads (every KB of tables is a line
     // less fetched ahead: 0.02 ms per KB and z,v pair at 128 x 128)
     return (size_t)Nz * 2 * O * O * 8 + (O <= 2 ? 0 : (size_t)Pv * 2 * O * O * 8) + (size_t)Nz * 4 + (size_t)Pv * 8 + 64 +
-           (size_t)Nz * 6 + 16;  // + line order of the z,v pair's line-wise phase [2][Nz] shorts, marks [2][Nz] bytes
+           (size_t)Nz * 6 + 16 +  // + line order of the z,v pair's line-wise phase [2][Nz] shorts, marks [2][Nz] bytes
+           (rho ? (size_t)(Pv / 32) * Nz * 8 + 8 : 0);  // RHO: per warp of a z slice, the partial v sums of the plane's rows
 }
 
 // ZONLY (with ZFIRST = false): the z sweep alone through the same planes -- for Courant numbers so different from
 // one v node to the next that the column walk of advect_z_kernel reads a different z row in almost every lane.
-template <int O, int CPL, bool ZFIRST, bool ZONLY, bool FULLV>
+// RHO (v,z pair only; o <= 2, Pv a multiple of 32, Nv = Pv): the charge density of the NEW state, rho = h_v sum_v w f
+// (PAPER.md:57), is formed from the results of the z sweep as they leave for global memory -- sldg_strang_step_host then
+// needs no further pass over f.
+template <int O, int CPL, bool ZFIRST, bool ZONLY, bool FULLV, bool RHO = false>
 __global__ void __launch_bounds__(FUSED_BLOCK, 1) fused_sweep_kernel(const double *__restrict__ fin,
                                                                        double *__restrict__ fout,
                                                                        const double *__restrict__ Ez, GridDev g,
                                                                        ShiftPoly spz, ShiftPoly spv, Basis bs,
                                                                        double tau_z, double tau_v, int NL, int col0,
-                                                                       int col1)
+                                                                       int col1, double *__restrict__ rho)
 {
     extern __shared__ __align__(16) unsigned char fused_smem[];
     const int Nz = g.N[2], nz = g.n[2], Nv = g.N[3], nv = g.n[3], Pv = g.Pv;
@@ -119,6 +123,7 @@ __global__ void __launch_bounds__(FUSED_BLOCK, 1) fused_sweep_kernel(const doubl
     short *order = reinterpret_cast<short *>(bars + 6);
     unsigned char *mark = reinterpret_cast<unsigned char *>(order + 2 * Nz);
     int *n_early = reinterpret_cast<int *>(bars + 5);
+    double *rho_part = reinterpret_cast<double *>((reinterpret_cast<uintptr_t>(mark + 2 * Nz) + 7) & ~(uintptr_t)7);  // RHO: [Pv / 32][Nz]
     if (ZFIRST) {
         for (int i = tid; i < 2 * Nz; i += FUSED_BLOCK) mark[i] = 0;
         __syncthreads();
@@ -205,10 +210,21 @@ __global__ void __launch_bounds__(FUSED_BLOCK, 1) fused_sweep_kernel(const doubl
     int col = col0 + blockIdx.x, par = 0;
     uint32_t phL[2] = {0, 0}, phH = 0;
     if (!ZONLY && col < ncol && tid < Nz) ez_next = __ldg(Ez + tid * plane_nodes + col);
+    // RHO: the previous plane's partial sums (one per warp of a z slice, written in its z sweep) -> rho, in a fixed order
+    auto flush_rho = [&](int pcol) {
+        if (tid < Nz) {
+            double sum = 0.0;
+            for (int q = 0; q < Pv / 32; ++q) sum += rho_part[q * Nz + tid];
+            rho[tid * plane_nodes + pcol] = g.h[3] * sum;
+        }
+    };
+    int prev_col = -1;
     for (; col < ncol; col += gridDim.x, par ^= 1) {
         double *tile = buf + (par ? NL * Pv : 0);
         const int ncolx = col + (int)gridDim.x;
         const double ez_cur = ez_next;
+        if (RHO && prev_col >= 0) flush_rho(prev_col);
+        prev_col = col;
         if (!ZONLY && ncolx < ncol && tid < Nz) ez_next = __ldg(Ez + tid * plane_nodes + ncolx);
         // ---- per line the (s, A, B) of its v shift (under the copies) ------------------------------------------
         if (!ZONLY && tid < Nz) {
@@ -464,6 +480,56 @@ __global__ void __launch_bounds__(FUSED_BLOCK, 1) fused_sweep_kernel(const doubl
 #pragma unroll
                 for (int m = 0; m < O; ++m) up[m] = tile[off + m * Pv];
                 double *w = dst + v + (long long)(zi0 * O) * g.sZ;
+                if constexpr (RHO && O <= 2) {
+                    // the same sweep in batches of 8 rows (8 / O cells); the weighted results of a batch are summed over the
+                    // warp's 32 v nodes by a butterfly that halves the values a lane holds at every exchange (9 exchanges
+                    // per 8 rows), lane l < 8 ending with the sum of row l of the batch
+                    constexpr int U = 8 / O;
+                    const double wv = bs.w[O][v % O];
+                    double *part = rho_part + (v >> 5) * Nz;
+#pragma unroll 1
+                    for (int i = zi0; i < zi1; i += U) {
+                        double x[8];
+#pragma unroll
+                        for (int u = 0; u < U; ++u) {
+                            if (i + u < zi1) {
+                                off += cstep;
+                                if (off >= NzPv) off -= NzPv;
+                                double un[O];
+#pragma unroll
+                                for (int m = 0; m < O; ++m) un[m] = tile[off + m * Pv];
+#pragma unroll
+                                for (int j = 0; j < O; ++j) {
+                                    double acc = 0.0;
+#pragma unroll
+                                    for (int m = 0; m < O; ++m) acc = fma(Az[j][m], up[m], acc);
+#pragma unroll
+                                    for (int m = 0; m < O; ++m) acc = fma(Bz[j][m], un[m], acc);
+                                    __stcs(w, acc);
+                                    w += g.sZ;
+                                    x[u * O + j] = wv * acc;
+                                }
+#pragma unroll
+                                for (int m = 0; m < O; ++m) up[m] = un[m];
+                            } else {
+#pragma unroll
+                                for (int j = 0; j < O; ++j) x[u * O + j] = 0.0;
+                            }
+                        }
+#pragma unroll
+                        for (int d = 4; d >= 1; d >>= 1) {
+                            const bool hi = (lane & d) != 0;
+#pragma unroll
+                            for (int k = 0; k < d; ++k) {
+                                const double send = hi ? x[k] : x[k + d], keep = hi ? x[k + d] : x[k];
+                                x[k] = keep + __shfl_xor_sync(0xffffffffu, send, d);
+                            }
+                        }
+                        x[0] += __shfl_xor_sync(0xffffffffu, x[0], 8);
+                        x[0] += __shfl_xor_sync(0xffffffffu, x[0], 16);
+                        if (lane < 8 && i + lane / O < zi1) part[(i + lane / O) * O + lane % O] = x[0];
+                    }
+                } else {
 #pragma unroll 2
                 for (int i = zi0; i < zi1; ++i) {
                     off += cstep;
@@ -484,6 +550,7 @@ __global__ void __launch_bounds__(FUSED_BLOCK, 1) fused_sweep_kernel(const doubl
 #pragma unroll
                     for (int m = 0; m < O; ++m) up[m] = un[m];
                 }
+                }
             }
         }
         fence_proxy_async();  // generic writes before the next bulk copies
@@ -491,12 +558,13 @@ __global__ void __launch_bounds__(FUSED_BLOCK, 1) fused_sweep_kernel(const doubl
         if (lane == 0) mbar_arrive(&bars[3]);
         compute_sync();  // the per-line tables are free for the next plane
     }
+    if (RHO && prev_col >= 0) flush_rho(prev_col);
 }
 
 }  // namespace
 
 // Whether the pair can run in this kernel (see launch_fused_sweeps); *NL_out = lines fetched one plane ahead.
-static bool fused_pair_fits(const sldg_ctx *c, bool z_first, bool z_only, int *NL_out, size_t *smem_out)
+static bool fused_pair_fits(const sldg_ctx *c, bool z_first, bool z_only, int *NL_out, size_t *smem_out, bool rho = false)
 {
     if (z_only) z_first = false;
     const GridDev &g = c->g;
@@ -506,7 +574,9 @@ static bool fused_pair_fits(const sldg_ctx *c, bool z_first, bool z_only, int *N
     const int Nz = g.N[2];
     // the per-line tables of the v shift (vs, vAB, the E_z prefetch) are filled by thread <-> line
     if (!z_only && Nz > FUSED_THREADS) return false;
-    const size_t tables = fused_table_bytes(Nz, g.Pv, O), row = (size_t)g.Pv * 8;
+    // the charge density from the z sweep of the v,z pair (RHO): o = 2, whole warps of v nodes, no padding of the v lines
+    if (rho && (z_first || z_only || O != 2 || g.Pv % 32 != 0 || g.N[3] != g.Pv)) return false;
+    const size_t tables = fused_table_bytes(Nz, g.Pv, O, rho), row = (size_t)g.Pv * 8;
     static const int budget_kb = getenv("SLDG_FUSED_KB") ? atoi(getenv("SLDG_FUSED_KB")) : 227;  // KB of dynamic shared memory the kernel may take (sm_100: 227 per block)
     const size_t budget = (size_t)budget_kb * 1024;
     if (tables + row * Nz > budget) return false;
@@ -521,31 +591,40 @@ static bool fused_pair_fits(const sldg_ctx *c, bool z_first, bool z_only, int *N
     return true;
 }
 
-bool fused_sweeps_supported(const sldg_ctx *c, bool z_first)
+bool fused_sweeps_supported(const sldg_ctx *c, bool z_first, bool rho)
 {
     int NL;
     size_t smem;
-    return fused_pair_fits(c, z_first, false, &NL, &smem);
+    return fused_pair_fits(c, z_first, false, &NL, &smem, rho);
 }
 
 // The pair (z then v, or v then z) in one pass over the planes (Y,X) with index Y * Nx + X in [col0, col1) (col1 < 0:
 // all from col0 on); returns cudaErrorNotSupported when the (z,v) plane does not fit (the caller then runs the two
 // separate kernels).
+// rho != nullptr (v,z pair only): the kernel also writes the charge density of its planes, rho[Nz][Ny][Nx].
 cudaError_t launch_fused_sweeps(sldg_ctx *c, const double *fin, double *fout, double tau_z, double tau_v, bool z_first,
-                                bool z_only, int col0, int col1)
+                                bool z_only, int col0, int col1, double *rho)
 {
     if (z_only) z_first = false;
     const GridDev &g = c->g;
     const int O = g.o[2];
     int NL;
     size_t smem;
-    if (!fused_pair_fits(c, z_first, z_only, &NL, &smem)) return cudaErrorNotSupported;
+    if (!fused_pair_fits(c, z_first, z_only, &NL, &smem, rho != nullptr)) return cudaErrorNotSupported;
     const bool cpl2 = g.n[3] <= 64;
     const bool fullv = g.n[3] == (cpl2 ? 64 : 128);  // every lane of the line-wise phase has all its cells
     if (col1 < 0) col1 = g.N[0] * g.N[1];
     const int ncol = col1 - col0;
     if (ncol <= 0) return cudaSuccess;
     const int grid = ncol < c->sm_count ? ncol : c->sm_count;
+    if (rho) {
+        auto kern = cpl2 ? fused_sweep_kernel<2, 2, false, false, false, true> : fused_sweep_kernel<2, 4, false, false, false, true>;
+        cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
+        kern<<<grid, FUSED_BLOCK, smem, c->stream>>>(fin, fout, c->Ez, g, c->sp_z, c->sp_v, c->basis, tau_z, tau_v, NL, col0, col1,
+                                                       rho);
+        c->launches++;
+        return cudaGetLastError();
+    }
 #define LAUNCH_F(OO)                                                                                              \
     do {                                                                                                          \
         auto kern = z_only ? fused_sweep_kernel<OO, 2, false, true, false>                                        \
@@ -557,7 +636,7 @@ cudaError_t launch_fused_sweeps(sldg_ctx *c, const double *fin, double *fout, do
                                     : fused_sweep_kernel<OO, 4, false, false, false>);                            \
         cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);                       \
         kern<<<grid, FUSED_BLOCK, smem, c->stream>>>(fin, fout, c->Ez, g, c->sp_z, c->sp_v, c->basis, tau_z,    \
-                                                       tau_v, NL, col0, col1);                                    \
+                                                       tau_v, NL, col0, col1, nullptr);                           \
     } while (0)
     if (O == 1) LAUNCH_F(1); else if (O == 2) LAUNCH_F(2); else LAUNCH_F(3);
 #undef LAUNCH_F

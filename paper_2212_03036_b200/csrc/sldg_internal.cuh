@@ -91,6 +91,11 @@ struct sldg_ctx {
     // z,v pair that follows is launched per chunk behind its event (0: no such upload in flight)
     int ez_chunks;
     cudaEvent_t ezev[SLDG_EZ_CHUNKS];
+    // sldg_strang_step_host: the v,z pair launched in rho_chunks chunks of y rows, each writing the charge density of its
+    // planes (fused RHO kernel) and followed by the download of those rows to rho_host on cstream (0: off)
+    int rho_chunks;
+    double *rho_host;
+    cudaEvent_t rhoev[SLDG_EZ_CHUNKS];
     int tile;               // z-tiled pair kernel: 1 when the whole plane does not fit, 2 first (SLDG_FORCE_TILE), 0 never (SLDG_NO_TILE)
     int fuse, last_fused;   // fuse: sldg_strang_step runs each pair of adjacent sweeps in one pass
     size_t n_partials;
@@ -127,8 +132,9 @@ cudaError_t launch_xy_apply(sldg_ctx *c, const double *fin, double *fout);
 cudaError_t count_weight_blocks(sldg_ctx *c, long long *total_host);
 // planes (Y,X) with index Y * Nx + X in [col0, col1); col1 < 0: all from col0 on
 cudaError_t launch_fused_sweeps(sldg_ctx *c, const double *fin, double *fout, double tau_z, double tau_v, bool z_first,
-                                bool z_only = false, int col0 = 0, int col1 = -1);
-bool fused_sweeps_supported(const sldg_ctx *c, bool z_first);  // launch_fused_sweeps would not return cudaErrorNotSupported
+                                bool z_only = false, int col0 = 0, int col1 = -1, double *rho = nullptr);
+// launch_fused_sweeps would not return cudaErrorNotSupported (rho: with the charge density from the v,z pair)
+bool fused_sweeps_supported(const sldg_ctx *c, bool z_first, bool rho = false);
 cudaError_t launch_tiled_sweeps(sldg_ctx *c, const double *fin, double *fout, double tau_z, double tau_v, bool z_first);
 size_t field_workspace_bytes(const sldg_params *p);
 void field_carve(sldg_ctx *c, char *base);
