@@ -603,7 +603,7 @@ def test_timing_history_matches_last_timing(torch):
 
 
 @pytest.mark.parametrize("no_fuse", [False, True])
-@pytest.mark.parametrize("cells", [(6, 7, 5, 12), (6, 7, 5, 16), (5, 9, 7, 64)])
+@pytest.mark.parametrize("cells", [(6, 7, 5, 12), (6, 7, 5, 16), (5, 9, 7, 64), (4, 8, 3, 96)])
 def test_strang_step_host_overlapped_transfers(torch, monkeypatch, no_fuse, cells):
     """sldg_strang_step_host uploads E_z in chunks of y rows under the fused z,v pair, which is then launched chunk by
     chunk: same bits of the state as the device-resident step with the fields set beforehand -- two steps with different
