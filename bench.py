@@ -579,7 +579,8 @@ def measure_itg(workload, K, Wm, layout, world, rank, local, barrier, with_e2e, 
                       "h2d_bytes_per_step": int(Ez_h.numel() * 8 + a_h.numel() * 8 + b_h.numel() * 8),
                       "d2h_bytes_per_step": int(rho_h.numel() * 8 + 8),
                       "what": "sldg_strang_step_host: pinned Ez,a,b -> device, Strang step, rho and mass -> host; "
-                              "f stays resident"}
+                              "f stays resident; the copies run on a second stream under the kernels where the data "
+                              "dependences allow (Ez and rho in chunks of y rows, the sweep pairs launched per chunk)"}
         s.check()
         del Ez_h, a_h, b_h, rho_h
     s.close()

@@ -310,8 +310,12 @@ int sldg_create(const sldg_params *p, double *f_a_dev, double *f_b_dev, void *wo
         return SLDG_ECUDA;
     }
     for (int k = 0; k < SLDG_EZ_CHUNKS; ++k)
-        if (cudaEventCreateWithFlags(&c->ezev[k], cudaEventDisableTiming) != cudaSuccess ||
-            cudaEventCreateWithFlags(&c->rhoev[k], cudaEventDisableTiming) != cudaSuccess) {
+        if (cudaEventCreateWithFlags(&c->ezev[k], cudaEventDisableTiming) != cudaSuccess) {
+            sldg_destroy(c);
+            return SLDG_ECUDA;
+        }
+    for (int k = 0; k < SLDG_RHO_CHUNKS; ++k)
+        if (cudaEventCreateWithFlags(&c->rhoev[k], cudaEventDisableTiming) != cudaSuccess) {
             sldg_destroy(c);
             return SLDG_ECUDA;
         }
@@ -339,10 +343,10 @@ int sldg_destroy(sldg_ctx *c)
     for (int k = 0; k < 2; ++k) {
         if (c->cev[k]) cudaEventDestroy(c->cev[k]);
     }
-    for (int k = 0; k < SLDG_EZ_CHUNKS; ++k) {
+    for (int k = 0; k < SLDG_EZ_CHUNKS; ++k)
         if (c->ezev[k]) cudaEventDestroy(c->ezev[k]);
+    for (int k = 0; k < SLDG_RHO_CHUNKS; ++k)
         if (c->rhoev[k]) cudaEventDestroy(c->rhoev[k]);
-    }
     delete c;
     return SLDG_OK;
 }
@@ -623,9 +627,9 @@ int sldg_strang_step_host(sldg_ctx *c, double dt, const double *Ez_host, const d
     // results (no further pass over f) and is launched in chunks of y rows, the download of a chunk's rows under the next
     // chunk (launch_pair); otherwise a reduction over f in slabs of z after the step, downloads under the next slab.  The
     // two differ in the order of the v sum (last bits).
-    const bool rho_fused = rho_host && c->fuse && c->tile != 2 && g.N[1] >= SLDG_EZ_CHUNKS && fused_sweeps_supported(c, false, true);
+    const bool rho_fused = rho_host && c->fuse && c->tile != 2 && g.N[1] >= SLDG_RHO_CHUNKS && fused_sweeps_supported(c, false, true);
     if (rho_fused) {
-        c->rho_chunks = SLDG_EZ_CHUNKS;
+        c->rho_chunks = SLDG_RHO_CHUNKS;
         c->rho_host = rho_host;
     }
     int rc = sldg_strang_step(c, dt);

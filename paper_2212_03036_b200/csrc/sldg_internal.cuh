@@ -13,6 +13,9 @@
 #ifndef SLDG_EZ_CHUNKS
 #define SLDG_EZ_CHUNKS 8   // y chunks of the E_z upload of sldg_strang_step_host
 #endif
+#ifndef SLDG_RHO_CHUNKS
+#define SLDG_RHO_CHUNKS 8  // y chunks of its rho download (the v,z pair forming the charge density)
+#endif
 #define SLDG_PV_ALIGN 16  // internal v-line pitch is a multiple of 16 doubles (128 B)
 
 // Doubles between two weight blocks of the 2d geometry in memory: o^4, at o = 3 padded to an even number (bulk
@@ -95,7 +98,7 @@ struct sldg_ctx {
     // planes (fused RHO kernel) and followed by the download of those rows to rho_host on cstream (0: off)
     int rho_chunks;
     double *rho_host;
-    cudaEvent_t rhoev[SLDG_EZ_CHUNKS];
+    cudaEvent_t rhoev[SLDG_RHO_CHUNKS];
     int tile;               // z-tiled pair kernel: 1 when the whole plane does not fit, 2 first (SLDG_FORCE_TILE), 0 never (SLDG_NO_TILE)
     int fuse, last_fused;   // fuse: sldg_strang_step runs each pair of adjacent sweeps in one pass
     size_t n_partials;
