@@ -122,7 +122,8 @@ int sldg_set_trace_order(sldg_ctx *ctx, int trace_order); /* used by sldg_strang
  * to the host, and synchronises the stream.  Pinned host buffers make the copies asynchronous.
  * Any of Ez_host / a_host+b_host / rho_host / mass_host may be NULL to skip that transfer.
  * The transfers overlap the kernels where the data dependences allow: E_z goes up in chunks of y rows, each chunk's
- * (z,v) planes swept as soon as it has arrived (when the z,v pair runs fused); a, b go up under the first sweeps.  rho:
+ * (z,v) planes swept as soon as it has arrived (when the z,v pair runs fused), or in one piece under the z sweep, which
+ * does not read it (when the pair is certain to run as two kernels); a, b go up under the first sweeps.  rho:
  * where the v,z pair runs fused at o = 2 with unpadded v lines of whole warps (Nv a multiple of 32), that kernel forms the
  * charge density from its own results -- no further pass over f -- and is launched in chunks of y rows, the rows of a
  * chunk coming down under the next chunk; otherwise a reduction over f in slabs of z, each slab coming down under the

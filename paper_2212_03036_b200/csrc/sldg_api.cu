@@ -495,9 +495,17 @@ static int do_pair(sldg_ctx *c, double tau, bool z_first, cudaEvent_t mid, int *
         if (e != cudaErrorNotSupported) return SLDG_ECUDA;
         cudaGetLastError();
     }
+    if (c->ez_pending && !z_first) {  // (not reached: the upload is only deferred ahead of a z,v pair)
+        cudaStreamWaitEvent(c->stream, c->ezev[0], 0);
+        c->ez_pending = 0;
+    }
     int rc = z_first ? do_z(c, tau) : do_v(c, tau);
     if (rc) return rc;
     cudaEventRecord(mid, c->stream);
+    if (c->ez_pending) {  // sldg_strang_step_host: E_z went up on the copy stream under the z sweep, which does not read it
+        cudaStreamWaitEvent(c->stream, c->ezev[0], 0);
+        c->ez_pending = 0;
+    }
     return z_first ? do_v(c, tau) : do_z(c, tau);
 }
 
@@ -596,12 +604,23 @@ int sldg_strang_step_host(sldg_ctx *c, double dt, const double *Ez_host, const d
     // [Nz][Ny][Nx] -- and the planes of a chunk are swept as soon as its rows have arrived (launch_pair): only the first
     // chunk's upload is exposed.  Otherwise one copy on the caller's stream ahead of the step.
     const bool ez_chunked = Ez_host && c->fuse && c->tile != 2 && g.N[1] >= SLDG_EZ_CHUNKS && fused_sweeps_supported(c, true);
-    if (Ez_host && !ez_chunked &&
+    // Where the z,v pair is certain to run as two kernels (no fused pairs, or the plane does not fit and the z-tiled kernel
+    // does not take this order), the z sweep does not read E_z: one copy on the copy stream under it, the v sweep waits.
+    static const bool force_tile = getenv("SLDG_FORCE_TILE") != nullptr;
+    const bool ez_deferred = Ez_host && !ez_chunked &&
+                             (!c->fuse || (!fused_sweeps_supported(c, true) && (c->tile == 0 || (g.o[2] == 3 && !force_tile))));
+    if (Ez_host && !ez_chunked && !ez_deferred &&
         cudaMemcpyAsync(c->Ez, Ez_host, (size_t)g.lines * 8, cudaMemcpyHostToDevice, c->stream) != cudaSuccess)
         return SLDG_ECUDA;
-    if (ez_chunked || a_host) {
+    if (ez_chunked || ez_deferred || a_host) {
         cudaEventRecord(c->cev[0], c->stream);
         cudaStreamWaitEvent(c->cstream, c->cev[0], 0);
+    }
+    if (ez_deferred) {
+        if (cudaMemcpyAsync(c->Ez, Ez_host, (size_t)g.lines * 8, cudaMemcpyHostToDevice, c->cstream) != cudaSuccess)
+            return SLDG_ECUDA;
+        cudaEventRecord(c->ezev[0], c->cstream);
+        c->ez_pending = 1;
     }
     if (ez_chunked) {
         const size_t pitch = (size_t)g.N[1] * g.N[0] * 8;
@@ -634,6 +653,7 @@ int sldg_strang_step_host(sldg_ctx *c, double dt, const double *Ez_host, const d
     }
     int rc = sldg_strang_step(c, dt);
     c->rho_chunks = 0;
+    c->ez_pending = 0;
     if (rc) return rc;
     if (rho_fused) {
         cudaEventRecord(c->cev[0], c->cstream);

@@ -93,6 +93,7 @@ struct sldg_ctx {
     // sldg_strang_step_host: E_z uploaded on cstream in ez_chunks chunks of y rows, chunk k complete at ezev[k]; the fused
     // z,v pair that follows is launched per chunk behind its event (0: no such upload in flight)
     int ez_chunks;
+    int ez_pending;         // ... or in one piece, complete at ezev[0]: the v sweep of an unfused z,v pair waits for it
     cudaEvent_t ezev[SLDG_EZ_CHUNKS];
     // sldg_strang_step_host: the v,z pair launched in rho_chunks chunks of y rows, each writing the charge density of its
     // planes (fused RHO kernel) and followed by the download of those rows to rho_host on cstream (0: off)
